@@ -1,0 +1,146 @@
+/* subcycle.h — C ABI of libsubcycle: one Berger–Oliger subcycled RK4 step over a nested-box AMR
+ * hierarchy with dense-output ghost fill, hand-written fp64 CUDA for sm_100a (B200).
+ *
+ * What the calls compute is fixed by the paper (arXiv 2503.09629, "PAPER.md"):
+ *   - RK4 stages and update ............................ PAPER.md:54-75   (Sec. II, eqs 1-9)
+ *   - dense output b_i(theta) and its derivatives ...... PAPER.md:79-96   (eqs 10-14)
+ *   - stage reconstruction at refinement ghosts ........ PAPER.md:98-109  (eqs 15-18)
+ *   - the subcycling recursion, steps 1-7 .............. PAPER.md:111-119
+ *   - the evolved system  d_t u = rho, d_t rho = Lap u . PAPER.md:222-226 (Sec. IV.A, eqs 39-40)
+ * and, where the paper is silent, by the readings S1..S24 listed in DESIGN.md.
+ *
+ * Conventions (all calls):
+ *   - return 0 (SC_OK) on success, a negative SC_ERR_* otherwise; nothing aborts or throws across the
+ *     ABI; sc_last_error() returns a thread-local message for the last failing call.
+ *   - every pointer says whether it is a HOST or a DEVICE pointer; the library never frees caller memory.
+ *   - all index quantities are int32; all field data are IEEE fp64.
+ */
+#ifndef SUBCYCLE_H_
+#define SUBCYCLE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  SC_OK = 0,
+  SC_ERR_INVALID_ARG = -1, /* null pointer, index out of range, non-finite dt, capacity too small */
+  SC_ERR_NESTING = -2,     /* box list violates the nesting rules below                           */
+  SC_ERR_UNSUPPORTED = -3, /* ref_ratio != 2, ghost < 3 or > 4, nlevels > SC_MAX_LEVELS ...         */
+  SC_ERR_OOM = -4,         /* arena too small / device allocation failed                          */
+  SC_ERR_CUDA = -5         /* a CUDA runtime/driver call failed (message has the CUDA error string) */
+};
+
+#define SC_MAX_LEVELS 16
+
+/* One box of one refinement level (nested levels, h^(l)/h^(l+1) = 2).
+ * lo[] is the index of the box's first interior cell in that level's GLOBAL cell index space
+ * [0, domain_cells[a]*2^level) per axis a = (x,y,z); n[] is the number of interior cells.
+ * Grids are cell-centred (reading S1): cell i of level l has centre xlo + (i+1/2)*dx_l. */
+typedef struct {
+  int32_t level;
+  int32_t lo[3];
+  int32_t n[3];
+} sc_box;
+
+/* Hierarchy description (HOST memory, read only during the call).
+ * Rules checked by sc_create_hierarchy (violations -> SC_ERR_NESTING unless noted):
+ *   - boxes sorted by level; level 0 is exactly one box with lo = 0 and n = domain_cells
+ *     (the periodic domain, reading S9); every level 0..nlevels-1 has at least one box;
+ *   - every level >= 1 box: lo and n even on every axis (it covers whole parent cells), n >= 8;
+ *     it lies inside ONE box of level-1 with at least 4 parent cells of margin to that box's
+ *     interior edge (reading S13: the 5-point prolongation footprint never touches parent ghosts);
+ *   - boxes of one level are disjoint and at least 4 parent cells (8 own cells) apart.
+ * The state has nfields second-order fields u_f with first-order partners rho_f = d_t u_f:
+ *   component index comp = f        -> u_f
+ *                   comp = nfields+f -> rho_f            (V = 2*nfields arrays per box)
+ * coupling: HOST pointer to nfields*nfields doubles, row-major A[f][j], or NULL for A = 0:
+ *   d_t u_f = rho_f,   d_t rho_f = Lap_h u_f + sum_j A[f][j] u_j       (BASELINE cfg 4)
+ * arena: optional DEVICE memory of at least sc_arena_bytes() bytes, 256-byte aligned, owned by the
+ *   caller, who keeps it alive and does not touch it until sc_destroy; NULL -> the library allocates.
+ * cuda_stream: a cudaStream_t (as void*) on which all work of this hierarchy is enqueued; NULL = the
+ *   legacy default stream. */
+typedef struct {
+  int32_t nlevels;
+  int32_t nboxes;
+  const sc_box* boxes;
+  int32_t ref_ratio;       /* must be 2                                      */
+  int32_t ghost;           /* ghost width g; 3 in all configurations (stencil radius is 2)  */
+  int32_t nfields;         /* F >= 1                                                        */
+  int32_t domain_cells[3]; /* level-0 cells per axis                                        */
+  double xlo[3], xhi[3];   /* physical extent of the level-0 domain                         */
+  const double* coupling;  /* HOST, F*F, or NULL                                            */
+  void* arena;             /* DEVICE or NULL                                                */
+  uint64_t arena_bytes;
+  void* cuda_stream;
+} sc_hierarchy_desc;
+
+typedef struct sc_hierarchy sc_hierarchy; /* opaque; created by sc_create_hierarchy, freed by sc_destroy */
+
+/* Bytes of device memory a hierarchy with this description needs (0 on an invalid description;
+ * sc_last_error says why). Host-only computation: works without a GPU. */
+uint64_t sc_arena_bytes(const sc_hierarchy_desc* desc);
+
+/* Validate the description, lay the boxes out in device memory, zero all
+ * state, build the TMA tensor maps. The time is set to 0. On failure *out is NULL.
+ * Fails with SC_ERR_CUDA when no CUDA device is usable: there is no CPU fallback. */
+int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out);
+
+/* Copy one component of one box into the current state y of that box.
+ * src: dense INTERIOR-ONLY array [k][j][i], i (x) fastest, n[0]*n[1]*n[2] doubles; HOST if
+ * src_on_device == 0, DEVICE otherwise. box is the box's index within its level (0-based, in the
+ * order given at creation). Ghost cells are never supplied: the first stage of every level-step
+ * refills them (reading S8). Enqueued on the hierarchy's stream; a host source is consumed before the
+ * call returns. */
+int32_t sc_set_state(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, const double* src,
+                     int32_t src_on_device);
+
+/* Advance the whole hierarchy by dt_coarse (steps 1-7).
+ * subcycling = 1: level l takes 2^l steps of dt_coarse/2^l; refinement-boundary ghosts of Y_1..Y_4 and
+ *   of y_{n+1} come from the parent's dense output (eqs 10-18) prolonged in space (reading S3);
+ *   fine-to-coarse restriction (reading S4) after each pair of child steps.
+ * subcycling = 0: 2^(nlevels-1) uniform steps of dt_coarse/2^(nlevels-1) on all levels, same-time
+ *   spatial prolongation after every stage, restriction once per uniform step (reading S11).
+ * Asynchronous: returns once the work is enqueued on the stream. */
+int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling);
+
+/* Copy one component of one box's current state y (interior only, same layout as sc_set_state) to dst
+ * (HOST if dst_on_device == 0, else DEVICE). Synchronises the hierarchy's stream before returning. */
+int32_t sc_read_level(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, double* dst,
+                      int32_t dst_on_device);
+
+/* Simulation time: the sum of dt_coarse over all sc_step calls. */
+double sc_time(const sc_hierarchy* h);
+
+/* Number of kernels the library has launched (or replayed inside CUDA graphs) for this hierarchy. */
+uint64_t sc_launch_count(const sc_hierarchy* h);
+
+/* Debug: the refinement-boundary ghost index map of a level >= 1 box, computed by the same device code
+ * the ghost kernel uses. For every ghost cell of the padded box, in canonical order (k, then j, then
+ * i over [-g, n+g), skipping the interior), 7 int32: (i, j, k) box-local fine index, (pi, pj, pk)
+ * parent-box-local index of the containing parent cell, and parity bits (px | py<<1 | pz<<2) where
+ * p = 1 means the fine centre sits at +dx_parent/4 from the parent centre. out: HOST, cap = capacity in
+ * int32. Returns the number of ghost cells (>= 0) or an error. */
+int64_t sc_debug_ghost_map(sc_hierarchy* h, int32_t level, int32_t box, int32_t* out, uint64_t cap);
+
+/* Debug: copy one component of the current state INCLUDING ghosts, dense [n2+2g][n1+2g][n0+2g], to HOST
+ * memory. Synchronises the stream. Ghost values are those of the last stage-5 fill. */
+int32_t sc_debug_read_padded(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, double* dst);
+
+/* Debug: which of the stored RK slopes / old state to read: slot 0 = y_old, 1..4 = k_1..k_4 of the last
+ * level-step of that box (interior only, HOST dst). */
+int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t slot, int32_t comp,
+                           double* dst);
+
+/* Free everything the library owns (never the caller's arena). Synchronises the stream. */
+int32_t sc_destroy(sc_hierarchy* h);
+
+/* Message of the last failing call on this thread; valid until the next sc_ call on this thread. */
+const char* sc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SUBCYCLE_H_ */

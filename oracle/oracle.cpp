@@ -1,0 +1,605 @@
+// oracle.cpp — TEST INFRASTRUCTURE, not product code.
+//
+// A plain, slow, obviously-correct CPU implementation (fp64, C++17, optional OpenMP over k-planes) of
+// what libsubcycle's hot path computes: one Berger–Oliger subcycled RK4 step over a nested-box AMR
+// hierarchy with dense-output ghost fill (arXiv 2503.09629; citations are PAPER.md line numbers).
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load
+// it. It shares no code, header, table or constant with the CUDA path (it does not include
+// include/subcycle.h) and follows the paper's equations in the paper's order and notation:
+//
+//   RK4, eqs (1)-(9) ....................... PAPER.md:54-75     -> rk4_level_step()
+//   dense output b_i(theta), eqs (10)-(13) . PAPER.md:79-91     -> b_coeff()
+//   time derivatives, eq (14) .............. PAPER.md:93-96     -> dense_stage()
+//   ghost stage vectors, eqs (15)-(18) ..... PAPER.md:98-109    -> dense_stage()
+//   recursion, steps 1-7 ................... PAPER.md:111-119   -> advance()
+//   wave system, eqs (39)-(40) ............. PAPER.md:222-226   -> rhs()
+//
+// Where the paper is silent the readings S1..S24 of DESIGN.md apply (cell-centred grids S1, 4th-order
+// centred Laplacian S2, quartic Lagrange prolongation S3, quintic Lagrange restriction S4, parent-step
+// h in f_y y'' S5, periodic level 0 S9, non-subcycled mode S11/S15). Interpolation weights are computed
+// here from the Lagrange formula, not tabulated; tests pin them to the rational values.
+//
+// Pins (tests/test_oracle_*.py, run with -m "not gpu"): dense-output invariants and the rational
+// coefficient table; scalar-ODE stage-order test; closed-form single-level amplification matrix;
+// polynomial exactness of prolongation / restriction / Laplacian; brute-force ghost index map;
+// plane-wave convergence ladder (order ~4); subcycled-vs-uniform agreement; linearity.
+// PARITY UNPINNED: bit-level values of the composite multi-level scheme have no closed form — the
+// oracle is the definition there ("Oracle pins").
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr int kStencilRadius = 2;
+
+// ---------------------------------------------------------------------------------------------
+// dense output, eqs (10)-(18)
+// ---------------------------------------------------------------------------------------------
+
+// m-th theta-derivative (m = 0..3) of b_i(theta), i = 1..4; eqs (11)-(13).
+double b_coeff(int i, int m, double th) {
+  switch (i) {
+    case 1:  // b1 = th - 3/2 th^2 + 2/3 th^3
+      if (m == 0) return th - 1.5 * th * th + (2.0 / 3.0) * th * th * th;
+      if (m == 1) return 1.0 - 3.0 * th + 2.0 * th * th;
+      if (m == 2) return -3.0 + 4.0 * th;
+      return 4.0;
+    case 2:
+    case 3:  // b2 = b3 = th^2 - 2/3 th^3
+      if (m == 0) return th * th - (2.0 / 3.0) * th * th * th;
+      if (m == 1) return 2.0 * th - 2.0 * th * th;
+      if (m == 2) return 2.0 - 4.0 * th;
+      return -4.0;
+    default:  // b4 = -1/2 th^2 + 2/3 th^3
+      if (m == 0) return -0.5 * th * th + (2.0 / 3.0) * th * th * th;
+      if (m == 1) return -th + 2.0 * th * th;
+      if (m == 2) return -1.0 + 4.0 * th;
+      return 4.0;
+  }
+}
+
+// Value that a refinement-boundary ghost cell of the child takes for RK "stage" of a child step that
+// starts at parent progress theta, evaluated at ONE parent cell from the parent's y_n (= y_old) and
+// k_1..k_4, which were computed with the parent's step hp. The child's step is h = hp/2 (S10).
+//   stage 1..4: Y_1..Y_4 by eqs (15)-(18) with y, y', y'', y''' from eqs (10),(14) at theta, and
+//               f_y y'' = 4 (k3 - k2) / hp^2 (reading S5: the parent's step);
+//   stage 5:    y at "theta" by eq (10) alone (the caller passes theta + 1/2).
+double dense_stage(int stage, double theta, double hp, double y_old, const double k[4]) {
+  double y = y_old, d1 = 0.0, d2 = 0.0, d3 = 0.0;
+  double s0 = 0.0;
+  for (int i = 1; i <= 4; ++i) {
+    s0 += b_coeff(i, 0, theta) * k[i - 1];
+    d1 += b_coeff(i, 1, theta) * k[i - 1];
+    d2 += b_coeff(i, 2, theta) * k[i - 1];
+    d3 += b_coeff(i, 3, theta) * k[i - 1];
+  }
+  y = y_old + hp * s0;  // eq (10)
+  d2 = d2 / hp;         // eq (14), m = 2
+  d3 = d3 / (hp * hp);  // eq (14), m = 3
+  if (stage == 1 || stage == 5) return y;  // eq (15) / eq (10)
+  const double h = 0.5 * hp;               // child step
+  const double fyy = 4.0 * (k[2] - k[1]) / (hp * hp);
+  if (stage == 2) return y + 0.5 * h * d1;                                      // eq (16)
+  if (stage == 3) return y + 0.5 * h * d1 + 0.25 * h * h * d2 + (h * h * h / 16.0) * (d3 - fyy);  // (17)
+  return y + h * d1 + 0.5 * h * h * d2 + (h * h * h / 8.0) * (d3 + fyy);        // eq (18)
+}
+
+// ---------------------------------------------------------------------------------------------
+// spatial operators
+// ---------------------------------------------------------------------------------------------
+
+// Lagrange basis weights: value at x of the polynomial through (nodes[m], f_m) = sum_m w[m] f_m.
+void lagrange_weights(const double* nodes, int n, double x, double* w) {
+  for (int m = 0; m < n; ++m) {
+    double v = 1.0;
+    for (int q = 0; q < n; ++q)
+      if (q != m) v *= (x - nodes[q]) / (nodes[m] - nodes[q]);
+    w[m] = v;
+  }
+}
+
+// Prolongation (S3): quartic through the 5 parent cells J-2..J+2 (centres at offsets -2..2 in units of
+// the parent spacing) evaluated at the fine centre: -1/4 (parity 0) or +1/4 (parity 1).
+void prolong_weights(int parity, double w[5]) {
+  const double nodes[5] = {-2.0, -1.0, 0.0, 1.0, 2.0};
+  lagrange_weights(nodes, 5, parity ? 0.25 : -0.25, w);
+}
+
+// Restriction (S4): quintic through the 6 fine cells 2J-2..2J+3, whose centres sit at -2.5..+2.5 fine
+// spacings from the parent centre, evaluated at the parent centre.
+void restrict_weights(double r[6]) {
+  const double nodes[6] = {-2.5, -1.5, -0.5, 0.5, 1.5, 2.5};
+  lagrange_weights(nodes, 6, 0.0, r);
+}
+
+inline int floor_div2(int a) { return (a >= 0) ? a / 2 : -((-a + 1) / 2); }
+inline int pos_mod(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
+
+// ---------------------------------------------------------------------------------------------
+// hierarchy
+// ---------------------------------------------------------------------------------------------
+struct Field {  // one padded array of one box: index (i,j,k) in [-g, n+g)
+  int n[3] = {0, 0, 0}, g = 0;
+  std::vector<double> v;
+  void init(const int nn[3], int gg) {
+    for (int a = 0; a < 3; ++a) n[a] = nn[a];
+    g = gg;
+    v.assign(size_t(n[0] + 2 * g) * (n[1] + 2 * g) * (n[2] + 2 * g), 0.0);
+  }
+  inline size_t idx(int i, int j, int k) const {
+    return size_t(i + g) + size_t(n[0] + 2 * g) * (size_t(j + g) + size_t(n[1] + 2 * g) * size_t(k + g));
+  }
+  inline double& at(int i, int j, int k) { return v[idx(i, j, k)]; }
+  inline double at(int i, int j, int k) const { return v[idx(i, j, k)]; }
+};
+
+struct BoxData {
+  int level = 0, lo[3] = {0, 0, 0}, n[3] = {0, 0, 0};
+  int parent = -1;  // index into Hier::boxes of the containing box on level-1
+  // per component c in [0, 2F): current state y, stage vector Y, start-of-step state y_old, slopes k1..k4
+  std::vector<Field> y, Y, y_old, k[4];
+};
+
+struct Hier {
+  int nlevels = 0, g = 3, F = 1;
+  int domain[3] = {0, 0, 0};
+  double xlo[3], xhi[3];
+  std::vector<double> A;  // F*F coupling or empty
+  std::vector<BoxData> boxes;
+  std::vector<std::vector<int>> level_boxes;
+  double time = 0.0;
+  double dx(int level, int a) const { return (xhi[a] - xlo[a]) / (double(domain[a]) * double(1 << level)); }
+};
+
+inline bool is_interior(const BoxData& b, int i, int j, int k) {
+  return i >= 0 && i < b.n[0] && j >= 0 && j < b.n[1] && k >= 0 && k < b.n[2];
+}
+
+// ---------------------------------------------------------------------------------------------
+// right-hand side f(Y): k_u = rho ; k_rho = Lap_h u + A u   (eqs 39-40 + BASELINE cfg 4; S2)
+// 4th-order centred second derivative (-1, 16, -30, 16, -1)/(12 dx^2) per axis.
+// ---------------------------------------------------------------------------------------------
+void rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vector<Field>& kout) {
+  const int F = H.F;
+  double inv12dx2[3];
+  for (int a = 0; a < 3; ++a) {
+    const double d = H.dx(b.level, a);
+    inv12dx2[a] = 1.0 / (12.0 * d * d);
+  }
+  for (int f = 0; f < F; ++f) {
+    const Field& u = Y[f];
+    const Field& rho = Y[F + f];
+    Field& ku = kout[f];
+    Field& kr = kout[F + f];
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < b.n[2]; ++k)
+      for (int j = 0; j < b.n[1]; ++j)
+        for (int i = 0; i < b.n[0]; ++i) {
+          const double dxx = (-u.at(i - 2, j, k) + 16.0 * u.at(i - 1, j, k) - 30.0 * u.at(i, j, k) +
+                              16.0 * u.at(i + 1, j, k) - u.at(i + 2, j, k)) * inv12dx2[0];
+          const double dyy = (-u.at(i, j - 2, k) + 16.0 * u.at(i, j - 1, k) - 30.0 * u.at(i, j, k) +
+                              16.0 * u.at(i, j + 1, k) - u.at(i, j + 2, k)) * inv12dx2[1];
+          const double dzz = (-u.at(i, j, k - 2) + 16.0 * u.at(i, j, k - 1) - 30.0 * u.at(i, j, k) +
+                              16.0 * u.at(i, j, k + 1) - u.at(i, j, k + 2)) * inv12dx2[2];
+          double src = 0.0;
+          if (!H.A.empty())
+            for (int q = 0; q < F; ++q) src += H.A[size_t(f) * F + q] * Y[q].at(i, j, k);
+          ku.at(i, j, k) = rho.at(i, j, k);
+          kr.at(i, j, k) = dxx + dyy + dzz + src;
+        }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// ghost fills
+// ---------------------------------------------------------------------------------------------
+
+// Level 0 (S9): every ghost cell takes the value of the interior cell at the periodically wrapped index.
+void periodic_fill(const BoxData& b, std::vector<Field>& Y) {
+  for (Field& f : Y) {
+    const int g = f.g;
+#pragma omp parallel for schedule(static)
+    for (int k = -g; k < b.n[2] + g; ++k)
+      for (int j = -g; j < b.n[1] + g; ++j)
+        for (int i = -g; i < b.n[0] + g; ++i) {
+          if (is_interior(b, i, j, k)) continue;
+          f.at(i, j, k) = f.at(pos_mod(i, b.n[0]), pos_mod(j, b.n[1]), pos_mod(k, b.n[2]));
+        }
+  }
+}
+
+// Spatial prolongation of a parent-cell field C (stored over the parent box, interior valid) into the
+// ghost cells of the child array `dst` (S3). Direct triple sum, x innermost then y then z.
+void prolong_into_ghosts(const BoxData& child, const BoxData& par, const Field& C, Field& dst) {
+  double w[2][5];
+  prolong_weights(0, w[0]);
+  prolong_weights(1, w[1]);
+  const int g = dst.g;
+#pragma omp parallel for schedule(static)
+  for (int k = -g; k < child.n[2] + g; ++k)
+    for (int j = -g; j < child.n[1] + g; ++j)
+      for (int i = -g; i < child.n[0] + g; ++i) {
+        if (is_interior(child, i, j, k)) continue;
+        const int I[3] = {child.lo[0] + i, child.lo[1] + j, child.lo[2] + k};  // level-global fine index
+        int J[3], p[3];
+        for (int a = 0; a < 3; ++a) {
+          const int Jg = floor_div2(I[a]);  // containing parent cell (global)
+          p[a] = I[a] - 2 * Jg;             // 0: fine centre at -dx_p/4, 1: at +dx_p/4
+          J[a] = Jg - par.lo[a];            // parent-box-local
+        }
+        double sz = 0.0;
+        for (int c = -2; c <= 2; ++c) {
+          double sy = 0.0;
+          for (int bb = -2; bb <= 2; ++bb) {
+            double sx = 0.0;
+            for (int a = -2; a <= 2; ++a) sx += w[p[0]][a + 2] * C.at(J[0] + a, J[1] + bb, J[2] + c);
+            sy += w[p[1]][bb + 2] * sx;
+          }
+          sz += w[p[2]][c + 2] * sy;
+        }
+        dst.at(i, j, k) = sz;
+      }
+}
+
+// fill(l, stage, theta) for a level >= 1 box in SUBCYCLED mode: evaluate the
+// parent's dense output at every parent cell (combine), then prolong once into the child's ghosts.
+void dense_ghost_fill(const Hier& H, const BoxData& child, const BoxData& par, std::vector<Field>& dst,
+                      int stage, double theta, double hp) {
+  Field C;
+  C.init(par.n, H.g);
+  // parent cells any ghost cell of the child can reach: ceil(g/2) cells beyond the child's coverage
+  // plus the 2-cell interpolation radius (all inside the parent's interior by the nesting rule S13)
+  const int reach = (H.g + 1) / 2 + 2;
+  int lo[3], hi[3];
+  for (int a = 0; a < 3; ++a) {
+    lo[a] = child.lo[a] / 2 - par.lo[a] - reach;
+    hi[a] = (child.lo[a] + child.n[a]) / 2 - par.lo[a] + reach;
+  }
+  for (int c = 0; c < 2 * H.F; ++c) {
+#pragma omp parallel for schedule(static)
+    for (int k = lo[2]; k < hi[2]; ++k)
+      for (int j = lo[1]; j < hi[1]; ++j)
+        for (int i = lo[0]; i < hi[0]; ++i) {
+          const double kk[4] = {par.k[0][c].at(i, j, k), par.k[1][c].at(i, j, k), par.k[2][c].at(i, j, k),
+                                par.k[3][c].at(i, j, k)};
+          C.at(i, j, k) = dense_stage(stage, theta, hp, par.y_old[c].at(i, j, k), kk);
+        }
+    prolong_into_ghosts(child, par, C, dst[c]);
+  }
+}
+
+// Restriction (PAPER.md:119 step 7, S4): every parent cell whose children lie in the child's interior
+// takes the quintic interpolant of the child's y (reads up to 2 child ghost layers).
+void restrict_to_parent(const Hier& H, const BoxData& child, BoxData& par) {
+  double r[6];
+  restrict_weights(r);
+  const int J0[3] = {child.lo[0] / 2 - par.lo[0], child.lo[1] / 2 - par.lo[1], child.lo[2] / 2 - par.lo[2]};
+  const int nc[3] = {child.n[0] / 2, child.n[1] / 2, child.n[2] / 2};
+  for (int c = 0; c < 2 * H.F; ++c) {
+    const Field& yc = child.y[c];
+    Field& yp = par.y[c];
+#pragma omp parallel for schedule(static)
+    for (int K = 0; K < nc[2]; ++K)
+      for (int J = 0; J < nc[1]; ++J)
+        for (int I = 0; I < nc[0]; ++I) {
+          double sz = 0.0;
+          for (int cc = 0; cc < 6; ++cc) {
+            double sy = 0.0;
+            for (int bb = 0; bb < 6; ++bb) {
+              double sx = 0.0;
+              for (int a = 0; a < 6; ++a) sx += r[a] * yc.at(2 * I - 2 + a, 2 * J - 2 + bb, 2 * K - 2 + cc);
+              sy += r[bb] * sx;
+            }
+            sz += r[cc] * sy;
+          }
+          yp.at(J0[0] + I, J0[1] + J, J0[2] + K) = sz;
+        }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// time stepping
+// ---------------------------------------------------------------------------------------------
+void axpy_interior(const BoxData& b, std::vector<Field>& out, const std::vector<Field>& y0, double a,
+                   const std::vector<Field>& kk) {
+  for (size_t c = 0; c < out.size(); ++c) {
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < b.n[2]; ++k)
+      for (int j = 0; j < b.n[1]; ++j)
+        for (int i = 0; i < b.n[0]; ++i) out[c].at(i, j, k) = y0[c].at(i, j, k) + a * kk[c].at(i, j, k);
+  }
+}
+
+void fill(Hier& H, int level, std::vector<Field> BoxData::*which, int stage, double theta, double dt) {
+  for (int ib : H.level_boxes[level]) {
+    BoxData& b = H.boxes[ib];
+    if (level == 0) periodic_fill(b, b.*which);
+    else dense_ghost_fill(H, b, H.boxes[b.parent], b.*which, stage, theta, 2.0 * dt);
+  }
+}
+
+// One RK4 step of all boxes of one level (eqs 1-9), ghosts by fill(); theta = where this step starts
+// inside the parent's step (0 or 1/2; ignored on level 0).
+void rk4_level_step(Hier& H, int level, double dt, double theta) {
+  const double a_s[3] = {0.5, 0.5, 1.0};
+  for (int ib : H.level_boxes[level]) {
+    BoxData& b = H.boxes[ib];
+    b.y_old = b.y;  // y_n
+  }
+  fill(H, level, &BoxData::y_old, 1, theta, dt);  // eq (15): Y_1 = y_n also in the ghosts
+  for (int ib : H.level_boxes[level]) H.boxes[ib].Y = H.boxes[ib].y_old;  // eq (6)
+  for (int s = 1; s <= 4; ++s) {
+    for (int ib : H.level_boxes[level]) rhs(H, H.boxes[ib], H.boxes[ib].Y, H.boxes[ib].k[s - 1]);  // (1)-(4)
+    if (s < 4) {
+      for (int ib : H.level_boxes[level]) {
+        BoxData& b = H.boxes[ib];
+        axpy_interior(b, b.Y, b.y_old, a_s[s - 1] * dt, b.k[s - 1]);  // eqs (7)-(9)
+      }
+      fill(H, level, &BoxData::Y, s + 1, theta, dt);  // eqs (16)-(18) in the ghosts
+    }
+  }
+  for (int ib : H.level_boxes[level]) {
+    BoxData& b = H.boxes[ib];
+    for (int c = 0; c < 2 * H.F; ++c) {
+#pragma omp parallel for schedule(static)
+      for (int k = 0; k < b.n[2]; ++k)
+        for (int j = 0; j < b.n[1]; ++j)
+          for (int i = 0; i < b.n[0]; ++i)
+            b.y[c].at(i, j, k) = b.y_old[c].at(i, j, k) +
+                                 (dt / 6.0) * (b.k[0][c].at(i, j, k) + 2.0 * b.k[1][c].at(i, j, k) +
+                                               2.0 * b.k[2][c].at(i, j, k) + b.k[3][c].at(i, j, k));  // eq (5)
+    }
+  }
+  fill(H, level, &BoxData::y, 5, theta + 0.5, dt);  // eq (10) at theta + 1/2 in the ghosts
+}
+
+// Steps 1-7.
+void advance(Hier& H, int level, double dt, double theta) {
+  rk4_level_step(H, level, dt, theta);
+  if (level + 1 < H.nlevels) {
+    advance(H, level + 1, 0.5 * dt, 0.0);
+    advance(H, level + 1, 0.5 * dt, 0.5);
+    for (int ib : H.level_boxes[level + 1]) restrict_to_parent(H, H.boxes[ib], H.boxes[H.boxes[ib].parent]);
+  }
+}
+
+// Non-subcycled mode (S11, S15): all levels take the same step dt; refinement ghosts are the plain
+// spatial prolongation of the parent's SAME stage vector; restriction once per step, finest first.
+void same_time_fill(Hier& H, int level, std::vector<Field> BoxData::*which) {
+  for (int ib : H.level_boxes[level]) {
+    BoxData& b = H.boxes[ib];
+    if (level == 0) { periodic_fill(b, b.*which); continue; }
+    const BoxData& par = H.boxes[b.parent];
+    for (int c = 0; c < 2 * H.F; ++c) prolong_into_ghosts(b, par, (par.*which)[c], (b.*which)[c]);
+  }
+}
+
+void uniform_step(Hier& H, double dt) {
+  const double a_s[3] = {0.5, 0.5, 1.0};
+  const int L = H.nlevels;
+  for (BoxData& b : H.boxes) b.y_old = b.y;
+  for (int l = 0; l < L; ++l) same_time_fill(H, l, &BoxData::y_old);
+  for (BoxData& b : H.boxes) b.Y = b.y_old;
+  for (int s = 1; s <= 4; ++s) {
+    for (BoxData& b : H.boxes) rhs(H, b, b.Y, b.k[s - 1]);
+    if (s < 4) {
+      for (BoxData& b : H.boxes) axpy_interior(b, b.Y, b.y_old, a_s[s - 1] * dt, b.k[s - 1]);
+      for (int l = 0; l < L; ++l) same_time_fill(H, l, &BoxData::Y);
+    }
+  }
+  for (BoxData& b : H.boxes)
+    for (int c = 0; c < 2 * H.F; ++c)
+#pragma omp parallel for schedule(static)
+      for (int k = 0; k < b.n[2]; ++k)
+        for (int j = 0; j < b.n[1]; ++j)
+          for (int i = 0; i < b.n[0]; ++i)
+            b.y[c].at(i, j, k) = b.y_old[c].at(i, j, k) +
+                                 (dt / 6.0) * (b.k[0][c].at(i, j, k) + 2.0 * b.k[1][c].at(i, j, k) +
+                                               2.0 * b.k[2][c].at(i, j, k) + b.k[3][c].at(i, j, k));
+  for (int l = 0; l < L; ++l) same_time_fill(H, l, &BoxData::y);
+  for (int l = L - 1; l >= 1; --l)
+    for (int ib : H.level_boxes[l]) restrict_to_parent(H, H.boxes[ib], H.boxes[H.boxes[ib].parent]);
+}
+
+// preconditions the loops above rely on (S13)
+bool validate(Hier& H, char* msg, size_t cap) {
+  auto fail = [&](const char* m) { snprintf(msg, cap, "%s", m); return false; };
+  if (H.nlevels < 1 || H.boxes.empty()) return fail("no levels");
+  if (H.g < kStencilRadius || H.g > 8) return fail("ghost width");
+  if (H.level_boxes[0].size() != 1) return fail("level 0 must be one box");
+  const BoxData& b0 = H.boxes[H.level_boxes[0][0]];
+  for (int a = 0; a < 3; ++a)
+    if (b0.lo[a] != 0 || b0.n[a] != H.domain[a] || b0.n[a] < H.g) return fail("level 0 must cover the domain");
+  const int margin = (H.g + 1) / 2 + 2;
+  for (int l = 1; l < H.nlevels; ++l) {
+    if (H.level_boxes[l].empty()) return fail("empty level");
+    for (int ib : H.level_boxes[l]) {
+      BoxData& b = H.boxes[ib];
+      b.parent = -1;
+      for (int a = 0; a < 3; ++a)
+        if ((b.lo[a] & 1) || (b.n[a] & 1) || b.n[a] < 8) return fail("box lo/n must be even, n >= 8");
+      for (int ip : H.level_boxes[l - 1]) {
+        const BoxData& p = H.boxes[ip];
+        bool inside = true;
+        for (int a = 0; a < 3; ++a) {
+          const int plo = b.lo[a] / 2 - p.lo[a], phi = (b.lo[a] + b.n[a]) / 2 - p.lo[a];
+          if (plo < margin || phi > p.n[a] - margin) inside = false;
+        }
+        if (inside) { b.parent = ip; break; }
+      }
+      if (b.parent < 0) return fail("box not properly nested in a parent box");
+      for (int jb : H.level_boxes[l]) {
+        if (jb == ib) continue;
+        const BoxData& o = H.boxes[jb];
+        bool apart = false;
+        for (int a = 0; a < 3; ++a)
+          if (b.lo[a] >= o.lo[a] + o.n[a] + 2 * margin || o.lo[a] >= b.lo[a] + b.n[a] + 2 * margin) apart = true;
+        if (!apart) return fail("sibling boxes too close");
+      }
+    }
+  }
+  return true;
+}
+
+BoxData* get_box(Hier* H, int level, int box) {
+  if (!H || level < 0 || level >= H->nlevels) return nullptr;
+  if (box < 0 || box >= int(H->level_boxes[level].size())) return nullptr;
+  return &H->boxes[H->level_boxes[level][box]];
+}
+
+thread_local char g_err[256] = "";
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// C interface (loaded with ctypes by oracle/__init__.py)
+// ---------------------------------------------------------------------------------------------
+extern "C" {
+
+const char* oc_last_error() { return g_err; }
+
+void oc_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+int oc_max_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// unit-level entry points used by the pins
+double oc_b(int i, int m, double theta) { return b_coeff(i, m, theta); }
+double oc_dense_stage(int stage, double theta, double hp, double y_old, const double* k4) {
+  return dense_stage(stage, theta, hp, y_old, k4);
+}
+void oc_prolong_weights(int parity, double* w5) { prolong_weights(parity, w5); }
+void oc_restrict_weights(double* r6) { restrict_weights(r6); }
+
+void* oc_create(int nlevels, int nboxes, const int* box_level, const int* box_lo, const int* box_n, int ghost,
+                int nfields, const int* domain_cells, const double* xlo, const double* xhi,
+                const double* coupling) {
+  Hier* H = new Hier;
+  H->nlevels = nlevels;
+  H->g = ghost;
+  H->F = nfields;
+  for (int a = 0; a < 3; ++a) { H->domain[a] = domain_cells[a]; H->xlo[a] = xlo[a]; H->xhi[a] = xhi[a]; }
+  if (coupling) H->A.assign(coupling, coupling + size_t(nfields) * nfields);
+  if (nlevels < 1 || nlevels > 30 || nboxes < 1 || nfields < 1) {
+    snprintf(g_err, sizeof g_err, "bad sizes");
+    delete H;
+    return nullptr;
+  }
+  H->level_boxes.resize(nlevels);
+  H->boxes.resize(nboxes);
+  for (int ib = 0; ib < nboxes; ++ib) {
+    BoxData& b = H->boxes[ib];
+    b.level = box_level[ib];
+    if (b.level < 0 || b.level >= nlevels || (ib > 0 && b.level < box_level[ib - 1])) {
+      snprintf(g_err, sizeof g_err, "boxes must be sorted by level");
+      delete H;
+      return nullptr;
+    }
+    for (int a = 0; a < 3; ++a) { b.lo[a] = box_lo[3 * ib + a]; b.n[a] = box_n[3 * ib + a]; }
+    H->level_boxes[b.level].push_back(ib);
+  }
+  if (!validate(*H, g_err, sizeof g_err)) { delete H; return nullptr; }
+  for (BoxData& b : H->boxes) {
+    const int V = 2 * nfields;
+    b.y.resize(V); b.Y.resize(V); b.y_old.resize(V);
+    for (int s = 0; s < 4; ++s) b.k[s].resize(V);
+    for (int c = 0; c < V; ++c) {
+      b.y[c].init(b.n, ghost); b.Y[c].init(b.n, ghost); b.y_old[c].init(b.n, ghost);
+      for (int s = 0; s < 4; ++s) b.k[s][c].init(b.n, ghost);
+    }
+  }
+  return H;
+}
+
+void oc_destroy(void* h) { delete static_cast<Hier*>(h); }
+
+int oc_set_state(void* h, int level, int box, int comp, const double* src) {
+  Hier* H = static_cast<Hier*>(h);
+  BoxData* b = get_box(H, level, box);
+  if (!b || !src || comp < 0 || comp >= 2 * H->F) return -1;
+  size_t q = 0;
+  for (int k = 0; k < b->n[2]; ++k)
+    for (int j = 0; j < b->n[1]; ++j)
+      for (int i = 0; i < b->n[0]; ++i) b->y[comp].at(i, j, k) = src[q++];
+  return 0;
+}
+
+// slot: 0 = y (current), 1 = y_old, 2..5 = k_1..k_4; padded != 0 -> include ghosts
+int oc_read(void* h, int level, int box, int slot, int comp, int padded, double* dst) {
+  Hier* H = static_cast<Hier*>(h);
+  BoxData* b = get_box(H, level, box);
+  if (!b || !dst || comp < 0 || comp >= 2 * H->F || slot < 0 || slot > 5) return -1;
+  const Field& f = slot == 0 ? b->y[comp] : slot == 1 ? b->y_old[comp] : b->k[slot - 2][comp];
+  const int e = padded ? H->g : 0;
+  size_t q = 0;
+  for (int k = -e; k < b->n[2] + e; ++k)
+    for (int j = -e; j < b->n[1] + e; ++j)
+      for (int i = -e; i < b->n[0] + e; ++i) dst[q++] = f.at(i, j, k);
+  return 0;
+}
+
+int oc_step(void* h, double dt_coarse, int subcycling) {
+  Hier* H = static_cast<Hier*>(h);
+  if (!H || !(dt_coarse == dt_coarse)) return -1;
+  if (subcycling) {
+    advance(*H, 0, dt_coarse, 0.0);
+  } else {
+    const int nsub = 1 << (H->nlevels - 1);
+    for (int q = 0; q < nsub; ++q) uniform_step(*H, dt_coarse / double(nsub));
+  }
+  H->time += dt_coarse;
+  return 0;
+}
+
+double oc_time(void* h) { return static_cast<Hier*>(h)->time; }
+
+// Ghost index map of a level >= 1 box: canonical order (k, j, i over the padded box, interior skipped);
+// 7 ints per ghost cell: i, j, k (box-local), pi, pj, pk (parent-box-local), parity bits px|py<<1|pz<<2.
+long long oc_ghost_map(void* h, int level, int box, int* out, unsigned long long cap) {
+  Hier* H = static_cast<Hier*>(h);
+  BoxData* b = get_box(H, level, box);
+  if (!b || level < 1) return -1;
+  const BoxData& par = H->boxes[b->parent];
+  const int g = H->g;
+  long long cnt = 0;
+  for (int k = -g; k < b->n[2] + g; ++k)
+    for (int j = -g; j < b->n[1] + g; ++j)
+      for (int i = -g; i < b->n[0] + g; ++i) {
+        if (is_interior(*b, i, j, k)) continue;
+        if (out && (unsigned long long)(7 * (cnt + 1)) <= cap) {
+          const int loc[3] = {i, j, k};
+          int* o = out + 7 * cnt;
+          int bits = 0;
+          for (int a = 0; a < 3; ++a) {
+            const int I = b->lo[a] + loc[a];
+            const int Jg = floor_div2(I);
+            o[a] = loc[a];
+            o[3 + a] = Jg - par.lo[a];
+            bits |= (I - 2 * Jg) << a;
+          }
+          o[6] = bits;
+        }
+        ++cnt;
+      }
+  return cnt;
+}
+
+}  // extern "C"
