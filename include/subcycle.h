@@ -28,7 +28,7 @@ enum {
   SC_OK = 0,
   SC_ERR_INVALID_ARG = -1, /* null pointer, index out of range, non-finite dt, capacity too small */
   SC_ERR_NESTING = -2,     /* box list violates the nesting rules below                           */
-  SC_ERR_UNSUPPORTED = -3, /* ref_ratio != 2, ghost < 3 or > 4, nlevels > SC_MAX_LEVELS ...         */
+  SC_ERR_UNSUPPORTED = -3, /* ref_ratio != 2, ghost outside [2,4], nlevels > SC_MAX_LEVELS, F > 32  */
   SC_ERR_OOM = -4,         /* arena too small / device allocation failed                          */
   SC_ERR_CUDA = -5         /* a CUDA runtime/driver call failed (message has the CUDA error string) */
 };
@@ -60,8 +60,9 @@ typedef struct {
  *   d_t u_f = rho_f,   d_t rho_f = Lap_h u_f + sum_j A[f][j] u_j       (BASELINE cfg 4)
  * arena: optional DEVICE memory of at least sc_arena_bytes() bytes, 256-byte aligned, owned by the
  *   caller, who keeps it alive and does not touch it until sc_destroy; NULL -> the library allocates.
- * cuda_stream: a cudaStream_t (as void*) on which all work of this hierarchy is enqueued; NULL = the
- *   legacy default stream. */
+ * cuda_stream: a cudaStream_t (as void*) on which all work of this hierarchy is enqueued (must not be
+ *   the legacy default stream: steps are captured into CUDA graphs); NULL -> the library creates and
+ *   owns a private non-blocking stream. */
 typedef struct {
   int32_t nlevels;
   int32_t nboxes;

@@ -1,0 +1,202 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerance (BASELINE.json north_star): max|delta| <= 1e-11 * max|u| in fp64; index maps and the
+set_state -> read_level round trip bit-exact. Run on the B200 box with `-m gpu`."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2503_09629_b200 as sc
+from paper_2503_09629_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+RTOL = 1e-11
+
+
+def _pair(w):
+    return sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+
+
+def _scale(O, w):
+    return max(np.max(np.abs(O.read_level(l, ib, c))) for l in range(w.nlevels)
+               for ib in range(len(w.level_boxes(l))) for c in range(w.ncomp))
+
+
+def _compare_state(G, O, w, padded=True, what="state"):
+    worst = 0.0
+    for c in range(w.ncomp):
+        # per-component scale: rho and u live on different scales; the criterion is relative to max|u|
+        pass
+    scale = _scale(O, w)
+    for l in range(w.nlevels):
+        for ib in range(len(w.level_boxes(l))):
+            for c in range(w.ncomp):
+                a = G.sc_debug_read_padded(l, ib, c) if padded else G.sc_read_level(l, ib, c)
+                b = O.read(l, ib, c, padded=padded)
+                d = np.max(np.abs(a - b))
+                assert np.isfinite(a).all(), (what, l, ib, c)
+                worst = max(worst, d)
+                assert d <= RTOL * scale, f"{what}: level {l} box {ib} comp {c}: max|d|={d:.3e} scale={scale:.3e}"
+    return worst / scale
+
+
+def test_set_read_roundtrip_bit_exact():
+    w = wl.ragged_small()
+    G = sc.Hierarchy.from_workload(w)
+    for l in range(w.nlevels):
+        for ib in range(len(w.level_boxes(l))):
+            for c in range(w.ncomp):
+                assert np.array_equal(G.sc_read_level(l, ib, c), w.initial_state(l, ib, c))
+    # device-side source and destination
+    import torch
+    src = torch.arange(40 * 24 * 28, dtype=torch.float64, device="cuda").reshape(28, 24, 40) * 0.5
+    G.sc_set_state(0, 0, 1, src)
+    out = torch.empty_like(src)
+    G.sc_read_level(0, 0, 1, out)
+    assert torch.equal(out, src)
+    G.close()
+
+
+def test_ghost_index_map_bit_exact():
+    w = wl.ragged_small()
+    G, O = _pair(w)
+    for l in (1, 2):
+        for ib in range(len(w.level_boxes(l))):
+            assert np.array_equal(G.sc_debug_ghost_map(l, ib), O.ghost_map(l, ib))
+    w = wl.cfg4(n=32, nlevels=4, nfields=1)
+    G2, O2 = sc.Hierarchy(w.boxes, w.domain_cells), oracle.OracleHierarchy(w.boxes, w.domain_cells)
+    for ib in (0, 1):
+        assert np.array_equal(G2.sc_debug_ghost_map(3, ib), O2.ghost_map(3, ib))
+
+
+def test_single_level_step_and_slopes():
+    """One periodic level: rhs + stage combine + periodic fill alone; also k_1..k_4 and y_old."""
+    w = wl.Workload("t", [wl.Box(0, (0, 0, 0), (40, 24, 28))], (40, 24, 28), nfields=2,
+                    coupling=wl.coupling_matrix(2), init=wl.multi_gaussian_init(3))
+    G, O = _pair(w)
+    for sub in (True, False, True):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+        _compare_state(G, O, w, what=f"single level sub={sub}")
+    for slot in range(0, 4):  # y_old, k1..k3 (k4 is not stored on a level without children)
+        for c in range(w.ncomp):
+            a = G.sc_debug_read_slot(0, 0, slot, c)
+            b = O.read(0, 0, c, slot=slot + 1)
+            s = max(np.max(np.abs(b)), 1e-300)
+            assert np.max(np.abs(a - b)) <= RTOL * s, (slot, c)
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_two_level_one_step_ghosts_slopes_restriction(sub):
+    """After ONE coarse step: ghosts of both levels (stage-5 fill), parent cells under the child
+    (restriction), child slopes."""
+    w = wl.cfg1()
+    G, O = _pair(w)
+    G.sc_step(w.dt_coarse, sub)
+    O.step(w.dt_coarse, sub)
+    _compare_state(G, O, w, what=f"cfg1 one step sub={sub}")
+    if sub:
+        for slot in range(0, 5):
+            for c in range(2):
+                a = G.sc_debug_read_slot(0, 0, slot, c)
+                b = O.read(0, 0, c, slot=slot + 1)
+                s = max(np.max(np.abs(b)), 1e-300)
+                assert np.max(np.abs(a - b)) <= RTOL * s, (slot, c)
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_cfg1_full_run(sub):
+    w = wl.cfg1()
+    G, O = _pair(w)
+    for _ in range(w.coarse_steps):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+    rel = _compare_state(G, O, w, what=f"cfg1 8 steps sub={sub}")
+    assert abs(G.sc_time() - O.time) < 1e-15
+    print(f"cfg1 sub={sub}: max rel diff {rel:.2e}")
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_ragged_multibox_coupled(sub):
+    """Non-cubic boxes, ragged tile tails, two sibling boxes on the finest level, F = 2 with coupling."""
+    w = wl.ragged_small()
+    G, O = _pair(w)
+    for _ in range(3):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+        _compare_state(G, O, w, what=f"ragged sub={sub}")
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_cfg3_shape_scaled(sub):
+    """4 nested levels (config 3 shape) at 48^3, 3 coarse steps."""
+    w = wl.cfg3(n=48, nlevels=4)
+    G, O = _pair(w)
+    for _ in range(3):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+    _compare_state(G, O, w, what=f"cfg3/48 sub={sub}")
+
+
+def test_cfg4_shape_scaled():
+    """BBH-shaped (config 4): 5 levels of 32^3, finest = two boxes, 6 coupled fields, 2 coarse steps."""
+    w = wl.cfg4(n=32, nlevels=5, nfields=6)
+    G, O = _pair(w)
+    for sub in (True, False):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+        _compare_state(G, O, w, what=f"cfg4/32 sub={sub}")
+
+
+def test_cfg2_rung_matches_oracle_and_exact_solution():
+    """Config 2, 32^3 rung to t = 1 (64 coarse steps): parity and the error against the exact plane wave."""
+    w = wl.cfg2(32)
+    G, O = _pair(w)
+    for _ in range(w.coarse_steps):
+        G.sc_step(w.dt_coarse, True)
+        O.step(w.dt_coarse, True)
+    _compare_state(G, O, w, what="cfg2/32")
+    for l in (0, 1):
+        err = np.max(np.abs(G.sc_read_level(l, 0, 0) - wl.plane_wave_exact(w, l, 0, 0, 1.0)))
+        assert 5.5e-5 < err < 7e-5, (l, err)
+
+
+def test_ghost_width_2_and_4():
+    for g in (2, 4):
+        w = wl.cfg1()
+        w.ghost = g
+        G, O = _pair(w)
+        G.sc_step(w.dt_coarse, True)
+        O.step(w.dt_coarse, True)
+        _compare_state(G, O, w, what=f"ghost={g}")
+
+
+def test_graph_replay_equals_eager(monkeypatch):
+    """CUDA-graph replay (default) and plain stream launches (SC_GRAPH=0) give identical bits."""
+    w = wl.cfg3(n=32, nlevels=3)
+    G1 = sc.Hierarchy.from_workload(w)
+    monkeypatch.setenv("SC_GRAPH", "0")
+    G2 = sc.Hierarchy.from_workload(w)
+    monkeypatch.delenv("SC_GRAPH")
+    for _ in range(3):
+        G1.sc_step(w.dt_coarse, True)
+        G2.sc_step(w.dt_coarse, True)
+    for l in range(3):
+        for c in range(2):
+            assert np.array_equal(G1.sc_debug_read_padded(l, 0, c), G2.sc_debug_read_padded(l, 0, c))
+    assert G1.sc_launch_count() == G2.sc_launch_count() > 0
+
+
+def test_error_paths_on_device():
+    w = wl.cfg1()
+    G = sc.Hierarchy.from_workload(w)
+    with pytest.raises(sc.SubcycleError):
+        G.sc_step(float("nan"))
+    with pytest.raises(sc.SubcycleError):
+        G.sc_step(-1.0)
+    with pytest.raises(sc.SubcycleError):
+        G.sc_read_level(5, 0, 0)
+    with pytest.raises(sc.SubcycleError):
+        G.sc_debug_ghost_map(0, 0)
+    G.sc_step(w.dt_coarse)  # still usable afterwards
+    G.close()

@@ -1,0 +1,107 @@
+"""Host-side checks of the C ABI that need no GPU: the library loads, exports every symbol declared in
+include/subcycle.h, validates hierarchy descriptions (nesting rules, S13/S20) and sizes the
+arena. No compute calls."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import paper_2503_09629_b200 as sc
+from paper_2503_09629_b200 import workloads as wl
+from paper_2503_09629_b200.binding import (SC_ERR_INVALID_ARG, SC_ERR_NESTING, SC_ERR_UNSUPPORTED, SubcycleError)
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def built():
+    from paper_2503_09629_b200 import build
+    build.build()
+    return sc.lib()
+
+
+def test_exports_every_declared_symbol(built):
+    hdr = open(os.path.join(ROOT, "include", "subcycle.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(sc_[a-z_]+)\s*\(", hdr)))
+    assert declared and set(declared) == set(sc.EXPORTS)
+    for name in declared:
+        assert hasattr(built, name), name
+
+
+def _bytes(w):
+    d, keep = sc.make_desc(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling)
+    return sc.sc_arena_bytes(d)
+
+
+def test_all_baseline_configs_validate_and_size(built):
+    gib = 1 << 30
+    sizes = {name: _bytes(w) / gib for name, w in
+             (("cfg1", wl.cfg1()), ("cfg2", wl.cfg2(128)), ("cfg3", wl.cfg3()), ("cfg4", wl.cfg4()),
+              ("cfg5", wl.cfg5()), ("ragged", wl.ragged_small()))}
+    # memory with ghosts cfg 3 ~ 1.0 GiB, cfg 5 ~ 11.3 GiB, cfg 4 ~ 18.7 GiB (+ pitch padding)
+    assert 0.9 < sizes["cfg3"] < 1.4
+    assert 10.5 < sizes["cfg5"] < 13.5
+    assert 17.0 < sizes["cfg4"] < 24.0
+    assert sizes["cfg5"] < 170  # fits one B200
+
+
+def test_work_accounting_matches_survey(built):
+    assert wl.cfg1().updates_per_coarse_step(True) == 98304
+    assert wl.cfg1().updates_per_coarse_step(False) == 131072
+    assert wl.cfg3().updates_per_coarse_step(True) == 31457280
+    assert wl.cfg3().updates_per_coarse_step(False) == 67108864
+    assert abs(wl.cfg4().updates_per_coarse_step(True) / 1.501e8 - 1) < 2e-3
+    assert abs(wl.cfg4().updates_per_coarse_step(False) / 4.341e8 - 1) < 2e-3
+    assert abs(wl.cfg5().updates_per_coarse_step(True) / 1.057e9 - 1) < 1e-3
+    assert abs(wl.cfg5().updates_per_coarse_step(False) / 3.221e9 - 1) < 1e-3
+
+
+def test_nesting_validator_rejects_bad_hierarchies(built):
+    L = sc.lib()
+    B = wl.Box
+
+    def rc(boxes, dom=(32, 32, 32), **kw):
+        d, keep = sc.make_desc(boxes, dom, **kw)
+        out = C.c_void_p()
+        r = L.sc_create_hierarchy(C.byref(d), C.byref(out))
+        assert not out.value or r == 0
+        if out.value:
+            L.sc_destroy(out)
+        return r, L.sc_last_error().decode()
+
+    base = [B(0, (0, 0, 0), (32, 32, 32))]
+    # config 4 as literally written (two 96^3 finest boxes at +-0.3 of the level-2 extent): not nested
+    lit = wl.nested_cubes(6, 96)
+    ext2 = 96 * 4 // 2
+    off = int(0.3 * ext2) * 16
+    c6 = 96 * 64 // 2
+    lit += [B(6, (c6 - off - 48, c6 - 48, c6 - 48), (96, 96, 96)), B(6, (c6 + off - 48, c6 - 48, c6 - 48), (96, 96, 96))]
+    assert rc(lit, (96, 96, 96))[0] == SC_ERR_NESTING
+    assert rc(base + [B(1, (9, 16, 16), (16, 16, 16))])[0] == SC_ERR_NESTING       # odd lo
+    assert rc(base + [B(1, (16, 16, 16), (15, 16, 16))])[0] == SC_ERR_NESTING      # odd n
+    assert rc(base + [B(1, (6, 16, 16), (16, 16, 16))])[0] == SC_ERR_NESTING       # margin 3 < 4
+    assert rc(base + [B(1, (8, 16, 16), (16, 16, 16))])[0] != SC_ERR_NESTING       # margin 4 ok
+    assert rc(base + [B(1, (8, 8, 8), (16, 16, 16)), B(1, (30, 8, 8), (16, 16, 16))])[0] == SC_ERR_NESTING  # gap 6 < 8
+    assert rc(base + [B(1, (8, 8, 8), (16, 16, 16)), B(1, (32, 8, 8), (16, 16, 16))])[0] != SC_ERR_NESTING  # gap 8 ok
+    assert rc([B(0, (0, 0, 0), (32, 32, 16))])[0] == SC_ERR_NESTING                # level 0 must cover the domain
+    assert rc(base + [B(2, (40, 40, 40), (16, 16, 16))], nlevels=3)[0] == SC_ERR_NESTING  # empty level 1
+    assert rc(base, ref_ratio=4)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, ghost=1)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, ghost=5)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, nfields=0)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, xlo=(1.0, -1.0, -1.0), xhi=(1.0, 1.0, 1.0))[0] == SC_ERR_INVALID_ARG
+    r, msg = rc(base + [B(1, (6, 16, 16), (16, 16, 16))])
+    assert "margin" in msg or "parent" in msg
+
+
+def test_null_and_range_errors_do_not_abort(built):
+    L = sc.lib()
+    assert L.sc_arena_bytes(None) == 0
+    assert L.sc_create_hierarchy(None, None) == SC_ERR_INVALID_ARG
+    assert L.sc_step(None, 0.1, 1) == SC_ERR_INVALID_ARG
+    assert L.sc_set_state(None, 0, 0, 0, None, 0) == SC_ERR_INVALID_ARG
+    assert L.sc_read_level(None, 0, 0, 0, None, 0) == SC_ERR_INVALID_ARG
+    assert L.sc_destroy(None) == 0
+    assert L.sc_time(None) == 0.0
