@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the subcycled RK4 AMR step on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--mode sub|uniform] [--impl reference]
+
+One "step" = one coarse step of the whole hierarchy (sc_step): every level's RK4 level-steps, all ghost
+fills and restrictions. Default workload: BASELINE.json configs[4] ("large scalar-wave hierarchy for the
+bandwidth roofline": 6 levels x 256^3, fp64, subcycled), the configuration the metric's "% of HBM
+roofline" is quoted on; it fits one GPU (12 GB). Prints ONE JSON line.
+
+N > 1 (launched by torchrun, one rank per GPU): the path does not shard (north_star: one GPU, no
+collectives) -> N independent replicas, "scaling": "weak"; NCCL is used only for the barrier and the
+max-over-ranks of the device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2503_09629_b200 import workloads as wl  # noqa: E402
+
+METRIC = "grid-point updates/s (all levels, fp64 RK4)"
+UNIT = "updates/s"
+
+
+def pick_workload(idx: int):
+    return {1: wl.cfg1, 2: lambda: wl.cfg2(128), 3: wl.cfg3, 4: wl.cfg4, 5: wl.cfg5}[idx]()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands on the host cores, bounded sample
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(w, max_levels: int):
+    """The first `max_levels` levels of the workload (same boxes, same inputs)."""
+    if w.nlevels <= max_levels:
+        return w, f"all {w.nlevels} levels"
+    boxes = [b for b in w.boxes if b.level < max_levels]
+    s = wl.Workload(w.name + f" [levels 0..{max_levels - 1}]", boxes, w.domain_cells, w.nfields, w.ghost,
+                    w.xlo, w.xhi, w.coupling, w.coarse_steps, w.init)
+    return s, f"levels 0..{max_levels - 1} of {w.nlevels} ({'+'.join(str(b.n[0]) + '^3' for b in boxes)})"
+
+
+def time_oracle(w, steps: int, warmup: int, sub: bool, max_levels: int):
+    import oracle
+
+    oracle.build()
+    s, what = oracle_sample(w, max_levels)
+    H = oracle.OracleHierarchy.from_workload(s)
+    for _ in range(warmup):
+        H.step(s.dt_coarse, sub)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        H.step(s.dt_coarse, sub)
+    dt = time.perf_counter() - t0
+    upd = s.updates_per_coarse_step(sub) * steps
+    return {"value": upd / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"{what}, {steps} coarse step(s), {'subcycled' if sub else 'uniform'}, {dt:.1f} s",
+            "_seconds": dt, "_steps": steps}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = pick_workload(args.config)
+    sub = args.mode == "sub"
+    r = time_oracle(w, max(1, args.steps), min(args.warmup, 1), sub, max_levels=args.oracle_levels)
+    ms = 1e3 * r.pop("_seconds") / r.pop("_steps")
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "mode": args.mode, "note": "CPU oracle on a bounded sample"},
+            "cpu_baseline": r,
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks sampling
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 6:
+                continue
+            try:
+                sm.append(float(t[0]))
+                mx.append(float(t[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, t[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+
+    import paper_2503_09629_b200 as sc
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — libsubcycle has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = pick_workload(args.config)
+    sub = args.mode == "sub"
+    dt = w.dt_coarse
+    H = sc.Hierarchy(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling, device=f"cuda:{local}")
+
+    # inputs: seeded synthetic state, staged in pinned host memory (also the e2e source buffers)
+    host_in, host_out = {}, {}
+    for l in range(w.nlevels):
+        for ib in range(len(w.level_boxes(l))):
+            for c in range(w.ncomp):
+                a = w.initial_state(l, ib, c)
+                t = torch.empty(a.shape, dtype=torch.float64).pin_memory()
+                t.numpy()[...] = a
+                host_in[(l, ib, c)] = t
+    state_bytes = sum(t.numel() * 8 for t in host_in.values())
+    for k, t in host_in.items():
+        H.sc_set_state(*k, t.numpy())
+    H.synchronize()
+
+    st = H.stream
+    upd_step = w.updates_per_coarse_step(sub)
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between two events ----------
+    for _ in range(args.warmup):
+        H.sc_step(dt, sub)
+    barrier()
+    n0 = H.sc_launch_count()
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for _ in range(args.steps):
+        H.sc_step(dt, sub)
+    e1.record(st)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = H.sc_launch_count() - n0
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * upd_step * args.steps / (ms_total * 1e-3)
+
+    # ---- per-kernel roofline: same steps launched one by one with an event pair per kernel ---------
+    peak, peak_src = measured_peaks()
+    H.sc_profile(True)
+    for _ in range(max(1, min(args.steps, 2))):
+        H.sc_step(dt, sub)
+    kinds = {}
+    for i, name in enumerate(H.KERNEL_KINDS):
+        n, ms, by = H.sc_profile_read(i)
+        if n:
+            kinds[name] = {"launches": n, "ms_total": ms, "avg_us": 1e3 * ms / n,
+                           "algorithmic_GBps": by / (ms * 1e-3) / 1e9, "frac": by / (ms * 1e-3) / 1e9 / peak,
+                           "bytes_per_launch": by / n}
+    H.sc_profile(False)
+    dom = max(kinds, key=lambda k: kinds[k]["ms_total"])
+    ksum = sum(k["ms_total"] for k in kinds.values())
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["algorithmic_GBps"], "peak": peak,
+                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom),
+                "peak_source": peak_src, "share_of_step": kinds[dom]["ms_total"] / ksum,
+                "bytes_per_launch": kinds[dom]["bytes_per_launch"], "avg_launch_us": kinds[dom]["avg_us"]}
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the whole state, step, D2H ---------
+    for k, t in host_in.items():
+        host_out[k] = torch.empty(t.shape, dtype=torch.float64).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        for k, t in host_in.items():
+            H.sc_set_state(*k, t.numpy())
+        H.sc_step(dt, sub)
+        for k, t in host_out.items():
+            H.sc_read_level(*k, t.numpy())
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = {"value": world * upd_step * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+           "d2h_bytes_per_step": state_bytes, "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps}
+    finite = all(bool(torch.isfinite(t).all()) for t in host_out.values())
+    H.close()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = time_oracle(w, 1, 0, sub, max_levels=args.oracle_levels)
+        cpu.pop("_seconds"), cpu.pop("_steps")
+
+    # model bytes of the whole step for the whole-step roofline fraction
+    step_bytes = sum(k["bytes_per_launch"] * k["launches"] for k in kinds.values()) / max(1, min(args.steps, 2))
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "mode": "subcycled" if sub else "uniform", "ghost": w.ghost,
+                       "nfields": w.nfields, "dt_coarse": dt, "updates_per_step": upd_step,
+                       "zone_cycles_per_step": w.zone_cycles_per_coarse_step(),
+                       "l2": "inputs larger than L2 (state + stage buffers %.1f GB)" % (H.arena_bytes / 1e9),
+                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "kernels": kinds, "zone_cycles_per_s": world * w.zone_cycles_per_coarse_step() * args.steps / (ms_total * 1e-3),
+            "step_algorithmic_GB": step_bytes / 1e9,
+            "step_roofline_frac": step_bytes / (ms_total / args.steps * 1e-3) / 1e9 / peak,
+            "finite": finite}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of the
+# dominant kernel (profiles/): filled in per round; None until a capture exists.
+TRAFFIC = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--mode", default="sub", choices=["sub", "uniform"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--oracle-levels", type=int, default=2,
+                    help="levels of the workload the CPU oracle is timed on (bounded sample)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

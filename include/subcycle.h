@@ -135,6 +135,16 @@ int32_t sc_debug_read_padded(sc_hierarchy* h, int32_t level, int32_t box, int32_
 int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t slot, int32_t comp,
                            double* dst);
 
+/* Per-kernel timing for the roofline report. sc_profile(h, 1): from now on sc_step launches its kernels
+ * one by one (no graph replay) with a CUDA-event pair around each on the hierarchy's stream;
+ * sc_profile(h, 0) stops and discards the records. sc_profile_read sums, over the records since
+ * enabling, for kernel kind 0 = rhs_stage, 1 = ghost_dense_prolong, 2 = periodic_fill, 3 = restrict:
+ * the number of launches, their total device time (ms) and their total ALGORITHMIC bytes (DESIGN.md
+ * "Rooflines": what the method must move, not what the kernel happened to move). Out pointers: HOST,
+ * may be NULL. Both calls synchronise the stream. */
+int32_t sc_profile(sc_hierarchy* h, int32_t enable);
+int32_t sc_profile_read(sc_hierarchy* h, int32_t kind, uint64_t* launches, double* ms, double* bytes);
+
 /* Free everything the library owns (never the caller's arena). Synchronises the stream. */
 int32_t sc_destroy(sc_hierarchy* h);
 

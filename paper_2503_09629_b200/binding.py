@@ -19,7 +19,7 @@ SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NESTING, SC_ERR_UNSUPPORTED, SC_ERR_OOM, SC_ER
 
 EXPORTS = ["sc_arena_bytes", "sc_create_hierarchy", "sc_set_state", "sc_step", "sc_read_level", "sc_time",
            "sc_launch_count", "sc_debug_ghost_map", "sc_debug_read_padded", "sc_debug_read_slot", "sc_destroy",
-           "sc_last_error"]
+           "sc_last_error", "sc_profile", "sc_profile_read"]
 
 
 class sc_box(C.Structure):
@@ -75,6 +75,11 @@ def lib():
         L.sc_debug_read_slot.argtypes = [H, C.c_int32, C.c_int32, C.c_int32, C.c_int32, dp]
         L.sc_destroy.restype = C.c_int32
         L.sc_destroy.argtypes = [H]
+        L.sc_profile.restype = C.c_int32
+        L.sc_profile.argtypes = [H, C.c_int32]
+        L.sc_profile_read.restype = C.c_int32
+        L.sc_profile_read.argtypes = [H, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_double),
+                                      C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -217,6 +222,17 @@ class Hierarchy:
         out = np.empty((b.n[2], b.n[1], b.n[0]), dtype=np.float64)
         _check(lib().sc_debug_read_slot(self._h, level, ibox, slot, comp, out.ctypes.data))
         return out
+
+    KERNEL_KINDS = ("rhs_stage", "ghost_dense_prolong", "periodic_fill", "restrict")
+
+    def sc_profile(self, enable: bool) -> None:
+        _check(lib().sc_profile(self._h, int(bool(enable))))
+
+    def sc_profile_read(self, kind: int):
+        """(launches, total ms, total algorithmic bytes) of one kernel kind since sc_profile(True)."""
+        n, ms, by = C.c_uint64(), C.c_double(), C.c_double()
+        _check(lib().sc_profile_read(self._h, kind, C.byref(n), C.byref(ms), C.byref(by)))
+        return int(n.value), float(ms.value), float(by.value)
 
     def synchronize(self) -> None:
         self._stream.synchronize()

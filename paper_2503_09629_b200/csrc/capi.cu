@@ -53,6 +53,12 @@ struct sc_hierarchy {
   uint64_t counting = 0;          // launches of the sequence being recorded
   bool use_graph = true;
   std::map<GraphKey, GraphEntry> graphs;
+  // per-launch CUDA-event timing (sc_profile): eager launches, one event pair per kernel
+  struct BoxTiles { GhostTile* dev = nullptr; int n = 0; int s0 = 0, s1 = 0; };
+  std::vector<BoxTiles> tiles;    // per box (levels >= 1): ghost-shell tile list on the device
+  bool profiling = false;
+  struct ProfRec { int kind; double bytes; cudaEvent_t e0, e1; };
+  std::vector<ProfRec> prof;
 
   double* slot(int box, int s) const {
     const BoxInfo& b = L.boxes[box];
@@ -109,6 +115,43 @@ struct Seq {
   uint64_t n = 0;
 };
 
+enum { KIND_RHS = 0, KIND_GHOST = 1, KIND_PERIODIC = 2, KIND_RESTRICT = 3, NKIND = 4 };
+
+// Algorithmic bytes per launch: what the method must move.
+double cells(const BoxView& v) { return (double)v.n[0] * v.n[1] * v.n[2]; }
+double shell_cells(const BoxView& v) {
+  return (double)(v.n[0] + 2 * v.g) * (v.n[1] + 2 * v.g) * (v.n[2] + 2 * v.g) - cells(v);
+}
+double footprint_cells(const BoxView& v) {  // parent cells a ghost fill of this box reads
+  // ghost cells sit in parent cells up to gc = ceil(g/2) beyond the child's coverage [0, nc); the 5-point
+  // interpolation adds 2 more on every side and reaches 2 cells into the coverage
+  const int gc = (v.g + 1) / 2;
+  double outer = 1.0, inner = 1.0;
+  for (int a = 0; a < 3; ++a) {
+    const int nc = v.n[a] / 2;
+    outer *= nc + 2 * gc + 4;
+    inner *= nc > 4 ? nc - 4 : 0;
+  }
+  return outer - inner;
+}
+double rhs_bytes(const BoxView& v, int V, int stage, bool keep_k) {
+  const double per = stage == 1 ? 3.0 : (stage == 4 ? (keep_k ? 7.0 : 6.0) : 4.0);
+  return 8.0 * per * V * cells(v);
+}
+
+void prof_begin(sc_hierarchy* h, int kind, double bytes) {
+  if (!h->profiling) return;
+  sc_hierarchy::ProfRec r{kind, bytes, nullptr, nullptr};
+  cudaEventCreate(&r.e0);
+  cudaEventCreate(&r.e1);
+  cudaEventRecord(r.e0, h->stream);
+  h->prof.push_back(r);
+}
+void prof_end(sc_hierarchy* h) {
+  if (!h->profiling) return;
+  cudaEventRecord(h->prof.back().e1, h->stream);
+}
+
 void rhs_level(Seq& q, int level, int stage, int sYin, int sYn, int sYout, double cdt, bool keep_k) {
   sc_hierarchy* h = q.h;
   for (int ib : h->L.level_boxes[level]) {
@@ -129,7 +172,9 @@ void rhs_level(Seq& q, int level, int stage, int sYin, int sYn, int sYout, doubl
       a.inv12dx2[d] = 1.0 / (12.0 * dx * dx);
     }
     a.A = h->coupling();
+    prof_begin(h, KIND_RHS, rhs_bytes(a.b, h->L.V, stage, keep_k));
     launch_rhs_stage(a, h->stream);
+    prof_end(h);
     ++q.n;
   }
 }
@@ -141,7 +186,9 @@ void fill_level_dense(Seq& q, int level, int sdst, int stage, double theta, doub
   for (int ib : h->L.level_boxes[level]) {
     const BoxInfo& b = h->L.boxes[ib];
     if (level == 0) {
+      prof_begin(h, KIND_PERIODIC, 16.0 * h->L.V * shell_cells(b.v));
       launch_periodic_fill(b.v, h->L.V, h->slot(ib, sdst), h->stream);
+      prof_end(h);
       ++q.n;
       continue;
     }
@@ -151,6 +198,8 @@ void fill_level_dense(Seq& q, int level, int sdst, int stage, double theta, doub
     a.V = h->L.V;
     a.dst = h->slot(ib, sdst);
     a.base = h->slot(b.parent, parent_yold);
+    a.tiles = h->tiles[ib].dev; a.ntiles = h->tiles[ib].n;
+    a.s0_doubles = h->tiles[ib].s0; a.s1_doubles = h->tiles[ib].s1;
     double c[4];
     dense_coeffs(stage, theta, c);
     a.use_k = 0;
@@ -159,7 +208,9 @@ void fill_level_dense(Seq& q, int level, int sdst, int stage, double theta, doub
       a.coef[j] = hp * c[j];
       if (c[j] != 0.0) a.use_k |= 1 << j;
     }
+    prof_begin(h, KIND_GHOST, 8.0 * h->L.V * ((1 + __builtin_popcount(a.use_k)) * footprint_cells(b.v) + shell_cells(b.v)));
     launch_ghost_fill(a, h->stream);
+    prof_end(h);
     ++q.n;
   }
 }
@@ -170,7 +221,9 @@ void fill_level_same_time(Seq& q, int level, int sdst, int sparent) {
   for (int ib : h->L.level_boxes[level]) {
     const BoxInfo& b = h->L.boxes[ib];
     if (level == 0) {
+      prof_begin(h, KIND_PERIODIC, 16.0 * h->L.V * shell_cells(b.v));
       launch_periodic_fill(b.v, h->L.V, h->slot(ib, sdst), h->stream);
+      prof_end(h);
       ++q.n;
       continue;
     }
@@ -181,8 +234,12 @@ void fill_level_same_time(Seq& q, int level, int sdst, int sparent) {
     a.dst = h->slot(ib, sdst);
     a.base = h->slot(b.parent, sparent);
     a.use_k = 0;
+    a.tiles = h->tiles[ib].dev; a.ntiles = h->tiles[ib].n;
+    a.s0_doubles = h->tiles[ib].s0; a.s1_doubles = h->tiles[ib].s1;
     for (int j = 0; j < 4; ++j) { a.k[j] = a.base; a.coef[j] = 0.0; }
+    prof_begin(h, KIND_GHOST, 8.0 * h->L.V * (footprint_cells(b.v) + shell_cells(b.v)));
     launch_ghost_fill(a, h->stream);
+    prof_end(h);
     ++q.n;
   }
 }
@@ -191,8 +248,10 @@ void restrict_level(Seq& q, int level) {  // level -> level-1, into the parents'
   sc_hierarchy* h = q.h;
   for (int ib : h->L.level_boxes[level]) {
     const BoxInfo& b = h->L.boxes[ib];
+    prof_begin(h, KIND_RESTRICT, 8.0 * h->L.V * (cells(b.v) + cells(b.v) / 8.0));
     launch_restrict(b.v, h->L.boxes[b.parent].v, h->L.V, h->slot(ib, q.cur[level]),
                     h->slot(b.parent, q.cur[level - 1]), h->stream);
+    prof_end(h);
     ++q.n;
   }
 }
@@ -350,6 +409,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   auto bail = [&](const char* what, cudaError_t e) {
     set_error(std::string(what) + ": " + cudaGetErrorString(e));
     if (h->staging) cudaFree(h->staging);
+    for (auto& bt : h->tiles) if (bt.dev) cudaFree(bt.dev);
     if (h->own_arena) cudaFree(h->arena);
     if (h->own_stream) cudaStreamDestroy(h->stream);
     delete h;
@@ -361,6 +421,18 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     ce = cudaMemcpyAsync(h->arena + h->L.coupling_offset, desc->coupling, sizeof(double) * h->L.F * h->L.F,
                          cudaMemcpyHostToDevice, h->stream);
     if (ce != cudaSuccess) return bail("copy coupling", ce);
+  }
+  h->tiles.resize(h->L.boxes.size());
+  for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
+    if (h->L.boxes[ib].level == 0) continue;
+    std::vector<GhostTile> tl;
+    size_t s0 = 0, s1 = 0;
+    build_ghost_tiles(h->L.boxes[ib].v, tl, &s0, &s1);
+    sc_hierarchy::BoxTiles& bt = h->tiles[ib];
+    bt.n = (int)tl.size(); bt.s0 = (int)s0; bt.s1 = (int)s1;
+    if ((ce = cudaMalloc(&bt.dev, sizeof(GhostTile) * tl.size())) != cudaSuccess) return bail("cudaMalloc(tiles)", ce);
+    if ((ce = cudaMemcpy(bt.dev, tl.data(), sizeof(GhostTile) * tl.size(), cudaMemcpyHostToDevice)) != cudaSuccess)
+      return bail("copy tiles", ce);
   }
   if ((ce = cudaStreamSynchronize(h->stream)) != cudaSuccess) return bail("sync", ce);
   h->cur.assign(h->L.nlevels, 0);
@@ -402,7 +474,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
   if (!std::isfinite(dt_coarse) || dt_coarse <= 0.0) { set_error("dt_coarse must be finite and > 0"); return SC_ERR_INVALID_ARG; }
   subcycling = subcycling ? 1 : 0;
   Seq q{h, h->cur, 0};
-  if (!h->use_graph) {
+  if (!h->use_graph || h->profiling) {
     record_step(q, dt_coarse, subcycling);
     SC_CUDA(cudaGetLastError());
     h->launches += q.n;
@@ -492,12 +564,42 @@ int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t 
   return read_array(h, gb, h->slot(gb, s) + (long long)comp * v.vol, dst, 0, 0);
 }
 
+int32_t sc_profile(sc_hierarchy* h, int32_t enable) {
+  if (!h) { set_error("null hierarchy"); return SC_ERR_INVALID_ARG; }
+  SC_CUDA(cudaStreamSynchronize(h->stream));
+  for (auto& r : h->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+  h->prof.clear();
+  h->profiling = enable != 0;
+  return SC_OK;
+}
+
+int32_t sc_profile_read(sc_hierarchy* h, int32_t kind, uint64_t* launches, double* ms, double* bytes) {
+  if (!h || kind < 0 || kind >= NKIND) { set_error("bad hierarchy or kind"); return SC_ERR_INVALID_ARG; }
+  SC_CUDA(cudaStreamSynchronize(h->stream));
+  uint64_t n = 0;
+  double t = 0.0, b = 0.0;
+  for (auto& r : h->prof) {
+    if (r.kind != kind) continue;
+    float e = 0.f;
+    SC_CUDA(cudaEventElapsedTime(&e, r.e0, r.e1));
+    t += e;
+    b += r.bytes;
+    ++n;
+  }
+  if (launches) *launches = n;
+  if (ms) *ms = t;
+  if (bytes) *bytes = b;
+  return SC_OK;
+}
+
 int32_t sc_destroy(sc_hierarchy* h) {
   if (!h) return SC_OK;
   cudaStreamSynchronize(h->stream);
+  for (auto& r : h->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   for (auto& kv : h->graphs)
     if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
   if (h->staging) cudaFree(h->staging);
+  for (auto& bt : h->tiles) if (bt.dev) cudaFree(bt.dev);
   if (h->own_arena && h->arena) cudaFree(h->arena);
   if (h->own_stream) cudaStreamDestroy(h->stream);
   delete h;

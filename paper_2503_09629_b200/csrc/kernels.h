@@ -33,6 +33,13 @@ void launch_rhs_stage(const RhsArgs& a, cudaStream_t st);
 //   ghost(dst) = P[ base + sum_j coef[j] * k[j] ]  over the parent's cells, P = 5x5x5 tensor Lagrange.
 // coef[j] already contains the parent step h_p (coef = h_p * c_j(stage, theta)); nk = number of leading
 // k arrays with a non-zero coefficient pattern (0 = pure prolongation of base).
+struct GhostTile {   // a piece of one ghost slab, box-local fine indices
+  int lo[3];
+  int n[3];
+  int axis;          // the slab's thin axis: 0 = x-slab, 1 = y-slab, 2 = z-slab
+  int pad;
+};
+
 struct GhostArgs {
   BoxView child, parent;
   int V;
@@ -41,7 +48,11 @@ struct GhostArgs {
   const double* k[4];   // parent k_1..k_4 slot bases
   double coef[4];
   int use_k;            // bit j set -> k[j] is read
+  const GhostTile* tiles;  // device; tile list of the child box (built once per box)
+  int ntiles;
+  int s0_doubles, s1_doubles;  // shared-memory staging sizes the tile list needs
 };
+void build_ghost_tiles(const BoxView& child, std::vector<GhostTile>& tiles, size_t* s0_doubles, size_t* s1_doubles);
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st);
 
 // a4: periodic ghost fill of the level-0 box (reading S9).
