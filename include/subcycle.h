@@ -130,15 +130,18 @@ int64_t sc_debug_ghost_map(sc_hierarchy* h, int32_t level, int32_t box, int32_t*
  * memory. Synchronises the stream. Ghost values are those of the last stage-5 fill. */
 int32_t sc_debug_read_padded(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, double* dst);
 
-/* Debug: which of the stored RK slopes / old state to read: slot 0 = y_old, 1..4 = k_1..k_4 of the last
- * level-step of that box (interior only, HOST dst). */
+/* Debug: what the library keeps of the last level-step of a box (S26), interior only, HOST dst:
+ * slot 1 = y_n (the state before that level-step), any comp; slot 2, 3, 4 = the stage vectors Y_2, Y_3, Y_4
+ * (eqs 7-9), rho components only (nfields <= comp < 2*nfields): for d_t u = rho the slope
+ * k_{s,u} is Y_{s,rho}, so the u-parts of the stage vectors and the slopes k_1..k_4 are never stored
+ * (Y_{s+1,u} = u_n + a_s dt Y_{s,rho};  k_{s,rho} = (Y_{s+1,rho} - rho_n) / (a_s dt)). */
 int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t slot, int32_t comp,
                            double* dst);
 
 /* Per-kernel timing for the roofline report. sc_profile(h, 1): from now on sc_step launches its kernels
  * one by one (no graph replay) with a CUDA-event pair around each on the hierarchy's stream;
  * sc_profile(h, 0) stops and discards the records. sc_profile_read sums, over the records since
- * enabling, for kernel kind 0 = rhs_stage, 1 = ghost_dense_prolong, 2 = periodic_fill, 3 = restrict:
+ * enabling, for kernel kind 0 = rk_stage, 1 = ghost_dense_prolong, 2 = periodic_fill, 3 = restrict:
  * the number of launches, their total device time (ms) and their total ALGORITHMIC bytes (DESIGN.md
  * "Rooflines": what the method must move, not what the kernel happened to move). Out pointers: HOST,
  * may be NULL. Both calls synchronise the stream. */

@@ -223,7 +223,7 @@ class Hierarchy:
         _check(lib().sc_debug_read_slot(self._h, level, ibox, slot, comp, out.ctypes.data))
         return out
 
-    KERNEL_KINDS = ("rhs_stage", "ghost_dense_prolong", "periodic_fill", "restrict")
+    KERNEL_KINDS = ("rk_stage", "ghost_dense_prolong", "periodic_fill", "restrict")
 
     def sc_profile(self, enable: bool) -> None:
         _check(lib().sc_profile(self._h, int(bool(enable))))

@@ -46,23 +46,25 @@ struct sc_hierarchy {
   bool own_stream = false;
   double* staging = nullptr;      // device, largest padded dense box
   size_t staging_bytes = 0;
-  std::vector<int> cur;           // per level: slot (0 or 2) that holds the current state y
-  std::vector<char> ghosts_valid; // per level: ghosts of y hold the last stage-5 fill (no set_state since)
+  std::vector<int> cur;           // per level: state slot (0 or 1) that holds the current state y
+  bool l0_ghosts_valid = false;   // level 0: ghosts of y hold the periodic copies (no set_state since)
   double time = 0.0;
   uint64_t launches = 0;
-  uint64_t counting = 0;          // launches of the sequence being recorded
   bool use_graph = true;
   std::map<GraphKey, GraphEntry> graphs;
-  // per-launch CUDA-event timing (sc_profile): eager launches, one event pair per kernel
-  struct BoxTiles { GhostTile* dev = nullptr; int n = 0; int s0 = 0, s1 = 0; };
+  struct BoxTiles { GhostTile* dev = nullptr; int n = 0; };
   std::vector<BoxTiles> tiles;    // per box (levels >= 1): ghost-shell tile list on the device
+  struct alignas(64) TMap { unsigned char bytes[128]; };
+  std::vector<TMap> tmaps;        // per box: CUtensorMap over all arrays of the box
+  std::vector<char> tmap_ok;
+  // per-launch CUDA-event timing (sc_profile): eager launches, one event pair per kernel
   bool profiling = false;
   struct ProfRec { int kind; double bytes; cudaEvent_t e0, e1; };
   std::vector<ProfRec> prof;
 
-  double* slot(int box, int s) const {
+  double* arr(int box, int array) const {
     const BoxInfo& b = L.boxes[box];
-    return reinterpret_cast<double*>(arena + b.arena_offset + (unsigned long long)s * b.slot_bytes);
+    return reinterpret_cast<double*>(arena + b.arena_offset) + (long long)array * b.v.vol;
   }
   const double* coupling() const {
     return L.has_coupling ? reinterpret_cast<const double*>(arena + L.coupling_offset) : nullptr;
@@ -80,9 +82,9 @@ namespace {
     }                                                                                    \
   } while (0)
 
-// Folded dense-output coefficients: ghost value of RK stage `stage` of a child step that starts at
-// parent progress theta is  P[ y_old^p + h_p * sum_j c_j k_j^p ]  with, from eqs (10)-(18)
-// and child step h = r h_p, r = 1/2:
+// Folded dense-output coefficients: the value of RK stage `stage` of a child step that starts at parent
+// progress theta is  y_old^p + h_p * sum_j c_j k_j^p  with, from eqs (10)-(18) and child
+// step h = r h_p, r = 1/2:
 //   stage 1, 5:  c = b(theta)                               (eq 15 / eq 10; stage 5 gets theta + 1/2)
 //   stage 2:     c = b + (r/2) b'                           (eq 16)
 //   stage 3:     c = b + (r/2) b' + (r^2/4) b'' + (r^3/16)(b''' - phi)   (eq 17)
@@ -111,13 +113,15 @@ void dense_coeffs(int stage, double th, double c[4]) {
 // ---- launch recording -----------------------------------------------------------------------
 struct Seq {
   sc_hierarchy* h;
-  std::vector<int> cur;  // working copy of the slot phases
+  std::vector<int> cur;  // working copy of the state-slot phases
+  bool l0_valid;         // working copy of l0_ghosts_valid
   uint64_t n = 0;
 };
 
-enum { KIND_RHS = 0, KIND_GHOST = 1, KIND_PERIODIC = 2, KIND_RESTRICT = 3, NKIND = 4 };
+enum { KIND_STAGE = 0, KIND_GHOST = 1, KIND_PERIODIC = 2, KIND_RESTRICT = 3, NKIND = 4 };
 
-// Algorithmic bytes per launch: what the method must move.
+// Algorithmic bytes per launch: every array a kernel must read once and every
+// array it must write once, in the formulation of sc_internal.h.
 double cells(const BoxView& v) { return (double)v.n[0] * v.n[1] * v.n[2]; }
 double shell_cells(const BoxView& v) {
   return (double)(v.n[0] + 2 * v.g) * (v.n[1] + 2 * v.g) * (v.n[2] + 2 * v.g) - cells(v);
@@ -134,9 +138,11 @@ double footprint_cells(const BoxView& v) {  // parent cells a ghost fill of this
   }
   return outer - inner;
 }
-double rhs_bytes(const BoxView& v, int V, int stage, bool keep_k) {
-  const double per = stage == 1 ? 3.0 : (stage == 4 ? (keep_k ? 7.0 : 6.0) : 4.0);
-  return 8.0 * per * V * cells(v);
+double stage_bytes(const BoxView& v, int F, int mode) {
+  // STAGE_12: read u_n, rho_n; write Y2r, Y3r.  STAGE_3: read u_n, Y2r, rho_n; write Y4r.
+  // STAGE_4: read u_n, Y3r, rho_n, Y2r, Y4r; write u_new, rho_new.
+  const double per = mode == STAGE_4 ? 7.0 : 4.0;
+  return 8.0 * per * F * cells(v);
 }
 
 void prof_begin(sc_hierarchy* h, int kind, double bytes) {
@@ -152,95 +158,132 @@ void prof_end(sc_hierarchy* h) {
   cudaEventRecord(h->prof.back().e1, h->stream);
 }
 
-void rhs_level(Seq& q, int level, int stage, int sYin, int sYn, int sYout, double cdt, bool keep_k) {
+// ---- one launch per (level, kernel): all boxes of the level -------------------------------------------
+void stage_level(Seq& q, int level, int mode, double dt) {
   sc_hierarchy* h = q.h;
-  for (int ib : h->L.level_boxes[level]) {
-    RhsArgs a{};
-    a.b = h->L.boxes[ib].v;
-    a.F = h->L.F;
-    a.stage = stage;
-    a.Yin = h->slot(ib, sYin);
-    a.yn = h->slot(ib, sYn);
-    a.kout = keep_k ? h->slot(ib, SLOT_K1 + stage - 1) : nullptr;
-    a.Yout = h->slot(ib, sYout);
-    a.k1 = h->slot(ib, SLOT_K1);
-    a.k2 = h->slot(ib, SLOT_K1 + 1);
-    a.k3 = h->slot(ib, SLOT_K1 + 2);
-    a.cdt = cdt;
+  const Layout& L = h->L;
+  const int yn = q.cur[level], ynew = 1 - yn;
+  for (int ib : L.level_boxes[level]) {
+    StageArgs a{};
+    a.b = L.boxes[ib].v;
+    a.F = L.F;
+    a.mode = mode;
+    a.a_yn = L.a_state(yn);
+    a.yn = h->arr(ib, a.a_yn);
+    a.a_R = mode == STAGE_12 ? L.a_state(yn) + L.F : (mode == STAGE_3 ? L.a_Y2r() : L.a_Y3r());
+    a.R = h->arr(ib, a.a_R);
+    a.Y2r = h->arr(ib, L.a_Y2r());
+    a.Y4r = h->arr(ib, L.a_Y4r());
+    a.out0 = mode == STAGE_12 ? h->arr(ib, L.a_Y2r()) : (mode == STAGE_3 ? h->arr(ib, L.a_Y4r()) : h->arr(ib, L.a_state(ynew)));
+    a.out1 = h->arr(ib, L.a_Y3r());
+    a.dt = dt;
     for (int d = 0; d < 3; ++d) {
-      const double dx = h->L.dx(level, d);
+      const double dx = L.dx(level, d);
       a.inv12dx2[d] = 1.0 / (12.0 * dx * dx);
     }
     a.A = h->coupling();
-    prof_begin(h, KIND_RHS, rhs_bytes(a.b, h->L.V, stage, keep_k));
-    launch_rhs_stage(a, h->stream);
+    a.scratch = L.has_coupling ? h->arr(ib, L.a_scratch()) : nullptr;
+    a.tmap = h->tmap_ok[ib] ? h->tmaps[ib].bytes : nullptr;
+    prof_begin(h, KIND_STAGE, stage_bytes(a.b, L.F, mode));
+    launch_stage(a, h->stream);
     prof_end(h);
     ++q.n;
   }
 }
 
-// ghosts of slot `sdst` of every box of `level`: periodic (level 0) or dense output of the parent
-// (subcycled: base = parent's y_old slot, coefficients of (stage, theta) times the parent step hp).
-void fill_level_dense(Seq& q, int level, int sdst, int stage, double theta, double hp, int parent_yold) {
+void periodic_level0(Seq& q, int first_array, int narrays) {
   sc_hierarchy* h = q.h;
-  for (int ib : h->L.level_boxes[level]) {
-    const BoxInfo& b = h->L.boxes[ib];
-    if (level == 0) {
-      prof_begin(h, KIND_PERIODIC, 16.0 * h->L.V * shell_cells(b.v));
-      launch_periodic_fill(b.v, h->L.V, h->slot(ib, sdst), h->stream);
-      prof_end(h);
-      ++q.n;
-      continue;
-    }
+  const int ib = h->L.level_boxes[0][0];
+  const BoxView& v = h->L.boxes[ib].v;
+  prof_begin(h, KIND_PERIODIC, 16.0 * narrays * shell_cells(v));
+  launch_periodic_fill(v, narrays, h->arr(ib, first_array), h->stream);
+  prof_end(h);
+  ++q.n;
+}
+
+void ghost_launch(Seq& q, int ib, GhostArgs& a) {
+  sc_hierarchy* h = q.h;
+  const BoxInfo& b = h->L.boxes[ib];
+  a.child = b.v;
+  a.parent = h->L.boxes[b.parent].v;
+  a.F = h->L.F;
+  a.tiles = h->tiles[ib].dev;
+  a.ntiles = h->tiles[ib].n;
+  prof_begin(h, KIND_GHOST, 8.0 * h->L.F * (a.nsrc * footprint_cells(b.v) + a.nout * shell_cells(b.v)));
+  launch_ghost_fill(a, h->stream);
+  prof_end(h);
+  ++q.n;
+}
+
+// Subcycled mode: ALL refinement-boundary ghosts one level-step of `level` (>= 1) needs, in one launch per
+// box, from the parent's stored (u_n, rho_n, Y2r, Y3r, Y4r) =: (u^p, K_1..K_4), K_j = k_{j,u}^p
+// (steps 2-6). With c^(s) = dense_coeffs(s, theta), parent step h_p, child step dt = h_p/2,
+// a = (1/2, 1/2, 1):
+//   shell of u_n    <- P[ u^p + h_p sum_j c^(1)_j K_j ]                               ghost of Y_1 (eq 15)
+//   shell of rho_n  <- P[ sum_j (c^(2)_j - c^(1)_j) / (a_1/2) K_j ] =: D_1,   u_n + a_1 dt D_1 = ghost of Y_{2,u} (eq 16)
+//   shell of Y2r    <- D_2 likewise from c^(3)                                        ghost of Y_{3,u} (eq 17)
+//   shell of Y3r    <- D_3 likewise from c^(4)                                        ghost of Y_{4,u} (eq 18)
+// (the stage kernels rebuild Y_{s+1,u} = u_n + a_s dt Y_{s,rho} on ghost cells exactly as on interior
+// cells; only ghosts of u are ever read, S25). If theta = 1/2 the step ends at the parent's t_{n+1}: eq (10)
+// at theta + 1/2 = 1 is the parent's own RK4 update, so the shells of y_{n+1} (all V components; the
+// restriction reads them) are P[u_new^p], P[rho_new^p] taken BEFORE the restriction into the parent. At
+// theta = 0 the y_{n+1} ghosts are the next step's Y_1 ghosts (S8) and are written by its launch.
+void fill_level_dense(Seq& q, int level, double theta, double dt) {
+  sc_hierarchy* h = q.h;
+  const Layout& L = h->L;
+  const double hp = 2.0 * dt;
+  const int yn = q.cur[level];
+  const int pnew = q.cur[level - 1], pold = 1 - pnew;  // the parent has already stepped
+  double c1[4], cs[4];
+  dense_coeffs(1, theta, c1);
+  for (int ib : L.level_boxes[level]) {
+    const int ip = L.boxes[ib].parent;
     GhostArgs a{};
-    a.child = b.v;
-    a.parent = h->L.boxes[b.parent].v;
-    a.V = h->L.V;
-    a.dst = h->slot(ib, sdst);
-    a.base = h->slot(b.parent, parent_yold);
-    a.tiles = h->tiles[ib].dev; a.ntiles = h->tiles[ib].n;
-    a.s0_doubles = h->tiles[ib].s0; a.s1_doubles = h->tiles[ib].s1;
-    double c[4];
-    dense_coeffs(stage, theta, c);
-    a.use_k = 0;
-    for (int j = 0; j < 4; ++j) {
-      a.k[j] = h->slot(b.parent, SLOT_K1 + j);
-      a.coef[j] = hp * c[j];
-      if (c[j] != 0.0) a.use_k |= 1 << j;
+    a.nsrc = 5;
+    a.src[0] = h->arr(ip, L.a_state(pold));
+    a.src[1] = h->arr(ip, L.a_state(pold) + L.F);
+    a.src[2] = h->arr(ip, L.a_Y2r());
+    a.src[3] = h->arr(ip, L.a_Y3r());
+    a.src[4] = h->arr(ip, L.a_Y4r());
+    a.nout = 4;
+    a.dst[0] = h->arr(ib, L.a_state(yn));
+    a.dst[1] = h->arr(ib, L.a_state(yn) + L.F);
+    a.dst[2] = h->arr(ib, L.a_Y2r());
+    a.dst[3] = h->arr(ib, L.a_Y3r());
+    a.coef[0][0] = 1.0;
+    for (int j = 0; j < 4; ++j) a.coef[0][1 + j] = hp * c1[j];
+    const double as[3] = {0.5, 0.5, 1.0};
+    for (int s = 0; s < 3; ++s) {
+      dense_coeffs(s + 2, theta, cs);
+      for (int j = 0; j < 4; ++j) a.coef[1 + s][1 + j] = 2.0 * (cs[j] - c1[j]) / as[s];  // h_p / (a_s dt) = 2 / a_s
     }
-    prof_begin(h, KIND_GHOST, 8.0 * h->L.V * ((1 + __builtin_popcount(a.use_k)) * footprint_cells(b.v) + shell_cells(b.v)));
-    launch_ghost_fill(a, h->stream);
-    prof_end(h);
-    ++q.n;
+    if (theta != 0.0) {
+      a.nsrc = 7;
+      a.src[5] = h->arr(ip, L.a_state(pnew));
+      a.src[6] = h->arr(ip, L.a_state(pnew) + L.F);
+      a.nout = 6;
+      a.dst[4] = h->arr(ib, L.a_state(1 - yn));
+      a.dst[5] = h->arr(ib, L.a_state(1 - yn) + L.F);
+      a.coef[4][5] = 1.0;
+      a.coef[5][6] = 1.0;
+    }
+    ghost_launch(q, ib, a);
   }
 }
 
-// uniform mode: ghosts = plain prolongation of the parent's slot `sparent` (same RK stage, same time)
-void fill_level_same_time(Seq& q, int level, int sdst, int sparent) {
+// Uniform mode (S11): ghosts = plain prolongation of the parent's arrays at the same time / stage.
+void fill_level_same_time(Seq& q, int level, int n, const int* child_arrays, const int* parent_arrays) {
   sc_hierarchy* h = q.h;
   for (int ib : h->L.level_boxes[level]) {
-    const BoxInfo& b = h->L.boxes[ib];
-    if (level == 0) {
-      prof_begin(h, KIND_PERIODIC, 16.0 * h->L.V * shell_cells(b.v));
-      launch_periodic_fill(b.v, h->L.V, h->slot(ib, sdst), h->stream);
-      prof_end(h);
-      ++q.n;
-      continue;
-    }
+    const int ip = h->L.boxes[ib].parent;
     GhostArgs a{};
-    a.child = b.v;
-    a.parent = h->L.boxes[b.parent].v;
-    a.V = h->L.V;
-    a.dst = h->slot(ib, sdst);
-    a.base = h->slot(b.parent, sparent);
-    a.use_k = 0;
-    a.tiles = h->tiles[ib].dev; a.ntiles = h->tiles[ib].n;
-    a.s0_doubles = h->tiles[ib].s0; a.s1_doubles = h->tiles[ib].s1;
-    for (int j = 0; j < 4; ++j) { a.k[j] = a.base; a.coef[j] = 0.0; }
-    prof_begin(h, KIND_GHOST, 8.0 * h->L.V * (footprint_cells(b.v) + shell_cells(b.v)));
-    launch_ghost_fill(a, h->stream);
-    prof_end(h);
-    ++q.n;
+    a.nsrc = a.nout = n;
+    for (int s = 0; s < n; ++s) {
+      a.src[s] = h->arr(ip, parent_arrays[s]);
+      a.dst[s] = h->arr(ib, child_arrays[s]);
+      a.coef[s][s] = 1.0;
+    }
+    ghost_launch(q, ib, a);
   }
 }
 
@@ -249,68 +292,78 @@ void restrict_level(Seq& q, int level) {  // level -> level-1, into the parents'
   for (int ib : h->L.level_boxes[level]) {
     const BoxInfo& b = h->L.boxes[ib];
     prof_begin(h, KIND_RESTRICT, 8.0 * h->L.V * (cells(b.v) + cells(b.v) / 8.0));
-    launch_restrict(b.v, h->L.boxes[b.parent].v, h->L.V, h->slot(ib, q.cur[level]),
-                    h->slot(b.parent, q.cur[level - 1]), h->stream);
+    launch_restrict(b.v, h->L.boxes[b.parent].v, h->L.V, h->arr(ib, h->L.a_state(q.cur[level])),
+                    h->arr(b.parent, h->L.a_state(q.cur[level - 1])), h->stream);
     prof_end(h);
     ++q.n;
   }
 }
 
-// One RK4 step of one level (eqs 1-9) with its five ghost fills. theta: start of this step inside the
-// parent's step. Slot roles: y_n = cur, Y_2 -> slot 1, Y_3 -> other, Y_4 -> slot 1, y_{n+1} -> other.
-void level_step(Seq& q, int level, double dt, double theta, bool first_fill) {
-  sc_hierarchy* h = q.h;
-  const int yn = q.cur[level], A = 1, B = 2 - yn;
-  const int pyold = level > 0 ? 2 - q.cur[level - 1] : 0;  // the parent already stepped: its y_n is "other"
-  const double hp = 2.0 * dt;
-  const bool has_child = level + 1 < h->L.nlevels;
-  if (first_fill) fill_level_dense(q, level, yn, 1, theta, hp, pyold);
-  rhs_level(q, level, 1, yn, yn, A, 0.5 * dt, true);
-  fill_level_dense(q, level, A, 2, theta, hp, pyold);
-  rhs_level(q, level, 2, A, yn, B, 0.5 * dt, true);
-  fill_level_dense(q, level, B, 3, theta, hp, pyold);
-  rhs_level(q, level, 3, B, yn, A, dt, true);
-  fill_level_dense(q, level, A, 4, theta, hp, pyold);
-  rhs_level(q, level, 4, A, yn, B, dt / 6.0, has_child);
-  fill_level_dense(q, level, B, 5, theta + 0.5, hp, pyold);
-  q.cur[level] = B;
+// One RK4 step of one level (eqs 1-9) with its ghost fills. theta: start of this step inside the parent's.
+void level_step(Seq& q, int level, double dt, double theta) {
+  const Layout& L = q.h->L;
+  const int yn = q.cur[level];
+  if (level == 0) {
+    if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
+  } else {
+    fill_level_dense(q, level, theta, dt);
+  }
+  stage_level(q, level, STAGE_12, dt);
+  if (level == 0) periodic_level0(q, L.a_Y2r(), 2 * L.F);  // Y2r and Y3r are adjacent
+  stage_level(q, level, STAGE_3, dt);
+  stage_level(q, level, STAGE_4, dt);
+  if (level == 0) {
+    periodic_level0(q, L.a_state(1 - yn), L.V);
+    q.l0_valid = true;
+  }
+  q.cur[level] = 1 - yn;
 }
 
 // steps 1-7 of PAPER.md:113-119
-void advance(Seq& q, int level, double dt, double theta, bool first_fill) {
-  level_step(q, level, dt, theta, first_fill);
+void advance(Seq& q, int level, double dt, double theta) {
+  level_step(q, level, dt, theta);
   if (level + 1 < q.h->L.nlevels) {
-    advance(q, level + 1, 0.5 * dt, 0.0, true);
-    // the stage-1 fill at theta = 1/2 would rewrite the values the stage-5 fill at 0 + 1/2 just wrote
-    // (same coefficients b(1/2), same parent data): skipped (reading S8)
-    advance(q, level + 1, 0.5 * dt, 0.5, false);
+    advance(q, level + 1, 0.5 * dt, 0.0);
+    advance(q, level + 1, 0.5 * dt, 0.5);
     restrict_level(q, level + 1);
   }
 }
 
 // non-subcycled step of all levels (reading S11/S15)
 void uniform_step(Seq& q, double dt) {
-  sc_hierarchy* h = q.h;
-  const int Lv = h->L.nlevels;
-  auto role = [&](int level, int which) {  // 0: y_n, 1: A, 2: B
-    return which == 0 ? q.cur[level] : (which == 1 ? 1 : 2 - q.cur[level]);
-  };
-  const double cdt[4] = {0.5 * dt, 0.5 * dt, dt, dt / 6.0};
-  const int yin_role[4] = {0, 1, 2, 1}, yout_role[4] = {1, 2, 1, 2};
-  for (int l = 0; l < Lv; ++l) fill_level_same_time(q, l, role(l, 0), l ? role(l - 1, 0) : 0);
-  for (int s = 1; s <= 4; ++s) {
-    for (int l = 0; l < Lv; ++l)
-      rhs_level(q, l, s, role(l, yin_role[s - 1]), role(l, 0), role(l, yout_role[s - 1]), cdt[s - 1], s < 4);
-    for (int l = 0; l < Lv; ++l)
-      fill_level_same_time(q, l, role(l, yout_role[s - 1]), l ? role(l - 1, yout_role[s - 1]) : 0);
+  const Layout& L = q.h->L;
+  const int Lv = L.nlevels, F = L.F;
+  // ghosts of y_n = (u_n, rho_n): from the parent's y_n after the last restriction
+  if (!q.l0_valid) periodic_level0(q, L.a_state(q.cur[0]), L.V);
+  for (int l = 1; l < Lv; ++l) {
+    const int ca[2] = {L.a_state(q.cur[l]), L.a_state(q.cur[l]) + F};
+    const int pa[2] = {L.a_state(q.cur[l - 1]), L.a_state(q.cur[l - 1]) + F};
+    fill_level_same_time(q, l, 2, ca, pa);
   }
-  for (int l = 0; l < Lv; ++l) q.cur[l] = 2 - q.cur[l];
+  for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_12, dt);
+  // ghosts of Y_{3,u}, Y_{4,u} = P[parent's Y_{3,u}, Y_{4,u}]  <=>  shells of Y2r, Y3r = P[parent's Y2r, Y3r]
+  periodic_level0(q, L.a_Y2r(), 2 * F);
+  for (int l = 1; l < Lv; ++l) {
+    const int ca[2] = {L.a_Y2r(), L.a_Y3r()};
+    fill_level_same_time(q, l, 2, ca, ca);
+  }
+  for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_3, dt);
+  for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_4, dt);
+  // ghosts of y_{n+1} from the parent's y_{n+1} before the restriction
+  periodic_level0(q, L.a_state(1 - q.cur[0]), L.V);
+  q.l0_valid = true;
+  for (int l = 1; l < Lv; ++l) {
+    const int ca[2] = {L.a_state(1 - q.cur[l]), L.a_state(1 - q.cur[l]) + F};
+    const int pa[2] = {L.a_state(1 - q.cur[l - 1]), L.a_state(1 - q.cur[l - 1]) + F};
+    fill_level_same_time(q, l, 2, ca, pa);
+  }
+  for (int l = 0; l < Lv; ++l) q.cur[l] = 1 - q.cur[l];
   for (int l = Lv - 1; l >= 1; --l) restrict_level(q, l);
 }
 
 void record_step(Seq& q, double dt_coarse, int subcycling) {
   if (subcycling) {
-    advance(q, 0, dt_coarse, 0.0, true);
+    advance(q, 0, dt_coarse, 0.0);
   } else {
     const int nsub = 1 << (q.h->L.nlevels - 1);
     for (int i = 0; i < nsub; ++i) uniform_step(q, dt_coarse / (double)nsub);
@@ -406,6 +459,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     if (s > smax) smax = s;
   }
   h->staging_bytes = smax;
+  h->tiles.resize(h->L.boxes.size());
   auto bail = [&](const char* what, cudaError_t e) {
     set_error(std::string(what) + ": " + cudaGetErrorString(e));
     if (h->staging) cudaFree(h->staging);
@@ -422,21 +476,24 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
                          cudaMemcpyHostToDevice, h->stream);
     if (ce != cudaSuccess) return bail("copy coupling", ce);
   }
-  h->tiles.resize(h->L.boxes.size());
   for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
     if (h->L.boxes[ib].level == 0) continue;
     std::vector<GhostTile> tl;
-    size_t s0 = 0, s1 = 0;
-    build_ghost_tiles(h->L.boxes[ib].v, tl, &s0, &s1);
+    build_ghost_tiles(h->L.boxes[ib].v, tl);
     sc_hierarchy::BoxTiles& bt = h->tiles[ib];
-    bt.n = (int)tl.size(); bt.s0 = (int)s0; bt.s1 = (int)s1;
+    bt.n = (int)tl.size();
+    if (tl.empty()) continue;
     if ((ce = cudaMalloc(&bt.dev, sizeof(GhostTile) * tl.size())) != cudaSuccess) return bail("cudaMalloc(tiles)", ce);
     if ((ce = cudaMemcpy(bt.dev, tl.data(), sizeof(GhostTile) * tl.size(), cudaMemcpyHostToDevice)) != cudaSuccess)
       return bail("copy tiles", ce);
   }
+  h->tmaps.resize(h->L.boxes.size());
+  h->tmap_ok.assign(h->L.boxes.size(), 0);
+  for (size_t ib = 0; ib < h->L.boxes.size(); ++ib)
+    h->tmap_ok[ib] = make_box_tensor_map(h->L.boxes[ib].v, h->L.boxes[ib].narrays, h->arr((int)ib, 0), h->tmaps[ib].bytes) ? 1 : 0;
   if ((ce = cudaStreamSynchronize(h->stream)) != cudaSuccess) return bail("sync", ce);
   h->cur.assign(h->L.nlevels, 0);
-  h->ghosts_valid.assign(h->L.nlevels, 0);
+  h->l0_ghosts_valid = false;
   const char* env = getenv("SC_KERNELS");
   select_kernels(env && !strcmp(env, "ref") ? 0 : 1);
   const char* eg = getenv("SC_GRAPH");
@@ -452,7 +509,7 @@ int32_t sc_set_state(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, 
   if (rc != SC_OK) return rc;
   if (!src) { set_error("null src"); return SC_ERR_INVALID_ARG; }
   const BoxView& v = h->L.boxes[gb].v;
-  double* dstarr = h->slot(gb, h->cur[level]) + (long long)comp * v.vol;
+  double* dstarr = h->arr(gb, h->L.a_state(h->cur[level]) + comp);
   const size_t bytes = sizeof(double) * (size_t)v.n[0] * v.n[1] * v.n[2];
   if (src_on_device) {
     launch_unpack(v, src, dstarr, h->stream);
@@ -465,7 +522,7 @@ int32_t sc_set_state(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, 
     SC_CUDA(cudaGetLastError());
     SC_CUDA(cudaStreamSynchronize(h->stream));
   }
-  h->ghosts_valid[level] = 0;
+  if (level == 0) h->l0_ghosts_valid = false;
   return SC_OK;
 }
 
@@ -473,7 +530,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
   if (!h) { set_error("null hierarchy"); return SC_ERR_INVALID_ARG; }
   if (!std::isfinite(dt_coarse) || dt_coarse <= 0.0) { set_error("dt_coarse must be finite and > 0"); return SC_ERR_INVALID_ARG; }
   subcycling = subcycling ? 1 : 0;
-  Seq q{h, h->cur, 0};
+  Seq q{h, h->cur, h->l0_ghosts_valid, 0};
   if (!h->use_graph || h->profiling) {
     record_step(q, dt_coarse, subcycling);
     SC_CUDA(cudaGetLastError());
@@ -482,6 +539,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
     GraphKey key{subcycling, 0, 0};
     memcpy(&key.dt_bits, &dt_coarse, sizeof(double));
     for (int l = 0; l < h->L.nlevels; ++l) key.phase |= (uint32_t)(h->cur[l] ? 1 : 0) << l;
+    if (h->l0_ghosts_valid) key.phase |= 1u << 31;
     auto it = h->graphs.find(key);
     if (it == h->graphs.end()) {
       cudaGraph_t g = nullptr;
@@ -507,7 +565,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
     q.cur = it->second.cur_after;
   }
   h->cur = q.cur;
-  for (auto& gv : h->ghosts_valid) gv = 1;
+  h->l0_ghosts_valid = true;
   h->time += dt_coarse;
   return SC_OK;
 }
@@ -518,8 +576,7 @@ int32_t sc_read_level(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp,
   int rc = check_box(h, level, box, comp, &gb);
   if (rc != SC_OK) return rc;
   if (!dst) { set_error("null dst"); return SC_ERR_INVALID_ARG; }
-  const BoxView& v = h->L.boxes[gb].v;
-  return read_array(h, gb, h->slot(gb, h->cur[level]) + (long long)comp * v.vol, dst, 0, dst_on_device);
+  return read_array(h, gb, h->arr(gb, h->L.a_state(h->cur[level]) + comp), dst, 0, dst_on_device);
 }
 
 double sc_time(const sc_hierarchy* h) { return h ? h->time : 0.0; }
@@ -550,18 +607,22 @@ int32_t sc_debug_read_padded(sc_hierarchy* h, int32_t level, int32_t box, int32_
   int rc = check_box(h, level, box, comp, &gb);
   if (rc != SC_OK) return rc;
   if (!dst) { set_error("null dst"); return SC_ERR_INVALID_ARG; }
-  const BoxView& v = h->L.boxes[gb].v;
-  return read_array(h, gb, h->slot(gb, h->cur[level]) + (long long)comp * v.vol, dst, 1, 0);
+  return read_array(h, gb, h->arr(gb, h->L.a_state(h->cur[level]) + comp), dst, 1, 0);
 }
 
 int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t slot, int32_t comp, double* dst) {
   int gb;
   int rc = check_box(h, level, box, comp, &gb);
   if (rc != SC_OK) return rc;
-  if (!dst || slot < 0 || slot > 4) { set_error("bad slot or null dst"); return SC_ERR_INVALID_ARG; }
-  const BoxView& v = h->L.boxes[gb].v;
-  const int s = slot == 0 ? 2 - h->cur[level] : SLOT_K1 + slot - 1;
-  return read_array(h, gb, h->slot(gb, s) + (long long)comp * v.vol, dst, 0, 0);
+  if (!dst) { set_error("null dst"); return SC_ERR_INVALID_ARG; }
+  const Layout& L = h->L;
+  int a;
+  if (slot == 1) a = L.a_state(1 - h->cur[level]) + comp;
+  else if (slot >= 2 && slot <= 4) {
+    if (comp < L.F) { set_error("stage vectors store the rho components only (comp >= nfields)"); return SC_ERR_INVALID_ARG; }
+    a = (slot == 2 ? L.a_Y2r() : (slot == 3 ? L.a_Y3r() : L.a_Y4r())) + comp - L.F;
+  } else { set_error("slot must be 1 (y_n) or 2..4 (Y_2..Y_4)"); return SC_ERR_INVALID_ARG; }
+  return read_array(h, gb, h->arr(gb, a), dst, 0, 0);
 }
 
 int32_t sc_profile(sc_hierarchy* h, int32_t enable) {

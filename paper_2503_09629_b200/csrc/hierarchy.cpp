@@ -76,7 +76,7 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
     b.v.py = s.n[1] + 2 * g;
     b.v.pz = s.n[2] + 2 * g;
     b.v.plane = (long long)b.v.px * b.v.py;
-    b.v.vol = b.v.plane * b.v.pz;
+    b.v.vol = (long long)round_up((unsigned long long)(b.v.plane * b.v.pz), 32);
     L->level_boxes[s.level].push_back(ib);
     L->boxes.push_back(b);
   }
@@ -117,17 +117,16 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
       }
     }
   }
-  // arena: boxes in order, each NSLOT slots of V arrays; 256-byte aligned pieces
+  // arena: boxes in order, each a run of narrays arrays of vol doubles (sc_internal.h); vol is a multiple
+  // of 32 doubles, so every array starts on a 256-byte boundary
   unsigned long long off = 0;
   for (BoxInfo& b : L->boxes) {
-    b.slot_bytes = round_up((unsigned long long)L->V * (unsigned long long)b.v.vol * sizeof(double), 256);
+    b.narrays = 2 * L->V + 3 * L->F + (L->has_coupling ? 2 * L->F : 0);
     b.arena_offset = off;
-    off += (unsigned long long)NSLOT * b.slot_bytes;
+    off += (unsigned long long)b.narrays * (unsigned long long)b.v.vol * sizeof(double);
   }
   L->coupling_offset = off;
   off += round_up((unsigned long long)L->F * L->F * sizeof(double), 256);
-  L->scratch_offset = off;
-  off += 4096;  // small scratch (debug maps are allocated separately)
   L->arena_bytes = off;
   return SC_OK;
 }

@@ -1,4 +1,4 @@
-// kernels.h — launch interface between the level scheduler and the CUDA kernels.
+// kernels.h — launch interface between the level scheduler (capi.cu) and the CUDA kernels.
 #ifndef SC_KERNELS_H_
 #define SC_KERNELS_H_
 
@@ -8,31 +8,52 @@
 
 namespace sc {
 
-// a1 / a2: k_s = f(Y_s) on the interior fused with the RK4 stage combine.
-//   stage 1..3:  k_s = f(Yin);  Yout = yn + cdt * k_s          (cdt = a_s * dt; eqs 1-3, 7-9)
-//   stage 4:     k_4 = f(Yin);  Yout = yn + cdt * (k1 + 2 k2 + 2 k3 + k4)   (cdt = dt/6; eqs 4-5)
-// f: k_u = rho, k_rho = Lap_h u + A u. All pointers are slot bases (V arrays).
-struct RhsArgs {
+// ------------------------------------------------------------------------------------------------
+// a1 / a2: the four RHS evaluations of one RK4 level-step (eqs 1-9) fused with
+// the stage combines, for  d_t u = rho,  d_t rho = Lap_h u + A u =: L u. Written on
+// the stored quantities (u_n, rho_n, Y2r, Y3r, Y4r) — see sc_internal.h and DESIGN.md S26:
+//   STAGE_12  (k_1, k_2):  Y2r = rho_n + dt/2 L u_n                       (k_{1,rho} = L u_n, eq 7)
+//                          Y3r = rho_n + dt/2 L (u_n + dt/2 rho_n)        (k_{2,rho} = L Y_{2,u}, eq 8)
+//   STAGE_3   (k_3):       Y4r = rho_n + dt   L (u_n + dt/2 Y2r)          (k_{3,rho} = L Y_{3,u}, eq 9)
+//   STAGE_4   (k_4, eq 5): k4r   = L (u_n + dt Y3r)
+//                          u_new   = u_n + dt/6 (rho_n + 2 Y2r + 2 Y3r + Y4r)
+//                          rho_new = rho_n + (Y2r-rho_n)/3 + 2 (Y3r-rho_n)/3 + (Y4r-rho_n)/3 + dt/6 k4r
+// Inputs marked (h) are read with their ghost cells (2 layers); everything is written on the interior only.
+// ------------------------------------------------------------------------------------------------
+enum { STAGE_12 = 0, STAGE_3 = 1, STAGE_4 = 2 };
+
+struct StageArgs {
   BoxView b;
   int F;
-  int stage;
-  const double* Yin;
-  const double* yn;
-  double* kout;       // k_s (may be null at stage 4 when no child level needs k_4)
-  double* Yout;       // Y_{s+1} or y_{n+1}
-  const double* k1;
-  const double* k2;
-  const double* k3;
-  double cdt;
-  double inv12dx2[3];
-  const double* A;    // device F*F or null
+  int mode;
+  const double* yn;    // (h) state slot of y_n: u_f at f*vol, rho_f at (F+f)*vol
+  const double* R;     // (h) F arrays: STAGE_12 -> rho_n (= yn + F*vol); STAGE_3 -> Y2r; STAGE_4 -> Y3r
+  const double* Y2r;   // STAGE_4 only, interior
+  const double* Y4r;   // STAGE_4 only, interior
+  double* out0;        // STAGE_12: Y2r;  STAGE_3: Y4r;  STAGE_4: state slot of y_{n+1}
+  double* out1;        // STAGE_12: Y3r
+  double dt;
+  double inv12dx2[3];  // 1 / (12 dx_a^2)
+  const double* A;     // device F*F row-major coupling, or null
+  double* scratch;     // 2F arrays (only when A != null): A u_n and A R of this stage
+  // TMA path: tensor map of the box (all arrays as the 4th dimension) and the array indices of yn / R
+  const void* tmap;    // host pointer to the box's CUtensorMap, or null -> direct-load kernel
+  int a_yn, a_R;
 };
-void launch_rhs_stage(const RhsArgs& a, cudaStream_t st);
+void launch_stage(const StageArgs& a, cudaStream_t st);
+// 128-byte CUtensorMap of a box: dims (px, py, pz, narrays), fp64, no swizzle. Returns false (and leaves the
+// direct-load kernel in charge) when the driver entry point is unavailable or the box violates a TMA limit.
+bool make_box_tensor_map(const BoxView& b, int narrays, void* base, void* out_map128);
 
-// a3: dense-output + prolongation ghost fill of a level >= 1 box:
-//   ghost(dst) = P[ base + sum_j coef[j] * k[j] ]  over the parent's cells, P = 5x5x5 tensor Lagrange.
-// coef[j] already contains the parent step h_p (coef = h_p * c_j(stage, theta)); nk = number of leading
-// k arrays with a non-zero coefficient pattern (0 = pure prolongation of base).
+// ------------------------------------------------------------------------------------------------
+// a3: refinement-boundary ghost fill. For every ghost cell of a level >= 1 box and every output o:
+//     dst[o](ghost) = P[ sum_s coef[o][s] * src[s] ]     P = 5x5x5 tensor quartic Lagrange (S3)
+// over parent arrays src[s]. The dense-output time polynomial (eqs 10-18) is folded into coef by the
+// scheduler, which asks for all ghost shells one child level-step needs in ONE launch. Field f of every
+// src/dst is f arrays further (src[s] + f*parent.vol, dst[o] + f*child.vol).
+// ------------------------------------------------------------------------------------------------
+constexpr int GF_MAX_SRC = 7, GF_MAX_OUT = 6;
+
 struct GhostTile {   // a piece of one ghost slab, box-local fine indices
   int lo[3];
   int n[3];
@@ -42,23 +63,21 @@ struct GhostTile {   // a piece of one ghost slab, box-local fine indices
 
 struct GhostArgs {
   BoxView child, parent;
-  int V;
-  double* dst;          // child slot base
-  const double* base;   // parent y_old (subcycled) or the parent's same-stage buffer (uniform)
-  const double* k[4];   // parent k_1..k_4 slot bases
-  double coef[4];
-  int use_k;            // bit j set -> k[j] is read
+  int F;
+  int nsrc, nout;
+  const double* src[GF_MAX_SRC];
+  double* dst[GF_MAX_OUT];
+  double coef[GF_MAX_OUT][GF_MAX_SRC];
   const GhostTile* tiles;  // device; tile list of the child box (built once per box)
   int ntiles;
-  int s0_doubles, s1_doubles;  // shared-memory staging sizes the tile list needs
 };
-void build_ghost_tiles(const BoxView& child, std::vector<GhostTile>& tiles, size_t* s0_doubles, size_t* s1_doubles);
+void build_ghost_tiles(const BoxView& child, std::vector<GhostTile>& tiles);
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st);
 
-// a4: periodic ghost fill of the level-0 box (reading S9).
-void launch_periodic_fill(const BoxView& b, int V, double* y, cudaStream_t st);
+// a4: periodic ghost fill of `narrays` consecutive arrays of the level-0 box (reading S9).
+void launch_periodic_fill(const BoxView& b, int narrays, double* y, cudaStream_t st);
 
-// a5: restriction child -> parent (reading S4).
+// a5: restriction child -> parent of V consecutive arrays (reading S4).
 void launch_restrict(const BoxView& child, const BoxView& parent, int V, const double* ychild,
                      double* yparent, cudaStream_t st);
 
@@ -66,7 +85,7 @@ void launch_restrict(const BoxView& child, const BoxView& parent, int V, const d
 void launch_pack(const BoxView& b, const double* padded, double* dense, int with_ghosts, cudaStream_t st);
 void launch_unpack(const BoxView& b, const double* dense, double* padded, cudaStream_t st);
 
-// debug: ghost index map with the same device index arithmetic as the ghost kernel
+// debug: ghost index map with the same device index arithmetic as the ghost kernels
 void launch_ghost_map(const BoxView& child, const BoxView& parent, int* out, cudaStream_t st);
 long long ghost_cell_count(const BoxView& b);
 

@@ -1,6 +1,7 @@
-// kernels_ref.cu — first, straightforward CUDA kernels of every step of the hot path (one thread per
-// output cell, gathers straight from global memory). They define the arithmetic of the CUDA path; the
-// tuned kernels in kernels_opt.cu must agree with them to rounding. Selected with SC_KERNELS=ref.
+// kernels_basic.cu — straightforward CUDA kernels of every step of the hot path (one thread per output
+// cell, gathers straight from global memory). They define the arithmetic of the CUDA path; the tuned
+// kernels (stage_tma.cu, ghost_tiled.cu, restrict_zmarch.cu) must agree with them to rounding. Selected
+// with SC_KERNELS=ref; also the home of the periodic fill, pack/unpack and the ghost-map debug kernel.
 //
 // Index conventions: box-local cell (i,j,k), i fastest; level-global index I = lo + i; the parent cell
 // containing fine cell I is I >> 1 (arithmetic shift = floor), its parity I & 1 (1: fine centre at
@@ -70,9 +71,27 @@ __device__ inline bool shell_cell(const BoxView& b, long long q, int& i, int& j,
 }
 
 // ------------------------------------------------------------------------------------------------
-// a1/a2  rhs + stage combine
+// a1/a2  the RK4 stage kernels, direct-load version: one thread per interior cell, every operand read
+// straight from global memory. Defines the arithmetic of the stage kernels (kernels.h); the TMA kernels
+// in stage_tma.cu must agree with it to rounding. Used for SC_KERNELS=ref and for boxes the TMA path
+// does not take.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) rhs_stage_ref(RhsArgs a) {
+namespace {
+// 13-point 4th-order Laplacian of W = u + c r at one cell (S2); c == 0 -> r is not read
+template <bool WITH_R>
+__device__ __forceinline__ double lap_w(const double* u, const double* r, double c, long long sy, long long sz,
+                                        const double w[3], double* centre) {
+  auto W = [&](long long d) { return WITH_R ? fma(c, r[d], u[d]) : u[d]; };
+  const double wc = W(0);
+  *centre = wc;
+  const double dxx = (-W(-2) + 16.0 * W(-1) - 30.0 * wc + 16.0 * W(1) - W(2)) * w[0];
+  const double dyy = (-W(-2 * sy) + 16.0 * W(-sy) - 30.0 * wc + 16.0 * W(sy) - W(2 * sy)) * w[1];
+  const double dzz = (-W(-2 * sz) + 16.0 * W(-sz) - 30.0 * wc + 16.0 * W(sz) - W(2 * sz)) * w[2];
+  return dxx + dyy + dzz;
+}
+}  // namespace
+
+__global__ void __launch_bounds__(256) stage_direct(StageArgs a) {
   const BoxView& b = a.b;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -80,53 +99,55 @@ __global__ void __launch_bounds__(256) rhs_stage_ref(RhsArgs a) {
   const int f = blockIdx.z / b.n[2];
   if (i >= b.n[0] || j >= b.n[1]) return;
   const long long o = cell_offset(b, i, j, k);
-  const long long sx = 1, sy = b.px, sz = b.plane;
-  const double* u = a.Yin + (long long)f * b.vol + o;
-  const double* r = a.Yin + (long long)(a.F + f) * b.vol + o;
-  const double uc = u[0];
-  const double dxx = (-u[-2 * sx] + 16.0 * u[-sx] - 30.0 * uc + 16.0 * u[sx] - u[2 * sx]) * a.inv12dx2[0];
-  const double dyy = (-u[-2 * sy] + 16.0 * u[-sy] - 30.0 * uc + 16.0 * u[sy] - u[2 * sy]) * a.inv12dx2[1];
-  const double dzz = (-u[-2 * sz] + 16.0 * u[-sz] - 30.0 * uc + 16.0 * u[sz] - u[2 * sz]) * a.inv12dx2[2];
-  double src = 0.0;
-  if (a.A)
-    for (int q = 0; q < a.F; ++q) src += a.A[f * a.F + q] * a.Yin[(long long)q * b.vol + o];
-  const double ku = r[0];
-  const double kr = dxx + dyy + dzz + src;
-  const long long ou = (long long)f * b.vol + o, orr = (long long)(a.F + f) * b.vol + o;
-  if (a.kout) {
-    a.kout[ou] = ku;
-    a.kout[orr] = kr;
-  }
-  if (a.stage < 4) {
-    a.Yout[ou] = a.yn[ou] + a.cdt * ku;
-    a.Yout[orr] = a.yn[orr] + a.cdt * kr;
+  const long long sy = b.px, sz = b.plane;
+  const int F = a.F;
+  const double* u = a.yn + (long long)f * b.vol + o;
+  const double* r = a.R + (long long)f * b.vol + o;
+  const double rho = a.yn[(long long)(F + f) * b.vol + o];
+  const double dt = a.dt;
+  // coupling  sum_j A_fj W_j  at this cell
+  auto couple = [&](double c) {
+    double s = 0.0;
+    if (a.A)
+      for (int q = 0; q < F; ++q) {
+        const double wq = fma(c, a.R[(long long)q * b.vol + o], a.yn[(long long)q * b.vol + o]);
+        s = fma(a.A[f * F + q], wq, s);
+      }
+    return s;
+  };
+  double wc;
+  if (a.mode == STAGE_12) {
+    double Lu = lap_w<false>(u, r, 0.0, sy, sz, a.inv12dx2, &wc);
+    if (a.A)
+      for (int q = 0; q < F; ++q) Lu = fma(a.A[f * F + q], a.yn[(long long)q * b.vol + o], Lu);
+    const double L2 = lap_w<true>(u, r, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt);
+    a.out0[(long long)f * b.vol + o] = fma(0.5 * dt, Lu, rho);
+    a.out1[(long long)f * b.vol + o] = fma(0.5 * dt, L2, rho);
+  } else if (a.mode == STAGE_3) {
+    const double L3 = lap_w<true>(u, r, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt);
+    a.out0[(long long)f * b.vol + o] = fma(dt, L3, rho);
   } else {
-    a.Yout[ou] = a.yn[ou] + a.cdt * (a.k1[ou] + 2.0 * a.k2[ou] + 2.0 * a.k3[ou] + ku);
-    a.Yout[orr] = a.yn[orr] + a.cdt * (a.k1[orr] + 2.0 * a.k2[orr] + 2.0 * a.k3[orr] + kr);
+    const double k4r = lap_w<true>(u, r, dt, sy, sz, a.inv12dx2, &wc) + couple(dt);
+    const double y2 = a.Y2r[(long long)f * b.vol + o], y3 = r[0], y4 = a.Y4r[(long long)f * b.vol + o];
+    const double third = 1.0 / 3.0;
+    a.out0[(long long)f * b.vol + o] = fma(dt / 6.0, (rho + y4) + 2.0 * (y2 + y3), u[0]);
+    a.out0[(long long)(F + f) * b.vol + o] =
+        rho + (third * ((y2 - rho) + (y4 - rho)) + (2.0 * third) * (y3 - rho)) + (dt / 6.0) * k4r;
   }
 }
 
-void launch_rhs_stage_ref(const RhsArgs& a, cudaStream_t st) {
+void launch_stage_direct(const StageArgs& a, cudaStream_t st) {
   dim3 blk(64, 4, 1);
   dim3 grd((a.b.n[0] + 63) / 64, (a.b.n[1] + 3) / 4, a.b.n[2] * a.F);
-  rhs_stage_ref<<<grd, blk, 0, st>>>(a);
+  stage_direct<<<grd, blk, 0, st>>>(a);
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3  dense output + prolongation, one thread per ghost cell, 125-point gather
+// a3  ghost fill, direct version: one thread per (ghost cell, field), 125-point gather per source
 // ------------------------------------------------------------------------------------------------
-__device__ inline double combine_parent(const GhostArgs& a, long long off) {
-  double v = a.base[off];
-  if (a.use_k & 1) v += a.coef[0] * a.k[0][off];
-  if (a.use_k & 2) v += a.coef[1] * a.k[1][off];
-  if (a.use_k & 4) v += a.coef[2] * a.k[2][off];
-  if (a.use_k & 8) v += a.coef[3] * a.k[3][off];
-  return v;
-}
-
-__global__ void __launch_bounds__(128) ghost_fill_ref(GhostArgs a, long long nshell) {
+__global__ void __launch_bounds__(128) ghost_fill_direct(GhostArgs a, long long nshell) {
   const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const int c = blockIdx.y;
+  const int f = blockIdx.y;
   if (q >= nshell) return;
   int i, j, k;
   if (!shell_cell(a.child, q, i, j, k)) return;
@@ -137,26 +158,41 @@ __global__ void __launch_bounds__(128) ghost_fill_ref(GhostArgs a, long long nsh
     J[d] = (I[d] >> 1) - a.parent.lo[d];
     p[d] = I[d] & 1;
   }
-  const long long pv = (long long)c * a.parent.vol;
-  double sz = 0.0;
-  for (int cc = -2; cc <= 2; ++cc) {
-    double sy = 0.0;
-    for (int bb = -2; bb <= 2; ++bb) {
-      double sx = 0.0;
-      const long long row = pv + cell_offset(a.parent, J[0], J[1] + bb, J[2] + cc);
+  const long long pv = (long long)f * a.parent.vol;
+  double acc[GF_MAX_OUT];
 #pragma unroll
-      for (int aa = -2; aa <= 2; ++aa) sx += c_wp[p[0]][aa + 2] * combine_parent(a, row + aa);
-      sy += c_wp[p[1]][bb + 2] * sx;
+  for (int o = 0; o < GF_MAX_OUT; ++o) acc[o] = 0.0;
+  for (int cc = -2; cc <= 2; ++cc)
+    for (int bb = -2; bb <= 2; ++bb) {
+      const long long row = pv + cell_offset(a.parent, J[0], J[1] + bb, J[2] + cc);
+      const double wyz = c_wp[p[1]][bb + 2] * c_wp[p[2]][cc + 2];
+      for (int aa = -2; aa <= 2; ++aa) {
+        const double w = wyz * c_wp[p[0]][aa + 2];
+        double v[GF_MAX_SRC];
+#pragma unroll
+        for (int s = 0; s < GF_MAX_SRC; ++s) v[s] = s < a.nsrc ? a.src[s][row + aa] : 0.0;
+#pragma unroll
+        for (int o = 0; o < GF_MAX_OUT; ++o) {
+          if (o < a.nout) {
+            double t = 0.0;
+#pragma unroll
+            for (int s = 0; s < GF_MAX_SRC; ++s)
+              if (s < a.nsrc) t = fma(a.coef[o][s], v[s], t);
+            acc[o] = fma(w, t, acc[o]);
+          }
+        }
+      }
     }
-    sz += c_wp[p[2]][cc + 2] * sy;
-  }
-  a.dst[(long long)c * a.child.vol + cell_offset(a.child, i, j, k)] = sz;
+  const long long dofs = (long long)f * a.child.vol + cell_offset(a.child, i, j, k);
+#pragma unroll
+  for (int o = 0; o < GF_MAX_OUT; ++o)
+    if (o < a.nout) a.dst[o][dofs] = acc[o];
 }
 
-void launch_ghost_fill_ref(const GhostArgs& a, cudaStream_t st) {
+void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st) {
   const long long ns = ghost_cell_count(a.child);
-  dim3 grd((unsigned)((ns + 127) / 128), a.V, 1);
-  ghost_fill_ref<<<grd, 128, 0, st>>>(a, ns);
+  dim3 grd((unsigned)((ns + 127) / 128), a.F, 1);
+  ghost_fill_direct<<<grd, 128, 0, st>>>(a, ns);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -173,7 +209,7 @@ __global__ void __launch_bounds__(128) periodic_fill_ref(BoxView b, double* y, l
   a[cell_offset(b, i, j, k)] = a[cell_offset(b, wrap(i, b.n[0]), wrap(j, b.n[1]), wrap(k, b.n[2]))];
 }
 
-void launch_periodic_fill_ref(const BoxView& b, int V, double* y, cudaStream_t st) {
+void launch_periodic_fill(const BoxView& b, int V, double* y, cudaStream_t st) {
   const long long ns = ghost_cell_count(b);
   dim3 grd((unsigned)((ns + 127) / 128), V, 1);
   periodic_fill_ref<<<grd, 128, 0, st>>>(b, y, ns);

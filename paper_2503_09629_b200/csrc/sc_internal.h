@@ -1,13 +1,21 @@
 // sc_internal.h — internal types of libsubcycle (not part of the ABI).
 //
-// Data layout in HBM: every box owns NSLOT = 7 slots; a slot holds the
-// V = 2F component arrays of the box back to back; a component array is the box padded by g ghost
-// cells, stored [z][y][x] with x contiguous:
+// Data layout in HBM. A box owns a run of equally sized ARRAYS; an array is one
+// scalar grid function on the box padded by g ghost cells, stored [z][y][x] with x contiguous:
 //     offset(i,j,k) = (XOFF + i) + px * ((j + g) + py * (k + g)),   i in [-g, n0+g) etc.
-// XOFF = 4 doubles puts interior cell i = 0 on a 32-byte sector boundary; px is a multiple of 16
-// doubles so every row starts on a 128-byte line. Slots 0..2 rotate between the roles y / Y_even /
-// y_old (PAPER.md:54-75 needs y_n, one stage vector being read and one being written); slots 3..6
-// hold k_1..k_4, which the child level reads for its dense-output ghost fill ("Store k").
+// XOFF = 4 doubles puts interior cell i = 0 on a 32-byte sector boundary; px is a multiple of 16 doubles so
+// every row starts on a 128-byte line (and every TMA global stride is a multiple of 16 bytes).
+// Arrays of a box, in order (F = number of fields, V = 2F):
+//     [0, V)            state slot 0:  u_0..u_{F-1}, rho_0..rho_{F-1}
+//     [V, 2V)           state slot 1   (slots 0/1 alternate between y_n and y_{n+1})
+//     [2V, 2V+F)        Y2r = rho-part of the stage vector Y_2 (eq 7)
+//     [2V+F, 2V+2F)     Y3r = rho-part of Y_3 (eq 8)
+//     [2V+2F, 2V+3F)    Y4r = rho-part of Y_4 (eq 9)
+//     [2V+3F, 2V+5F)    only if a coupling matrix is set: scratch for A*u_n and A*R of the current stage
+// The u-parts of the stage vectors and the slopes k_1..k_4 are never materialised (S26): for
+// d_t u = rho the slope k_{s,u} IS Y_{s,rho}, so Y_{s+1,u} = u_n + a_s dt Y_{s,rho} is rebuilt where it is
+// needed, and k_{s,rho} = (Y_{s+1,rho} - rho_n)/(a_s dt). After a level-step the child level reads
+// (u_n, rho_n, Y2r, Y3r, Y4r) of its parent for the dense-output ghost fill ("Store k").
 #ifndef SC_INTERNAL_H_
 #define SC_INTERNAL_H_
 
@@ -29,8 +37,6 @@ namespace sc {
 constexpr int XOFF = 4;        // doubles of left padding in x (>= max ghost width)
 constexpr int MAX_GHOST = 4;
 constexpr int MIN_GHOST = 2;   // stencil radius of the 4th-order Laplacian; restriction reads 2 layers
-constexpr int NSLOT = 7;       // 3 rotating state buffers + k1..k4
-constexpr int SLOT_K1 = 3;
 constexpr int MAX_FIELDS = 32;
 
 // Geometry of one box's arrays; passed by value to kernels.
@@ -42,7 +48,7 @@ struct BoxView {
   int py;          // rows per plane  = n[1] + 2g
   int pz;          // planes          = n[2] + 2g
   long long plane; // px * py
-  long long vol;   // doubles per component array = px * py * pz (multiple of 32)
+  long long vol;   // doubles per array = px * py * pz (multiple of 32)
 };
 
 SC_HD inline long long cell_offset(const BoxView& b, int i, int j, int k) {
@@ -53,9 +59,9 @@ struct BoxInfo {
   BoxView v;
   int level;
   int index_in_level;
-  int parent;            // global box index on level-1, or -1
-  unsigned long long arena_offset;  // bytes, start of slot 0
-  unsigned long long slot_bytes;    // bytes of one slot (V arrays)
+  int parent;                       // global box index on level-1, or -1
+  unsigned long long arena_offset;  // bytes, start of array 0
+  int narrays;                      // arrays this box owns
 };
 
 struct Layout {
@@ -65,10 +71,15 @@ struct Layout {
   std::vector<BoxInfo> boxes;
   std::vector<std::vector<int>> level_boxes;
   unsigned long long coupling_offset = 0;   // bytes into the arena (F*F doubles) if has_coupling
-  unsigned long long scratch_offset = 0;
   unsigned long long arena_bytes = 0;
   bool has_coupling = false;
   double dx(int level, int a) const { return (xhi[a] - xlo[a]) / ((double)domain[a] * (double)(1u << level)); }
+  // first array index of each role
+  int a_state(int slot) const { return slot * V; }
+  int a_Y2r() const { return 2 * V; }
+  int a_Y3r() const { return 2 * V + F; }
+  int a_Y4r() const { return 2 * V + 2 * F; }
+  int a_scratch() const { return 2 * V + 3 * F; }
 };
 
 // Validate a description and compute the layout. Host only, no CUDA calls.

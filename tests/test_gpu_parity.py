@@ -78,12 +78,23 @@ def test_single_level_step_and_slopes():
         G.sc_step(w.dt_coarse, sub)
         O.step(w.dt_coarse, sub)
         _compare_state(G, O, w, what=f"single level sub={sub}")
-    for slot in range(0, 4):  # y_old, k1..k3 (k4 is not stored on a level without children)
-        for c in range(w.ncomp):
-            a = G.sc_debug_read_slot(0, 0, slot, c)
-            b = O.read(0, 0, c, slot=slot + 1)
-            s = max(np.max(np.abs(b)), 1e-300)
-            assert np.max(np.abs(a - b)) <= RTOL * s, (slot, c)
+    _compare_stored_stages(G, O, w, 0, 0, w.dt_coarse)
+
+
+def _compare_stored_stages(G, O, w, level, ib, dt):
+    """What the CUDA path keeps of a level-step (S26): y_n and the rho-parts of Y_2, Y_3, Y_4, against
+    the oracle's y_old and Y_{s+1,rho} = rho_n + a_s dt k_{s,rho} (eqs 7-9) built from its stored slopes."""
+    F = w.nfields
+    for c in range(w.ncomp):
+        a, b = G.sc_debug_read_slot(level, ib, 1, c), O.read(level, ib, c, slot=O.SLOT_YOLD)
+        assert np.max(np.abs(a - b)) <= RTOL * max(np.max(np.abs(b)), 1e-300), ("y_n", c)
+    for s, a_s in ((2, 0.5), (3, 0.5), (4, 1.0)):
+        for f in range(F):
+            b = O.read(level, ib, F + f, slot=O.SLOT_YOLD) + a_s * dt * O.read(level, ib, F + f, slot=O.SLOT_K1 + s - 2)
+            a = G.sc_debug_read_slot(level, ib, s, F + f)
+            assert np.max(np.abs(a - b)) <= RTOL * max(np.max(np.abs(b)), 1e-300), (s, f)
+    with pytest.raises(sc.SubcycleError):
+        G.sc_debug_read_slot(level, ib, 2, 0)  # the u-part of a stage vector is never stored
 
 
 @pytest.mark.parametrize("sub", [True, False])
@@ -96,12 +107,8 @@ def test_two_level_one_step_ghosts_slopes_restriction(sub):
     O.step(w.dt_coarse, sub)
     _compare_state(G, O, w, what=f"cfg1 one step sub={sub}")
     if sub:
-        for slot in range(0, 5):
-            for c in range(2):
-                a = G.sc_debug_read_slot(0, 0, slot, c)
-                b = O.read(0, 0, c, slot=slot + 1)
-                s = max(np.max(np.abs(b)), 1e-300)
-                assert np.max(np.abs(a - b)) <= RTOL * s, (slot, c)
+        _compare_stored_stages(G, O, w, 0, 0, w.dt_coarse)
+        _compare_stored_stages(G, O, w, 1, 0, w.dt_coarse / 2)
 
 
 @pytest.mark.parametrize("sub", [True, False])
