@@ -116,6 +116,7 @@ struct Seq {
   std::vector<int> cur;  // working copy of the state-slot phases
   bool l0_valid;         // working copy of l0_ghosts_valid
   uint64_t n = 0;
+  bool sub = true;       // subcycled mode (parents keep k_4 for their children)
 };
 
 enum { KIND_STAGE = 0, KIND_GHOST = 1, KIND_PERIODIC = 2, KIND_RESTRICT = 3, NKIND = 4 };
@@ -138,10 +139,9 @@ double footprint_cells(const BoxView& v) {  // parent cells a ghost fill of this
   }
   return outer - inner;
 }
-double stage_bytes(const BoxView& v, int F, int mode) {
-  // STAGE_12: read u_n, rho_n; write Y2r, Y3r.  STAGE_3: read u_n, Y2r, rho_n; write Y4r.
-  // STAGE_4: read u_n, Y3r, rho_n, Y2r, Y4r; write u_new, rho_new.
-  const double per = mode == STAGE_4 ? 7.0 : 4.0;
+double stage_bytes(const BoxView& v, int F, int mode, int write_Y4r) {
+  // STAGE_12: read u_n, rho_n; write Y2r, Y3r.  STAGE_34: read u_n, rho_n, Y2r, Y3r; write u_new, rho_new [, Y4r].
+  const double per = mode == STAGE_12 ? 4.0 : (write_Y4r ? 7.0 : 6.0);
   return 8.0 * per * F * cells(v);
 }
 
@@ -168,23 +168,24 @@ void stage_level(Seq& q, int level, int mode, double dt) {
     a.b = L.boxes[ib].v;
     a.F = L.F;
     a.mode = mode;
+    // the slope k_4 (= Y4r) is kept only where a child level reads it for its dense-output ghosts
+    a.write_Y4r = (q.sub && level + 1 < L.nlevels) ? 1 : 0;
     a.a_yn = L.a_state(yn);
+    a.a_Y2r = L.a_Y2r();
+    a.a_Y3r = L.a_Y3r();
     a.yn = h->arr(ib, a.a_yn);
-    a.a_R = mode == STAGE_12 ? L.a_state(yn) + L.F : (mode == STAGE_3 ? L.a_Y2r() : L.a_Y3r());
-    a.R = h->arr(ib, a.a_R);
     a.Y2r = h->arr(ib, L.a_Y2r());
+    a.Y3r = h->arr(ib, L.a_Y3r());
     a.Y4r = h->arr(ib, L.a_Y4r());
-    a.out0 = mode == STAGE_12 ? h->arr(ib, L.a_Y2r()) : (mode == STAGE_3 ? h->arr(ib, L.a_Y4r()) : h->arr(ib, L.a_state(ynew)));
-    a.out1 = h->arr(ib, L.a_Y3r());
+    a.ynew = h->arr(ib, L.a_state(ynew));
     a.dt = dt;
     for (int d = 0; d < 3; ++d) {
       const double dx = L.dx(level, d);
       a.inv12dx2[d] = 1.0 / (12.0 * dx * dx);
     }
     a.A = h->coupling();
-    a.scratch = L.has_coupling ? h->arr(ib, L.a_scratch()) : nullptr;
     a.tmap = h->tmap_ok[ib] ? h->tmaps[ib].bytes : nullptr;
-    prof_begin(h, KIND_STAGE, stage_bytes(a.b, L.F, mode));
+    prof_begin(h, KIND_STAGE, stage_bytes(a.b, L.F, mode, a.write_Y4r));
     launch_stage(a, h->stream);
     prof_end(h);
     ++q.n;
@@ -310,8 +311,7 @@ void level_step(Seq& q, int level, double dt, double theta) {
   }
   stage_level(q, level, STAGE_12, dt);
   if (level == 0) periodic_level0(q, L.a_Y2r(), 2 * L.F);  // Y2r and Y3r are adjacent
-  stage_level(q, level, STAGE_3, dt);
-  stage_level(q, level, STAGE_4, dt);
+  stage_level(q, level, STAGE_34, dt);
   if (level == 0) {
     periodic_level0(q, L.a_state(1 - yn), L.V);
     q.l0_valid = true;
@@ -347,8 +347,7 @@ void uniform_step(Seq& q, double dt) {
     const int ca[2] = {L.a_Y2r(), L.a_Y3r()};
     fill_level_same_time(q, l, 2, ca, ca);
   }
-  for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_3, dt);
-  for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_4, dt);
+  for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_34, dt);
   // ghosts of y_{n+1} from the parent's y_{n+1} before the restriction
   periodic_level0(q, L.a_state(1 - q.cur[0]), L.V);
   q.l0_valid = true;
@@ -362,6 +361,7 @@ void uniform_step(Seq& q, double dt) {
 }
 
 void record_step(Seq& q, double dt_coarse, int subcycling) {
+  q.sub = subcycling != 0;
   if (subcycling) {
     advance(q, 0, dt_coarse, 0.0);
   } else {

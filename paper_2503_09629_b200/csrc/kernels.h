@@ -11,38 +11,41 @@ namespace sc {
 // ------------------------------------------------------------------------------------------------
 // a1 / a2: the four RHS evaluations of one RK4 level-step (eqs 1-9) fused with
 // the stage combines, for  d_t u = rho,  d_t rho = Lap_h u + A u =: L u. Written on
-// the stored quantities (u_n, rho_n, Y2r, Y3r, Y4r) — see sc_internal.h and DESIGN.md S26:
+// the stored quantities (u_n, rho_n, Y2r, Y3r, Y4r) — see sc_internal.h and DESIGN.md S26. Because
+// k_{s,u} = Y_{s,rho}, the stage vectors Y_3 and Y_4 depend on Y_2 only through arrays the FIRST kernel
+// already produced, so one level-step is TWO launches:
 //   STAGE_12  (k_1, k_2):  Y2r = rho_n + dt/2 L u_n                       (k_{1,rho} = L u_n, eq 7)
 //                          Y3r = rho_n + dt/2 L (u_n + dt/2 rho_n)        (k_{2,rho} = L Y_{2,u}, eq 8)
-//   STAGE_3   (k_3):       Y4r = rho_n + dt   L (u_n + dt/2 Y2r)          (k_{3,rho} = L Y_{3,u}, eq 9)
-//   STAGE_4   (k_4, eq 5): k4r   = L (u_n + dt Y3r)
-//                          u_new   = u_n + dt/6 (rho_n + 2 Y2r + 2 Y3r + Y4r)
+//   STAGE_34  (k_3, k_4):  Y4r = rho_n + dt   L (u_n + dt/2 Y2r)          (k_{3,rho} = L Y_{3,u}, eq 9)
+//                          k4r   = L (u_n + dt Y3r)                       (k_{4,rho} = L Y_{4,u})
+//                          u_new   = u_n + dt/6 (rho_n + 2 Y2r + 2 Y3r + Y4r)                       (eq 5)
 //                          rho_new = rho_n + (Y2r-rho_n)/3 + 2 (Y3r-rho_n)/3 + (Y4r-rho_n)/3 + dt/6 k4r
-// Inputs marked (h) are read with their ghost cells (2 layers); everything is written on the interior only.
+// Inputs marked (h) are read with 2 ghost layers; everything is written on the interior only. Y4r is
+// stored only when a child level needs it for its dense-output ghost fill (write_Y4r).
 // ------------------------------------------------------------------------------------------------
-enum { STAGE_12 = 0, STAGE_3 = 1, STAGE_4 = 2 };
+enum { STAGE_12 = 0, STAGE_34 = 1 };
 
 struct StageArgs {
   BoxView b;
   int F;
   int mode;
-  const double* yn;    // (h) state slot of y_n: u_f at f*vol, rho_f at (F+f)*vol
-  const double* R;     // (h) F arrays: STAGE_12 -> rho_n (= yn + F*vol); STAGE_3 -> Y2r; STAGE_4 -> Y3r
-  const double* Y2r;   // STAGE_4 only, interior
-  const double* Y4r;   // STAGE_4 only, interior
-  double* out0;        // STAGE_12: Y2r;  STAGE_3: Y4r;  STAGE_4: state slot of y_{n+1}
-  double* out1;        // STAGE_12: Y3r
+  int write_Y4r;
+  const double* yn;    // (h) state slot of y_n: u_f at f*vol (h), rho_f at (F+f)*vol ((h) in STAGE_12)
+  double* Y2r;         // F arrays: written by STAGE_12, read (h) by STAGE_34
+  double* Y3r;         // F arrays: written by STAGE_12, read (h) by STAGE_34
+  double* Y4r;         // F arrays: written by STAGE_34 if write_Y4r
+  double* ynew;        // state slot of y_{n+1} (STAGE_34)
   double dt;
   double inv12dx2[3];  // 1 / (12 dx_a^2)
   const double* A;     // device F*F row-major coupling, or null
-  double* scratch;     // 2F arrays (only when A != null): A u_n and A R of this stage
-  // TMA path: tensor map of the box (all arrays as the 4th dimension) and the array indices of yn / R
+  // TMA path: tensor map of the box (all arrays as the 4th dimension) and the array indices of the roles
   const void* tmap;    // host pointer to the box's CUtensorMap, or null -> direct-load kernel
-  int a_yn, a_R;
+  int a_yn, a_Y2r, a_Y3r;
 };
 void launch_stage(const StageArgs& a, cudaStream_t st);
-// 128-byte CUtensorMap of a box: dims (px, py, pz, narrays), fp64, no swizzle. Returns false (and leaves the
-// direct-load kernel in charge) when the driver entry point is unavailable or the box violates a TMA limit.
+// 128-byte CUtensorMap of a box: dims (px, py, pz, narrays), fp64, no swizzle, box = the stage kernels'
+// halo tile. Returns false (and leaves the direct-load kernel in charge) when the driver entry point is
+// unavailable or the box violates a TMA limit.
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, void* out_map128);
 
 // ------------------------------------------------------------------------------------------------

@@ -101,38 +101,37 @@ __global__ void __launch_bounds__(256) stage_direct(StageArgs a) {
   const long long o = cell_offset(b, i, j, k);
   const long long sy = b.px, sz = b.plane;
   const int F = a.F;
-  const double* u = a.yn + (long long)f * b.vol + o;
-  const double* r = a.R + (long long)f * b.vol + o;
+  const long long fo = (long long)f * b.vol + o;
+  const double* u = a.yn + fo;
   const double rho = a.yn[(long long)(F + f) * b.vol + o];
   const double dt = a.dt;
-  // coupling  sum_j A_fj W_j  at this cell
-  auto couple = [&](double c) {
+  // coupling  sum_q A_fq (u_q + c R_q)  at this cell
+  auto couple = [&](double c, const double* R) {
     double s = 0.0;
     if (a.A)
       for (int q = 0; q < F; ++q) {
-        const double wq = fma(c, a.R[(long long)q * b.vol + o], a.yn[(long long)q * b.vol + o]);
+        const double uq = a.yn[(long long)q * b.vol + o];
+        const double wq = R ? fma(c, R[(long long)q * b.vol + o], uq) : uq;
         s = fma(a.A[f * F + q], wq, s);
       }
     return s;
   };
   double wc;
   if (a.mode == STAGE_12) {
-    double Lu = lap_w<false>(u, r, 0.0, sy, sz, a.inv12dx2, &wc);
-    if (a.A)
-      for (int q = 0; q < F; ++q) Lu = fma(a.A[f * F + q], a.yn[(long long)q * b.vol + o], Lu);
-    const double L2 = lap_w<true>(u, r, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt);
-    a.out0[(long long)f * b.vol + o] = fma(0.5 * dt, Lu, rho);
-    a.out1[(long long)f * b.vol + o] = fma(0.5 * dt, L2, rho);
-  } else if (a.mode == STAGE_3) {
-    const double L3 = lap_w<true>(u, r, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt);
-    a.out0[(long long)f * b.vol + o] = fma(dt, L3, rho);
+    const double* rhoarr = a.yn + (long long)F * b.vol;
+    const double Lu = lap_w<false>(u, u, 0.0, sy, sz, a.inv12dx2, &wc) + couple(0.0, nullptr);
+    const double L2 = lap_w<true>(u, rhoarr + fo, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt, rhoarr);
+    a.Y2r[fo] = fma(0.5 * dt, Lu, rho);
+    a.Y3r[fo] = fma(0.5 * dt, L2, rho);
   } else {
-    const double k4r = lap_w<true>(u, r, dt, sy, sz, a.inv12dx2, &wc) + couple(dt);
-    const double y2 = a.Y2r[(long long)f * b.vol + o], y3 = r[0], y4 = a.Y4r[(long long)f * b.vol + o];
+    const double L3 = lap_w<true>(u, a.Y2r + fo, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt, a.Y2r);
+    const double k4r = lap_w<true>(u, a.Y3r + fo, dt, sy, sz, a.inv12dx2, &wc) + couple(dt, a.Y3r);
+    const double y2 = a.Y2r[fo], y3 = a.Y3r[fo], y4 = fma(dt, L3, rho);
     const double third = 1.0 / 3.0;
-    a.out0[(long long)f * b.vol + o] = fma(dt / 6.0, (rho + y4) + 2.0 * (y2 + y3), u[0]);
-    a.out0[(long long)(F + f) * b.vol + o] =
+    a.ynew[fo] = fma(dt / 6.0, (rho + y4) + 2.0 * (y2 + y3), u[0]);
+    a.ynew[(long long)F * b.vol + fo] =
         rho + (third * ((y2 - rho) + (y4 - rho)) + (2.0 * third) * (y3 - rho)) + (dt / 6.0) * k4r;
+    if (a.write_Y4r) a.Y4r[fo] = y4;
   }
 }
 

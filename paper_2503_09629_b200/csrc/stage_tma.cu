@@ -1,0 +1,359 @@
+// stage_tma.cu — tuned RK4 stage kernels (eqs 1-9 on the wave system
+// PAPER.md:222-226), sm_100a: z-march with TMA-staged halo planes.
+//
+// One CTA owns a TX x TY column of cells and marches through a chunk of z-planes. Every plane of every
+// halo-read array arrives in shared memory as a (TX+4) x (TY+4) tile through ONE TMA tiled load
+// (cp.async.bulk.tensor.4d, box dims (x, y, 1 plane, 1 array)) signalled on an mbarrier; NST planes are in
+// flight so HBM latency never meets a warp. A thread owns two x-adjacent cells (16-byte shared loads and
+// 16-byte coalesced global stores) and NEVER re-reads a plane: the 4th-order Laplacian (S2) is applied in
+// scatter form — when plane p arrives its in-plane part goes to the accumulator of output plane p and its
+// value to the accumulators of p-2, p-1, p+1, p+2 — so the z-direction lives in registers and each shared
+// value is loaded once. Output plane p-2 is complete when plane p has arrived.
+// Algorithmic traffic per cell and field (doubles): STAGE_12 reads u, rho, writes Y2r, Y3r (4);
+// STAGE_34 reads u, rho, Y2r, Y3r, writes u_new, rho_new [, Y4r] (6 or 7). 10-11 per RK4 step.
+// Neighbouring z-chunks march in OPPOSITE directions away from / towards their common boundary, so the 4
+// halo planes two chunks share are requested at the same time and the second request hits L2.
+#include <cuda.h>
+
+#include <cstdlib>
+#include <cstring>
+#include <type_traits>
+
+#include "kernels.h"
+
+namespace sc {
+
+void launch_stage_direct(const StageArgs& a, cudaStream_t st);
+
+namespace {
+
+constexpr int TX = 32, TY = 16;              // cells per CTA column
+constexpr int HX = TX + 4, HY = TY + 4;      // halo tile
+constexpr int NTHR = (TX / 2) * TY;          // 256 threads, two cells each
+constexpr int TILE_DOUBLES = HX * HY;        // 720 doubles = 5760 B (multiple of 128 B)
+constexpr int NST = 4;                       // planes in flight
+static_assert((TILE_DOUBLES * 8) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
+                                            uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, "
+      "%5}], [%6];" ::"r"(dst),
+      "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
+      : "memory");
+}
+
+struct TmaStageParams {
+  BoxView b;
+  int F, nchunks, chunk, write_Y4r;
+  int a_yn, a_Y2r, a_Y3r;
+  const double* yn;
+  double* Y2r;
+  double* Y3r;
+  double* Y4r;
+  double* ynew;
+  double dt;
+  double w[3];  // 1 / (12 dx_a^2)
+};
+
+// values of one array around the thread's two cells (x, x+1) in the current plane
+struct Nbr {
+  double2 xa, xb, xc;          // row y: columns x-2..x+3
+  double2 ym2, ym1, yp1, yp2;  // columns x, x+1 of rows y-2, y-1, y+1, y+2
+};
+__device__ __forceinline__ Nbr load_nbr(const double* tile, int tx, int ty) {
+  Nbr n;
+  const double2* r = reinterpret_cast<const double2*>(tile + (ty + 2) * HX + 2 * tx);
+  n.xa = r[0]; n.xb = r[1]; n.xc = r[2];
+  n.ym2 = *reinterpret_cast<const double2*>(tile + (ty + 0) * HX + 2 * tx + 2);
+  n.ym1 = *reinterpret_cast<const double2*>(tile + (ty + 1) * HX + 2 * tx + 2);
+  n.yp1 = *reinterpret_cast<const double2*>(tile + (ty + 3) * HX + 2 * tx + 2);
+  n.yp2 = *reinterpret_cast<const double2*>(tile + (ty + 4) * HX + 2 * tx + 2);
+  return n;
+}
+__device__ __forceinline__ double2 load_centre(const double* tile, int tx, int ty) {
+  return *reinterpret_cast<const double2*>(tile + (ty + 2) * HX + 2 * tx + 2);
+}
+__device__ __forceinline__ double2 fma2(double c, double2 a, double2 b) {
+  return make_double2(fma(c, a.x, b.x), fma(c, a.y, b.y));
+}
+__device__ __forceinline__ Nbr axpy(double c, const Nbr& r, const Nbr& u) {  // u + c r
+  Nbr n;
+  n.xa = fma2(c, r.xa, u.xa); n.xb = fma2(c, r.xb, u.xb); n.xc = fma2(c, r.xc, u.xc);
+  n.ym2 = fma2(c, r.ym2, u.ym2); n.ym1 = fma2(c, r.ym1, u.ym1);
+  n.yp1 = fma2(c, r.yp1, u.yp1); n.yp2 = fma2(c, r.yp2, u.yp2);
+  return n;
+}
+// in-plane part of the 13-point Laplacian at the two cells: wx d_xx + wy d_yy - 30 wz centre
+__device__ __forceinline__ double2 inplane(const Nbr& n, double wx, double wy, double c30) {
+  const double x0 = 16.0 * (n.xa.y + n.xb.y) - (n.xa.x + n.xc.x);
+  const double x1 = 16.0 * (n.xb.x + n.xc.x) - (n.xa.y + n.xc.y);
+  const double y0 = 16.0 * (n.ym1.x + n.yp1.x) - (n.ym2.x + n.yp2.x);
+  const double y1 = 16.0 * (n.ym1.y + n.yp1.y) - (n.ym2.y + n.yp2.y);
+  return make_double2(fma(wx, x0, fma(wy, y0, -c30 * n.xb.x)), fma(wx, x1, fma(wy, y1, -c30 * n.xb.y)));
+}
+
+// Scatter one arrived plane into the five pending accumulators. R = arrival index mod 5 (compile time), so
+// slot (R + d) mod 5 belongs to output plane (arrival + d). The slot of arrival + 2 is created here.
+template <int R>
+__device__ __forceinline__ void scatter(double2 (&acc)[5], double2 centre_term, double2 zc) {
+  acc[(R + 3) % 5].x -= zc.x;                      acc[(R + 3) % 5].y -= zc.y;
+  acc[(R + 4) % 5].x = fma(16.0, zc.x, acc[(R + 4) % 5].x);
+  acc[(R + 4) % 5].y = fma(16.0, zc.y, acc[(R + 4) % 5].y);
+  acc[R].x += centre_term.x;                       acc[R].y += centre_term.y;
+  acc[(R + 1) % 5].x = fma(16.0, zc.x, acc[(R + 1) % 5].x);
+  acc[(R + 1) % 5].y = fma(16.0, zc.y, acc[(R + 1) % 5].y);
+  acc[(R + 2) % 5] = make_double2(-zc.x, -zc.y);
+}
+
+}  // namespace
+
+template <int MODE>
+__global__ void __launch_bounds__(NTHR, 2)
+    stage_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ TmaStageParams p) {
+  constexpr int NH = MODE == STAGE_12 ? 2 : 3;  // halo-read arrays per plane
+  extern __shared__ unsigned char smraw[];
+  // [NST][NH] tiles, 128-byte aligned for TMA, then NST mbarriers
+  const uint32_t s0 = (smem_u32(smraw) + 127u) & ~127u;
+  double* const tiles = reinterpret_cast<double*>(smraw + (s0 - smem_u32(smraw)));
+  const uint32_t bar0 = s0 + NST * NH * TILE_DOUBLES * 8;
+
+  const BoxView& b = p.b;
+  const int tid = threadIdx.x, tx = tid % (TX / 2), ty = tid / (TX / 2);
+  const int X0 = blockIdx.x * TX, Y0 = blockIdx.y * TY;
+  const int f = blockIdx.z / p.nchunks, c = blockIdx.z % p.nchunks;
+  const int zc0 = c * p.chunk, zc1 = min(b.n[2], zc0 + p.chunk);
+  const int narr = zc1 - zc0 + 4;              // planes that arrive: the chunk plus 2 halo planes each side
+  const int dir = (c & 1) ? 1 : -1;            // neighbouring chunks march in opposite directions
+  const int zs = dir > 0 ? zc0 - 2 : zc1 + 1;  // first plane to arrive
+  int arr[NH];
+  arr[0] = p.a_yn + f;
+  if (MODE == STAGE_12) arr[1] = p.a_yn + p.F + f;
+  else { arr[1] = p.a_Y2r + f; arr[NH - 1] = p.a_Y3r + f; }
+
+  auto issue = [&](int it) {  // one thread: arm the stage's mbarrier and request the plane's tiles
+    const int st = it % NST;
+    const uint32_t bar = bar0 + 8 * st;
+    mbar_expect_tx(bar, NH * TILE_DOUBLES * 8);
+#pragma unroll
+    for (int h = 0; h < NH; ++h)
+      tma_load_4d(s0 + (st * NH + h) * TILE_DOUBLES * 8, &tmap, XOFF + X0 - 2, b.g + Y0 - 2, b.g + zs + dir * it,
+                  arr[h], bar);
+  };
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NST; ++s) mbar_init(bar0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    for (int it = 0; it < NST && it < narr; ++it) issue(it);
+  }
+  __syncthreads();
+
+  const bool active = (X0 + 2 * tx < b.n[0]) && (Y0 + ty < b.n[1]);
+  const long long cell0 = cell_offset(b, X0 + 2 * tx, Y0 + ty, 0);
+  const double dt = p.dt, hdt = 0.5 * p.dt, third = 1.0 / 3.0, dt6 = p.dt / 6.0;
+  // accumulator A collects Y2r (STAGE_12) / Y4r (STAGE_34); B collects Y3r / rho_new - Y4r/3
+  const double sA = MODE == STAGE_12 ? hdt : dt, sB = MODE == STAGE_12 ? hdt : dt6;
+  const double wxA = sA * p.w[0], wyA = sA * p.w[1], wzA = sA * p.w[2], cA = 30.0 * (wxA + wyA + wzA);
+  const double wxB = sB * p.w[0], wyB = sB * p.w[1], wzB = sB * p.w[2], cB = 30.0 * (wxB + wyB + wzB);
+  double2 accA[5], accB[5], Pu[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) accA[q] = accB[q] = Pu[q] = make_double2(0.0, 0.0);
+  const double* __restrict__ rho_g = p.yn + (long long)(p.F + f) * b.vol + cell0;
+  double2 rho_nxt = make_double2(0.0, 0.0);
+  (void)rho_g;
+
+  auto step = [&](auto Rc, int it) {
+    constexpr int R = decltype(Rc)::value;
+    const int st = it % NST;
+    const bool inpl = it >= 2 && it < narr - 2;
+    const int z = zs + dir * it;
+    double2 rho_c = rho_nxt;
+    if (MODE == STAGE_34) {  // rho_n is read at the centre only: plain global load, one plane ahead
+      const int itn = it + 1;
+      if (active && itn >= 2 && itn < narr - 2)
+        rho_nxt = __ldg(reinterpret_cast<const double2*>(rho_g + (long long)(z + dir) * b.plane));
+    }
+    mbar_wait(bar0 + 8 * st, (it / NST) & 1);
+    const double* __restrict__ t0 = tiles + (st * NH) * TILE_DOUBLES;
+    double2 ctA = make_double2(0.0, 0.0), ctB = ctA, zcA, zcB;
+    if (MODE == STAGE_12) {
+      if (inpl) {
+        const Nbr u = load_nbr(t0, tx, ty), r = load_nbr(t0 + TILE_DOUBLES, tx, ty);
+        const Nbr w = axpy(hdt, r, u);
+        const double2 iu = inplane(u, wxA, wyA, cA), iw = inplane(w, wxB, wyB, cB);
+        ctA = make_double2(r.xb.x + iu.x, r.xb.y + iu.y);
+        ctB = make_double2(r.xb.x + iw.x, r.xb.y + iw.y);
+        zcA = make_double2(wzA * u.xb.x, wzA * u.xb.y);
+        zcB = make_double2(wzB * w.xb.x, wzB * w.xb.y);
+      } else {
+        const double2 uc = load_centre(t0, tx, ty), rc = load_centre(t0 + TILE_DOUBLES, tx, ty);
+        const double2 wc = fma2(hdt, rc, uc);
+        zcA = make_double2(wzA * uc.x, wzA * uc.y);
+        zcB = make_double2(wzB * wc.x, wzB * wc.y);
+      }
+    } else {
+      if (inpl) {
+        const Nbr u = load_nbr(t0, tx, ty);
+        const Nbr y2 = load_nbr(t0 + TILE_DOUBLES, tx, ty), y3 = load_nbr(t0 + 2 * TILE_DOUBLES, tx, ty);
+        const Nbr w3 = axpy(hdt, y2, u), w4 = axpy(dt, y3, u);
+        const double2 i3 = inplane(w3, wxA, wyA, cA), i4 = inplane(w4, wxB, wyB, cB);
+        ctA = make_double2(rho_c.x + i3.x, rho_c.y + i3.y);
+        const double prx = rho_c.x + (third * (y2.xb.x - rho_c.x) + (2.0 * third) * (y3.xb.x - rho_c.x)) - third * rho_c.x;
+        const double pry = rho_c.y + (third * (y2.xb.y - rho_c.y) + (2.0 * third) * (y3.xb.y - rho_c.y)) - third * rho_c.y;
+        ctB = make_double2(prx + i4.x, pry + i4.y);
+        Pu[R] = make_double2(fma(dt6, rho_c.x + 2.0 * (y2.xb.x + y3.xb.x), u.xb.x),
+                             fma(dt6, rho_c.y + 2.0 * (y2.xb.y + y3.xb.y), u.xb.y));
+        zcA = make_double2(wzA * w3.xb.x, wzA * w3.xb.y);
+        zcB = make_double2(wzB * w4.xb.x, wzB * w4.xb.y);
+      } else {
+        const double2 uc = load_centre(t0, tx, ty);
+        const double2 w3 = fma2(hdt, load_centre(t0 + TILE_DOUBLES, tx, ty), uc);
+        const double2 w4 = fma2(dt, load_centre(t0 + 2 * TILE_DOUBLES, tx, ty), uc);
+        zcA = make_double2(wzA * w3.x, wzA * w3.y);
+        zcB = make_double2(wzB * w4.x, wzB * w4.y);
+      }
+    }
+    scatter<R>(accA, ctA, zcA);
+    scatter<R>(accB, ctB, zcB);
+    if (it >= 4 && active) {  // output plane z - 2 dir is complete
+      const long long o = (long long)f * b.vol + cell0 + (long long)(z - 2 * dir) * b.plane;
+      const double2 a = accA[(R + 3) % 5], bb = accB[(R + 3) % 5];
+      if (MODE == STAGE_12) {
+        *reinterpret_cast<double2*>(p.Y2r + o) = a;
+        *reinterpret_cast<double2*>(p.Y3r + o) = bb;
+      } else {
+        const double2 pu = Pu[(R + 3) % 5];
+        *reinterpret_cast<double2*>(p.ynew + o) = make_double2(fma(dt6, a.x, pu.x), fma(dt6, a.y, pu.y));
+        *reinterpret_cast<double2*>(p.ynew + (long long)p.F * b.vol + o) =
+            make_double2(fma(third, a.x, bb.x), fma(third, a.y, bb.y));
+        if (p.write_Y4r) *reinterpret_cast<double2*>(p.Y4r + o) = a;
+      }
+    }
+    __syncthreads();  // every thread is done with stage st: refill it with the plane NST arrivals ahead
+    if (tid == 0 && it + NST < narr) issue(it + NST);
+  };
+
+  for (int it0 = 0; it0 < narr; it0 += 5) {
+    step(std::integral_constant<int, 0>{}, it0);
+    if (it0 + 1 < narr) step(std::integral_constant<int, 1>{}, it0 + 1);
+    if (it0 + 2 < narr) step(std::integral_constant<int, 2>{}, it0 + 2);
+    if (it0 + 3 < narr) step(std::integral_constant<int, 3>{}, it0 + 3);
+    if (it0 + 4 < narr) step(std::integral_constant<int, 4>{}, it0 + 4);
+  }
+}
+
+// ---- host ------------------------------------------------------------------------------------------
+namespace {
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) != cudaSuccess ||
+        qr != cudaDriverEntryPointSuccess) {
+      cudaGetLastError();
+      p = nullptr;
+    }
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+template <int MODE>
+size_t stage_smem() { return (size_t)NST * (MODE == STAGE_12 ? 2 : 3) * TILE_DOUBLES * 8 + NST * 8 + 128; }
+
+// z-chunks per column: enough CTAs to fill the machine in whole waves, as few halo planes as possible
+int pick_chunks(const BoxView& b, int F, int ctas_per_sm) {
+  static const int forced = [] { const char* e = getenv("SC_ZCHUNKS"); return e ? atoi(e) : 0; }();
+  static const int nsm = [] {
+    int dev = 0, n = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    return n > 0 ? n : 148;
+  }();
+  if (forced > 0) return forced < b.n[2] ? forced : b.n[2];
+  const long long cols = (long long)((b.n[0] + TX - 1) / TX) * ((b.n[1] + TY - 1) / TY) * F;
+  const long long slots = (long long)nsm * ctas_per_sm;
+  int best = 1;
+  double best_cost = 1e300;
+  const int maxch = b.n[2] / 8 > 1 ? b.n[2] / 8 : 1;
+  for (int nch = 1; nch <= maxch; ++nch) {
+    const int ch = (b.n[2] + nch - 1) / nch;
+    const long long ctas = cols * ((b.n[2] + ch - 1) / ch);
+    const long long waves = (ctas + slots - 1) / slots;
+    const double cost = (double)waves * (ch + 4 + 6);  // time ~ waves x (planes marched + pipeline fill)
+    if (cost < best_cost - 1e-9) { best_cost = cost; best = nch; }
+  }
+  return best;
+}
+
+template <int MODE>
+void launch_zmarch(const StageArgs& a, cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    cudaFuncSetAttribute(stage_zmarch<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage_smem<MODE>());
+    configured = true;
+  }
+  TmaStageParams p{};
+  p.b = a.b;
+  p.F = a.F;
+  p.nchunks = pick_chunks(a.b, a.F, 2);
+  p.chunk = (a.b.n[2] + p.nchunks - 1) / p.nchunks;
+  p.nchunks = (a.b.n[2] + p.chunk - 1) / p.chunk;
+  p.write_Y4r = a.write_Y4r;
+  p.a_yn = a.a_yn; p.a_Y2r = a.a_Y2r; p.a_Y3r = a.a_Y3r;
+  p.yn = a.yn; p.Y2r = a.Y2r; p.Y3r = a.Y3r; p.Y4r = a.Y4r; p.ynew = a.ynew;
+  p.dt = a.dt;
+  for (int d = 0; d < 3; ++d) p.w[d] = a.inv12dx2[d];
+  dim3 grd((a.b.n[0] + TX - 1) / TX, (a.b.n[1] + TY - 1) / TY, p.nchunks * a.F);
+  stage_zmarch<MODE><<<grd, NTHR, stage_smem<MODE>(), st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
+}
+
+}  // namespace
+
+bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, void* out_map128) {
+  EncodeTiledFn enc = encode_tiled();
+  if (!enc) return false;
+  if (b.px > (1 << 30) || (reinterpret_cast<uintptr_t>(base) & 15)) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)b.px, (cuuint64_t)b.py, (cuuint64_t)b.pz, (cuuint64_t)narrays};
+  const cuuint64_t strides[3] = {(cuuint64_t)b.px * 8, (cuuint64_t)b.plane * 8, (cuuint64_t)b.vol * 8};
+  const cuuint32_t box[4] = {HX, HY, 1, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUtensorMap m;
+  const CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap is 128 bytes");
+  memcpy(out_map128, &m, 128);
+  return true;
+}
+
+void launch_stage_tma(const StageArgs& a, cudaStream_t st) {
+  if (a.A || !a.tmap) { launch_stage_direct(a, st); return; }
+  if (a.mode == STAGE_12) launch_zmarch<STAGE_12>(a, st);
+  else launch_zmarch<STAGE_34>(a, st);
+}
+
+}  // namespace sc
