@@ -55,7 +55,8 @@ struct sc_hierarchy {
   struct BoxTiles { GhostTile* dev = nullptr; int n = 0; };
   std::vector<BoxTiles> tiles;    // per box (levels >= 1): ghost-shell tile list on the device
   struct alignas(64) TMap { unsigned char bytes[128]; };
-  std::vector<TMap> tmaps;        // per box: CUtensorMap over all arrays of the box
+  std::vector<TMap> tmaps;        // per box: CUtensorMap over all arrays of the box (stage-kernel tile)
+  std::vector<TMap> rmaps;        // per box: same tensor, box = the restriction kernel's fine-plane pair
   std::vector<char> tmap_ok;
   // per-launch CUDA-event timing (sc_profile): eager launches, one event pair per kernel
   bool profiling = false;
@@ -293,8 +294,15 @@ void restrict_level(Seq& q, int level) {  // level -> level-1, into the parents'
   for (int ib : h->L.level_boxes[level]) {
     const BoxInfo& b = h->L.boxes[ib];
     prof_begin(h, KIND_RESTRICT, 8.0 * h->L.V * (cells(b.v) + cells(b.v) / 8.0));
-    launch_restrict(b.v, h->L.boxes[b.parent].v, h->L.V, h->arr(ib, h->L.a_state(q.cur[level])),
-                    h->arr(b.parent, h->L.a_state(q.cur[level - 1])), h->stream);
+    RestrictArgs a{};
+    a.child = b.v;
+    a.parent = h->L.boxes[b.parent].v;
+    a.V = h->L.V;
+    a.a_child = h->L.a_state(q.cur[level]);
+    a.ychild = h->arr(ib, a.a_child);
+    a.yparent = h->arr(b.parent, h->L.a_state(q.cur[level - 1]));
+    a.tmap = h->tmap_ok[ib] ? h->rmaps[ib].bytes : nullptr;
+    launch_restrict(a, h->stream);
     prof_end(h);
     ++q.n;
   }
@@ -489,8 +497,12 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   }
   h->tmaps.resize(h->L.boxes.size());
   h->tmap_ok.assign(h->L.boxes.size(), 0);
-  for (size_t ib = 0; ib < h->L.boxes.size(); ++ib)
-    h->tmap_ok[ib] = make_box_tensor_map(h->L.boxes[ib].v, h->L.boxes[ib].narrays, h->arr((int)ib, 0), h->tmaps[ib].bytes) ? 1 : 0;
+  h->rmaps.resize(h->L.boxes.size());
+  for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
+    const BoxInfo& b = h->L.boxes[ib];
+    h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
+                     make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
+  }
   if ((ce = cudaStreamSynchronize(h->stream)) != cudaSuccess) return bail("sync", ce);
   h->cur.assign(h->L.nlevels, 0);
   h->l0_ghosts_valid = false;

@@ -7,11 +7,13 @@ namespace sc {
 
 void launch_stage_direct(const StageArgs& a, cudaStream_t st);
 void launch_stage_tma(const StageArgs& a, cudaStream_t st);
-bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, void* out_map128);
+bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned box[4], void* out_map128);
+void stage_box_dims(unsigned box[4]);
+void restrict_box_dims(unsigned box[4]);
 void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
 void launch_ghost_fill_tiled(const GhostArgs& a, cudaStream_t st);
 void launch_restrict_ref(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st);
-void launch_restrict_opt(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st);
+void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st);
 
 static int g_mode = 1;
 void select_kernels(int mode) { g_mode = mode; }
@@ -25,12 +27,15 @@ void launch_ghost_fill(const GhostArgs& a, cudaStream_t st) {
   if (g_mode == 0 || a.ntiles == 0) launch_ghost_fill_direct(a, st);
   else launch_ghost_fill_tiled(a, st);
 }
-void launch_restrict(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st) {
-  if (g_mode == 0) launch_restrict_ref(ch, pa, V, yc, yp, st);
-  else launch_restrict_opt(ch, pa, V, yc, yp, st);
+void launch_restrict(const RestrictArgs& a, cudaStream_t st) {
+  if (g_mode == 0) launch_restrict_ref(a.child, a.parent, a.V, a.ychild, a.yparent, st);
+  else launch_restrict_opt(a, st);
 }
-bool make_box_tensor_map(const BoxView& b, int narrays, void* base, void* out_map128) {
-  return make_box_tensor_map_tma(b, narrays, base, out_map128);
+bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128) {
+  unsigned box[4];
+  if (kind == 0) stage_box_dims(box);
+  else restrict_box_dims(box);
+  return make_box_tensor_map_tma(b, narrays, base, box, out_map128);
 }
 
 }  // namespace sc

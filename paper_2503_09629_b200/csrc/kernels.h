@@ -43,10 +43,10 @@ struct StageArgs {
   int a_yn, a_Y2r, a_Y3r;
 };
 void launch_stage(const StageArgs& a, cudaStream_t st);
-// 128-byte CUtensorMap of a box: dims (px, py, pz, narrays), fp64, no swizzle, box = the stage kernels'
-// halo tile. Returns false (and leaves the direct-load kernel in charge) when the driver entry point is
-// unavailable or the box violates a TMA limit.
-bool make_box_tensor_map(const BoxView& b, int narrays, void* base, void* out_map128);
+// 128-byte CUtensorMaps of a box: dims (px, py, pz, narrays), fp64, no swizzle; kind 0: box = the stage
+// kernels' halo tile, kind 1: box = the restriction kernel's pair of fine planes. Returns false (and leaves
+// the direct-load kernels in charge) when the driver entry point is unavailable or a TMA limit is violated.
+bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128);
 
 // ------------------------------------------------------------------------------------------------
 // a3: refinement-boundary ghost fill. For every ghost cell of a level >= 1 box and every output o:
@@ -81,8 +81,15 @@ void launch_ghost_fill(const GhostArgs& a, cudaStream_t st);
 void launch_periodic_fill(const BoxView& b, int narrays, double* y, cudaStream_t st);
 
 // a5: restriction child -> parent of V consecutive arrays (reading S4).
-void launch_restrict(const BoxView& child, const BoxView& parent, int V, const double* ychild,
-                     double* yparent, cudaStream_t st);
+struct RestrictArgs {
+  BoxView child, parent;
+  int V;
+  const double* ychild;  // child state, component 0 (read with 2 ghost layers)
+  double* yparent;       // parent state, component 0
+  const void* tmap;      // host pointer to the child's kind-1 CUtensorMap, or null -> direct-load kernel
+  int a_child;           // array index of ychild in the child's tensor map
+};
+void launch_restrict(const RestrictArgs& a, cudaStream_t st);
 
 // interior-only <-> padded copies for sc_set_state / sc_read_level (device src/dst, dense [k][j][i])
 void launch_pack(const BoxView& b, const double* padded, double* dense, int with_ghosts, cudaStream_t st);

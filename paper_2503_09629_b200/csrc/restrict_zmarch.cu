@@ -1,95 +1,178 @@
-// restrict_zmarch.cu — tuned restriction kernel (a5, reading S4).
-// One CTA owns RPX x RPY parent columns and marches through the child's z-planes; each fine plane is
-// staged in shared memory, reduced in x then y by the 6-point weights, and kept in a 6-deep register ring
-// that is contracted in z every second plane. Each fine value is read once per CTA.
+// restrict_zmarch.cu — tuned restriction kernel (PAPER.md:119 step 7; operator = reading
+// S4: tensor-product quintic Lagrange (3,-25,150,150,-25,3)/256 on fine cells 2J-2 .. 2J+3 per axis).
+//
+// One CTA owns RPX x RPY parent columns and marches through a chunk of parent planes. Fine planes arrive in
+// PAIRS (2m, 2m+1) as one TMA tiled load each (box = fine tile x 2 planes) into a ring of NSTR stages, so
+// several pairs are always in flight and DRAM latency (and its tail) never meets a warp.
+//   x: a thread owns two x-adjacent parents of one fine row: it reads the 8 fine values under them (four
+//      16-byte shared loads, conflict-free by the lane -> (column, row) mapping and the 70-double pitch)
+//      and reduces them to two x-restricted values per plane;
+//   z: scatter form in registers — the pair completes parent plane m-1 and feeds the pending accumulators
+//      of m and m+1 (by the symmetry of the operator the same code marches down);
+//   y: only the completed x,z-restricted plane goes through shared memory (double-buffered, one
+//      __syncthreads per pair) for the 6-point y reduction and the coalesced store.
+// Neighbouring z-chunks march in opposite directions (as in stage_tma.cu) so their shared planes hit L2.
+#include <cuda.h>
+
+#include <cstdlib>
+
 #include "kernels.h"
 
 namespace sc {
 
-// ====================================================================================================
-// restriction: z-march
-// ====================================================================================================
+void launch_restrict_ref(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st);
+
 namespace {
-constexpr int RPX = 32, RPY = 8;            // parent cells per CTA in x, y  (256 threads, one column each)
-constexpr int RFX = 2 * RPX + 4, RFY = 2 * RPY + 4;  // fine plane tile incl. the 2-cell halo
+constexpr int RPX = 32, RPY = 6;              // parent cells per CTA in x, y
+constexpr int RFY = 2 * RPY + 4;              // 16 fine rows incl. the 2-row halo
+constexpr int RPITCH = 2 * RPX + 6;           // 70: fine row incl. halo (68) + 2 pad columns (bank spread)
+constexpr int RNT = 256;                      // 16 parent pairs x 16 fine rows
+constexpr int RSTAGE = 2 * RFY * RPITCH;      // doubles per stage (one pair of fine planes) = 2240
+constexpr int NSTR = 3;                       // pairs in flight (3 CTAs/SM x 3 x 17.5 KB)
+constexpr int SXP = 40;                       // pitch of the x,z-restricted plane (bank spread)
+constexpr double R0 = 3.0 / 256.0, R1 = -25.0 / 256.0, R2 = 150.0 / 256.0;
+static_assert((RSTAGE * 8) % 128 == 0, "TMA destination must stay 128-byte aligned");
+static_assert(RNT == (RPX / 2) * RFY, "one thread per (parent pair, fine row)");
+
 __device__ __forceinline__ double lagr6(double a, double b, double c, double d, double e, double f) {
-  return (3.0 / 256.0) * (a + f) + (-25.0 / 256.0) * (b + e) + (150.0 / 256.0) * (c + d);
+  return R0 * (a + f) + R1 * (b + e) + R2 * (c + d);
 }
+__device__ __forceinline__ uint32_t smem_u32r(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_wait_r(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+
+struct RestrictParams {
+  BoxView ch, pa;
+  int a_child;       // array index (in the child's tensor map) of component 0 of the child's state
+  int pz_per_cta, nzc;
+  double* yp;        // parent state, component 0
+};
 }  // namespace
 
-__global__ void __launch_bounds__(RPX* RPY) restrict_zmarch(BoxView ch, BoxView pa, const double* __restrict__ yc,
-                                                            double* __restrict__ yp, int pz_per_cta) {
-  __shared__ double sF[RFY][RFX];   // fine plane tile
-  __shared__ double sX[RFY][RPX];   // after the x reduction
-  const int tx = threadIdx.x % RPX, ty = threadIdx.x / RPX;
+__global__ void __launch_bounds__(RNT, 3)
+    restrict_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ RestrictParams p) {
+  extern __shared__ unsigned char rsm[];
+  const uint32_t s0 = (smem_u32r(rsm) + 127u) & ~127u;
+  const double* const tiles = reinterpret_cast<const double*>(rsm + (s0 - smem_u32r(rsm)));  // [NSTR][2][RFY][RPITCH]
+  double* const sX = const_cast<double*>(tiles) + NSTR * RSTAGE;                              // [2][RFY][SXP]
+  const uint32_t bar0 = s0 + (NSTR * RSTAGE + 2 * RFY * SXP) * 8;
+
+  const BoxView& ch = p.ch;
+  const BoxView& pa = p.pa;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int xp = (lane & 3) | ((lane >> 3) << 2);   // parent pair 0..15  -> parents 2xp, 2xp+1
+  const int row = 2 * warp + ((lane >> 2) & 1);     // fine row 0..15 of the tile
   const int X0 = blockIdx.x * RPX, Y0 = blockIdx.y * RPY;
-  const int nzc = (ch.n[2] / 2 + pz_per_cta - 1) / pz_per_cta;
-  const int comp = blockIdx.z / nzc;
-  const int Z0 = (blockIdx.z % nzc) * pz_per_cta;
-  const int Z1 = min(Z0 + pz_per_cta, ch.n[2] / 2);
-  const int npx = ch.n[0] / 2, npy = ch.n[1] / 2;
-  const double* __restrict__ src = yc + (long long)comp * ch.vol;
-  double* __restrict__ dst = yp + (long long)comp * pa.vol;
-  const int P0 = (ch.lo[0] >> 1) - pa.lo[0], P1 = (ch.lo[1] >> 1) - pa.lo[1], P2 = (ch.lo[2] >> 1) - pa.lo[2];
-  // fine extent actually needed by this CTA (ragged tiles)
-  const int fx = min(RFX, 2 * (npx - X0) + 4), fy = min(RFY, 2 * (npy - Y0) + 4);
-  const int nload = fx * fy;
-  const bool active = (X0 + tx < npx) && (Y0 + ty < npy);
-  double ring[6];
-#pragma unroll
-  for (int q = 0; q < 6; ++q) ring[q] = 0.0;
-  // fine planes 2*Z0-2 .. 2*Z1+1 ; parent plane Z is complete after fine plane 2Z+3
-  constexpr int NPRE = (RFX * RFY + RPX * RPY - 1) / (RPX * RPY);
-  double pre[NPRE];
-  auto load_plane = [&](int kf) {
-#pragma unroll
-    for (int q = 0; q < NPRE; ++q) {
-      const int idx = threadIdx.x + q * (RPX * RPY);
-      if (idx < nload) {
-        const int x = idx % fx, y = idx / fx;
-        pre[q] = src[cell_offset(ch, 2 * X0 - 2 + x, 2 * Y0 - 2 + y, kf)];
-      }
-    }
+  const int comp = blockIdx.z / p.nzc, chunk = blockIdx.z % p.nzc;
+  const int npx = ch.n[0] / 2, npy = ch.n[1] / 2, npz = ch.n[2] / 2;
+  const int Z0 = chunk * p.pz_per_cta, Z1 = min(Z0 + p.pz_per_cta, npz);
+  const int dir = (chunk & 1) ? 1 : -1;
+  const int npairs = Z1 - Z0 + 2;  // fine-plane pairs m = Z0-1 .. Z1
+  auto pair_m = [&](int i) { return dir > 0 ? Z0 - 1 + i : Z1 - i; };
+  auto issue = [&](int i) {
+    const int st = i % NSTR;
+    const uint32_t bar = bar0 + 8 * st;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(RSTAGE * 8) : "memory");
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, "
+        "%5}], [%6];" ::"r"(s0 + st * RSTAGE * 8),
+        "l"(&tmap), "r"(XOFF + 2 * X0 - 2), "r"(ch.g + 2 * Y0 - 2), "r"(ch.g + 2 * pair_m(i)), "r"(p.a_child + comp),
+        "r"(bar)
+        : "memory");
   };
-  const int kf0 = 2 * Z0 - 2, kf1 = 2 * Z1 + 1;
-  load_plane(kf0);
-  for (int kf = kf0; kf <= kf1; ++kf) {
+  if (tid == 0) {
 #pragma unroll
-    for (int q = 0; q < NPRE; ++q) {
-      const int idx = threadIdx.x + q * (RPX * RPY);
-      if (idx < nload) sF[idx / fx][idx % fx] = pre[q];
-    }
-    __syncthreads();
-    if (kf < kf1) load_plane(kf + 1);  // prefetch the next plane while this one is reduced
-    for (int idx = threadIdx.x; idx < RPX * fy; idx += RPX * RPY) {
-      const int x = idx % RPX, y = idx / RPX;
-      const double* r = &sF[y][2 * x];
-      sX[y][x] = lagr6(r[0], r[1], r[2], r[3], r[4], r[5]);
-    }
-    __syncthreads();
-    const double v = lagr6(sX[2 * ty][tx], sX[2 * ty + 1][tx], sX[2 * ty + 2][tx], sX[2 * ty + 3][tx],
-                           sX[2 * ty + 4][tx], sX[2 * ty + 5][tx]);
+    for (int s = 0; s < NSTR; ++s)
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar0 + 8 * s), "r"(1));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    for (int i = 0; i < NSTR && i < npairs; ++i) issue(i);
+  }
+  __syncthreads();
+
+  const int P0 = (ch.lo[0] >> 1) - pa.lo[0], P1 = (ch.lo[1] >> 1) - pa.lo[1], P2 = (ch.lo[2] >> 1) - pa.lo[2];
+  const int tx = tid % RPX, ty = tid / RPX;  // y-pass: one thread per parent cell (ty < RPY)
+  const bool active = ty < RPY && (X0 + tx < npx) && (Y0 + ty < npy);
+  double* __restrict__ dst = p.yp + (long long)comp * pa.vol + cell_offset(pa, P0 + X0 + tx, P1 + Y0 + ty, P2);
+  double2 a0 = make_double2(0.0, 0.0), a1 = a0;  // pending z-accumulators: planes m - dir (completes next), m
+  for (int i = 0; i < npairs; ++i) {
+    const int st = i % NSTR;
+    mbar_wait_r(bar0 + 8 * st, (i / NSTR) & 1);
+    const double* t = tiles + st * RSTAGE + row * RPITCH + 4 * xp;
+    double2 xr[2];  // x-restricted values of the two planes (lower z first)
 #pragma unroll
-    for (int q = 0; q < 5; ++q) ring[q] = ring[q + 1];
-    ring[5] = v;
-    const int rel = kf - kf0;  // 0-based plane counter; parent plane Z0 + m completes at rel = 2m + 5
-    if (rel >= 5 && ((rel - 5) & 1) == 0 && active) {
-      const int Z = Z0 + (rel - 5) / 2;
-      dst[cell_offset(pa, P0 + X0 + tx, P1 + Y0 + ty, P2 + Z)] =
-          lagr6(ring[0], ring[1], ring[2], ring[3], ring[4], ring[5]);
+    for (int q = 0; q < 2; ++q) {
+      const double2* r = reinterpret_cast<const double2*>(t + q * (RFY * RPITCH));
+      const double2 a = r[0], b = r[1], c = r[2], d = r[3];
+      xr[q] = make_double2(lagr6(a.x, a.y, b.x, b.y, c.x, c.y), lagr6(b.x, b.y, c.x, c.y, d.x, d.y));
+    }
+    const double2 f = dir > 0 ? xr[0] : xr[1], s = dir > 0 ? xr[1] : xr[0];  // first / second in marching order
+    const double2 done = make_double2(a0.x + (R1 * f.x + R0 * s.x), a0.y + (R1 * f.y + R0 * s.y));
+    a0 = make_double2(a1.x + R2 * (f.x + s.x), a1.y + R2 * (f.y + s.y));
+    a1 = make_double2(R0 * f.x + R1 * s.x, R0 * f.y + R1 * s.y);
+    double* sx = sX + (i & 1) * (RFY * SXP);
+    if (i >= 2) *reinterpret_cast<double2*>(sx + row * SXP + 2 * xp) = done;
+    __syncthreads();  // the x,z-restricted plane is visible; every thread is done with stage st
+    if (tid == 0 && i + NSTR < npairs) issue(i + NSTR);
+    if (i >= 2 && active) {
+      const double* c = sx + 2 * ty * SXP + tx;
+      dst[(long long)(pair_m(i) - dir) * pa.plane] =
+          lagr6(c[0], c[SXP], c[2 * SXP], c[3 * SXP], c[4 * SXP], c[5 * SXP]);
     }
   }
 }
 
-void launch_restrict_opt(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st) {
+namespace {
+size_t restrict_smem() { return (size_t)(NSTR * RSTAGE + 2 * RFY * SXP) * 8 + NSTR * 8 + 128; }
+}  // namespace
+
+void restrict_box_dims(unsigned box[4]) { box[0] = RPITCH; box[1] = RFY; box[2] = 2; box[3] = 1; }
+
+void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st) {
+  if (!a.tmap) { launch_restrict_ref(a.child, a.parent, a.V, a.ychild, a.yparent, st); return; }
+  static const int forced = [] { const char* e = getenv("SC_RCHUNKS"); return e ? atoi(e) : 0; }();
+  static const int nsm = [] {
+    int dev = 0, n = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    return n > 0 ? n : 148;
+  }();
+  static bool configured = false;
+  if (!configured) {
+    cudaFuncSetAttribute(restrict_zmarch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)restrict_smem());
+    configured = true;
+  }
+  const BoxView& ch = a.child;
   const int npx = ch.n[0] / 2, npy = ch.n[1] / 2, npz = ch.n[2] / 2;
   const int gx = (npx + RPX - 1) / RPX, gy = (npy + RPY - 1) / RPY;
-  // enough CTAs for ~4 per SM: split z into chunks of at least 8 parent planes
-  int pz = npz;
-  while (pz > 8 && (long long)gx * gy * V * ((npz + pz - 1) / pz) < 148 * 6) pz = (pz + 1) / 2;
-  const int nzc = (npz + pz - 1) / pz;
-  dim3 grd(gx, gy, nzc * V);
-  restrict_zmarch<<<grd, RPX * RPY, 0, st>>>(ch, pa, yc, yp, pz);
+  // z-chunks: whole waves of CTAs (3 per SM), few halo pairs
+  const long long cols = (long long)gx * gy * a.V, slots = 3LL * nsm;
+  int best = 1;
+  double best_cost = 1e300;
+  const int maxch = npz / 4 > 1 ? npz / 4 : 1;
+  for (int nch = 1; nch <= maxch; ++nch) {
+    const int pz = (npz + nch - 1) / nch;
+    const long long ctas = cols * ((npz + pz - 1) / pz);
+    const double cost = (double)((ctas + slots - 1) / slots) * (pz + 2 + 3);
+    if (cost < best_cost - 1e-9) { best_cost = cost; best = nch; }
+  }
+  if (forced > 0) best = forced < npz ? forced : npz;
+  RestrictParams p{};
+  p.ch = ch;
+  p.pa = a.parent;
+  p.a_child = a.a_child;
+  p.pz_per_cta = (npz + best - 1) / best;
+  p.nzc = (npz + p.pz_per_cta - 1) / p.pz_per_cta;
+  p.yp = a.yparent;
+  dim3 grd(gx, gy, p.nzc * a.V);
+  restrict_zmarch<<<grd, RNT, restrict_smem(), st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
 }
 
 }  // namespace sc

@@ -332,13 +332,15 @@ void launch_zmarch(const StageArgs& a, cudaStream_t st) {
 
 }  // namespace
 
-bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, void* out_map128) {
+void stage_box_dims(unsigned box[4]) { box[0] = HX; box[1] = HY; box[2] = 1; box[3] = 1; }
+
+bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned bx[4], void* out_map128) {
   EncodeTiledFn enc = encode_tiled();
   if (!enc) return false;
   if (b.px > (1 << 30) || (reinterpret_cast<uintptr_t>(base) & 15)) return false;
   const cuuint64_t dims[4] = {(cuuint64_t)b.px, (cuuint64_t)b.py, (cuuint64_t)b.pz, (cuuint64_t)narrays};
   const cuuint64_t strides[3] = {(cuuint64_t)b.px * 8, (cuuint64_t)b.plane * 8, (cuuint64_t)b.vol * 8};
-  const cuuint32_t box[4] = {HX, HY, 1, 1};
+  const cuuint32_t box[4] = {bx[0], bx[1], bx[2], bx[3]};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   CUtensorMap m;
   const CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
