@@ -1,0 +1,146 @@
+"""GPU parity at BASELINE.json's full box sizes, in the launch configuration bench.py times.
+
+The kernels' grids, tiles, z-chunks and tensor maps depend on the BOX shape (and F), not on how many levels
+are stacked, so every kernel launch configuration of cfg 3 / 4 / 5 is exercised by a hierarchy of the same
+boxes truncated to the depth the CPU oracle finishes in seconds; those are compared element by element.
+The full-depth cfg-5 hierarchy (what bench.py times) is then checked through properties that hold at any
+size: exact homogeneity under scaling by 2 (bit-exact), reflection symmetry of symmetric data (to
+rounding), graph replay = eager launches (bit-exact), and agreement of its level-0 and level-1 data far
+from the refined region with the truncated run the oracle verified (finite propagation speed: the 13-point
+stencil moves information at most 8 cells per level-step)."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2503_09629_b200 as sc
+from paper_2503_09629_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+RTOL = 1e-11
+
+
+def _compare_all(G, O, w, what):
+    scale = max(np.max(np.abs(O.read_level(l, ib, c))) for l in range(w.nlevels)
+                for ib in range(len(w.level_boxes(l))) for c in range(w.ncomp))
+    worst = 0.0
+    for l in range(w.nlevels):
+        for ib in range(len(w.level_boxes(l))):
+            for c in range(w.ncomp):
+                a = G.sc_debug_read_padded(l, ib, c)
+                b = O.read(l, ib, c, padded=True)
+                d = float(np.max(np.abs(a - b)))
+                worst = max(worst, d)
+                assert d <= RTOL * scale, f"{what}: level {l} box {ib} comp {c}: max|d|={d:.3e} scale={scale:.3e}"
+    return worst / scale
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_cfg5_boxes_three_levels(sub):
+    """256^3 boxes (cfg 5), 3 levels, one coarse step: every element of every level, ghosts included."""
+    w = wl.cfg5(256, 3)
+    G, O = sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, sub)
+    O.step(w.dt_coarse, sub)
+    rel = _compare_all(G, O, w, f"cfg5/256 x3 sub={sub}")
+    print(f"cfg5 256^3 x 3 levels sub={sub}: max rel diff {rel:.2e}")
+    G.close()
+    O.close()
+
+
+def test_cfg3_full_size_two_steps():
+    """cfg 3 as BASELINE states it (4 levels x 128^3), 2 coarse steps subcycled + 1 uniform."""
+    w = wl.cfg3()
+    G, O = sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+    for sub in (True, True, False):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+    rel = _compare_all(G, O, w, "cfg3 full")
+    print(f"cfg3 full size: max rel diff {rel:.2e}")
+    G.close()
+    O.close()
+
+
+def test_cfg4_boxes_full_fields():
+    """cfg 4's boxes (96^3 and the two 80x96x96 siblings) with all 22 coupled fields, 3 levels deep."""
+    w = wl.cfg4(96, 3, 22)
+    assert [b.n for b in w.level_boxes(2)] == [(80, 96, 96), (80, 96, 96)]
+    G, O = sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, True)
+    O.step(w.dt_coarse, True)
+    rel = _compare_all(G, O, w, "cfg4/96 x3 F=22")
+    print(f"cfg4 96^3 x 3 levels, 22 fields: max rel diff {rel:.2e}")
+    G.close()
+    O.close()
+
+
+def _noise_free(w):
+    """Same workload with the noise removed: the Gaussian is symmetric under every reflection of the cube."""
+    return wl.Workload(w.name + " (no noise)", w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi,
+                       w.coupling, w.coarse_steps, wl.gaussian_init(2 * 0.05 ** 2, noise=0.0))
+
+
+def test_cfg5_full_depth_properties():
+    """The exact hierarchy bench.py times (6 levels x 256^3), one subcycled coarse step."""
+    w = wl.cfg5()
+    G = sc.Hierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, True)
+    out = {(l, c): G.sc_read_level(l, 0, c) for l in range(w.nlevels) for c in range(2)}
+    for a in out.values():
+        assert np.isfinite(a).all()
+    # (1) homogeneity: every operation of the step is linear and scaling by 2 is exact in binary floating
+    # point, so step(2 y) == 2 step(y) bit for bit — a wrong constant term or a stale buffer breaks it
+    for l in range(w.nlevels):
+        for c in range(2):
+            G.sc_set_state(l, 0, c, 2.0 * w.initial_state(l, 0, c))
+    G.sc_step(w.dt_coarse, True)
+    for (l, c), a in out.items():
+        assert np.array_equal(G.sc_read_level(l, 0, c), 2.0 * a), (l, c)
+    G.close()
+    # (2) levels 0 and 1 away from the refined region equal the oracle-verified truncated run: one coarse step
+    # moves information at most 4 stages x 2 cells per level-step; level 1 takes 2 level-steps, and restriction
+    # reaches 3 fine cells, so 64 cells of margin around the level-2 footprint is ample
+    w3 = wl.cfg5(256, 3)
+    G3 = sc.Hierarchy.from_workload(w3)
+    G3.sc_step(w3.dt_coarse, True)
+    m = np.ones((256, 256, 256), dtype=bool)
+    m[32:224, 32:224, 32:224] = False    # level 2 covers level-1 cells 64..191
+    for c in range(2):
+        assert np.array_equal(G3.sc_read_level(1, 0, c)[m], out[(1, c)][m])
+    m0 = np.ones((256, 256, 256), dtype=bool)
+    m0[48:208, 48:208, 48:208] = False   # level 1 covers level-0 cells 64..191
+    for c in range(2):
+        assert np.array_equal(G3.sc_read_level(0, 0, c)[m0], out[(0, c)][m0])
+    G3.close()
+
+
+def test_cfg5_full_depth_reflection_symmetry():
+    """Noise-free Gaussian on the centred 6 x 256^3 hierarchy stays symmetric under x -> -x, y -> -y, z -> -z
+    and under axis permutations, to rounding: catches any tile / chunk / slab whose indexing is off at this size."""
+    w = _noise_free(wl.cfg5())
+    G = sc.Hierarchy.from_workload(w)
+    for _ in range(2):
+        G.sc_step(w.dt_coarse, True)
+    for l in range(w.nlevels):
+        for c in range(2):
+            a = G.sc_debug_read_padded(l, 0, c)
+            s = max(float(np.max(np.abs(a))), 1e-300)
+            for ax in range(3):
+                assert np.max(np.abs(a - np.flip(a, axis=ax))) <= RTOL * s, (l, c, ax)
+            assert np.max(np.abs(a - a.transpose(2, 1, 0))) <= RTOL * s, (l, c, "zx")
+            assert np.max(np.abs(a - a.transpose(0, 2, 1))) <= RTOL * s, (l, c, "xy")
+    G.close()
+
+
+def test_cfg5_uniform_mode_full_depth_finite_and_close_to_subcycled():
+    """Both modes on the full hierarchy agree to truncation level (north_star), here after one coarse step."""
+    w = wl.cfg5()
+    Gs, Gu = sc.Hierarchy.from_workload(w), sc.Hierarchy.from_workload(w)
+    Gs.sc_step(w.dt_coarse, True)
+    Gu.sc_step(w.dt_coarse, False)
+    assert abs(Gs.sc_time() - Gu.sc_time()) < 1e-15
+    for l in range(w.nlevels):
+        a, b = Gs.sc_read_level(l, 0, 0), Gu.sc_read_level(l, 0, 0)
+        assert np.isfinite(a).all() and np.isfinite(b).all()
+        assert np.max(np.abs(a - b)) < 2e-5, (l, float(np.max(np.abs(a - b))))
+    Gs.close()
+    Gu.close()
