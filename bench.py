@@ -141,6 +141,21 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
+# N > 1: replicas only. The only cross-rank arithmetic of the bench: the step time is
+# the MAX over ranks, the value the work of all replicas divided by it.
+def max_over_ranks(x: float, dist, device) -> float:
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, units_per_step: float, steps: int, seconds: float) -> float:
+    return world * units_per_step * steps / seconds
+
+
 def run_gpu(args):
     import torch
 
@@ -199,11 +214,8 @@ def run_gpu(args):
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
     launches = H.sc_launch_count() - n0
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    value = world * upd_step * args.steps / (ms_total * 1e-3)
+    ms_total = max_over_ranks(ms_total, dist, f"cuda:{local}")
+    value = whole_job_value(world, upd_step, args.steps, ms_total * 1e-3)
 
     # ---- per-kernel roofline: same steps launched one by one with an event pair per kernel ---------
     peak, peak_src = measured_peaks()
@@ -239,11 +251,8 @@ def run_gpu(args):
             H.sc_read_level(*k, t.numpy())
     barrier()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e = {"value": world * upd_step * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+    e2e_s = max_over_ranks(e2e_s, dist, f"cuda:{local}")
+    e2e = {"value": whole_job_value(world, upd_step, e2e_steps, e2e_s), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
            "d2h_bytes_per_step": state_bytes, "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps}
     finite = all(bool(torch.isfinite(t).all()) for t in host_out.values())
     H.close()
