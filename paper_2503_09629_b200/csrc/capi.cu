@@ -51,6 +51,10 @@ struct sc_hierarchy {
   double time = 0.0;
   uint64_t launches = 0;
   bool use_graph = true;
+  bool debug_sync = false;
+  uint64_t debug_seq = 0;
+  int debug_kind = 0;
+  std::string debug_fail;
   std::map<GraphKey, GraphEntry> graphs;
   struct BoxTiles { GhostTile* dev = nullptr; int n = 0; };
   std::vector<BoxTiles> tiles;    // per box (levels >= 1): ghost-shell tile list on the device
@@ -58,6 +62,9 @@ struct sc_hierarchy {
   std::vector<TMap> tmaps;        // per box: CUtensorMap over all arrays of the box (stage-kernel tile)
   std::vector<TMap> rmaps;        // per box: same tensor, box = the restriction kernel's fine-plane pair
   std::vector<char> tmap_ok;
+  struct GMaps { TMap m[3]; };
+  std::vector<GMaps> gmaps;       // per box: ghost-fill footprint maps of the box as PARENT (thin axis x, y, z)
+  std::vector<char> gmap_ok;
   // per-launch CUDA-event timing (sc_profile): eager launches, one event pair per kernel
   bool profiling = false;
   struct ProfRec { int kind; double bytes; cudaEvent_t e0, e1; };
@@ -147,6 +154,7 @@ double stage_bytes(const BoxView& v, int F, int mode, int write_Y4r) {
 }
 
 void prof_begin(sc_hierarchy* h, int kind, double bytes) {
+  h->debug_kind = kind;
   if (!h->profiling) return;
   sc_hierarchy::ProfRec r{kind, bytes, nullptr, nullptr};
   cudaEventCreate(&r.e0);
@@ -155,6 +163,14 @@ void prof_begin(sc_hierarchy* h, int kind, double bytes) {
   h->prof.push_back(r);
 }
 void prof_end(sc_hierarchy* h) {
+  if (h->debug_sync) {  // SC_DEBUG_SYNC=1 (with SC_GRAPH=0): name the first failing launch
+    const cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess && h->debug_fail.empty()) {
+      h->debug_fail = "launch #" + std::to_string(h->debug_seq) + " (kind " + std::to_string(h->debug_kind) + ") failed: " + cudaGetErrorString(e);
+      fprintf(stderr, "libsubcycle: %s\n", h->debug_fail.c_str());
+    }
+    ++h->debug_seq;
+  }
   if (!h->profiling) return;
   cudaEventRecord(h->prof.back().e1, h->stream);
 }
@@ -209,9 +225,15 @@ void ghost_launch(Seq& q, int ib, GhostArgs& a) {
   a.child = b.v;
   a.parent = h->L.boxes[b.parent].v;
   a.F = h->L.F;
+  a.parent_base = h->arr(b.parent, 0);
+  a.child_base = h->arr(ib, 0);
   a.tiles = h->tiles[ib].dev;
   a.ntiles = h->tiles[ib].n;
-  prof_begin(h, KIND_GHOST, 8.0 * h->L.F * (a.nsrc * footprint_cells(b.v) + a.nout * shell_cells(b.v)));
+  a.tmaps = h->gmap_ok[b.parent] ? h->gmaps[b.parent].m[0].bytes : nullptr;
+  double bytes = 0.0;
+  for (int p = 0; p < a.nprob; ++p)
+    bytes += 8.0 * h->L.F * (a.prob[p].nsrc * footprint_cells(b.v) + a.prob[p].nout * shell_cells(b.v));
+  prof_begin(h, KIND_GHOST, bytes);
   launch_ghost_fill(a, h->stream);
   prof_end(h);
   ++q.n;
@@ -239,35 +261,37 @@ void fill_level_dense(Seq& q, int level, double theta, double dt) {
   double c1[4], cs[4];
   dense_coeffs(1, theta, c1);
   for (int ib : L.level_boxes[level]) {
-    const int ip = L.boxes[ib].parent;
     GhostArgs a{};
-    a.nsrc = 5;
-    a.src[0] = h->arr(ip, L.a_state(pold));
-    a.src[1] = h->arr(ip, L.a_state(pold) + L.F);
-    a.src[2] = h->arr(ip, L.a_Y2r());
-    a.src[3] = h->arr(ip, L.a_Y3r());
-    a.src[4] = h->arr(ip, L.a_Y4r());
-    a.nout = 4;
-    a.dst[0] = h->arr(ib, L.a_state(yn));
-    a.dst[1] = h->arr(ib, L.a_state(yn) + L.F);
-    a.dst[2] = h->arr(ib, L.a_Y2r());
-    a.dst[3] = h->arr(ib, L.a_Y3r());
-    a.coef[0][0] = 1.0;
-    for (int j = 0; j < 4; ++j) a.coef[0][1 + j] = hp * c1[j];
+    a.nprob = 1;
+    GhostProblem& d = a.prob[0];
+    d.nsrc = 5;
+    d.src_arr[0] = L.a_state(pold);
+    d.src_arr[1] = L.a_state(pold) + L.F;
+    d.src_arr[2] = L.a_Y2r();
+    d.src_arr[3] = L.a_Y3r();
+    d.src_arr[4] = L.a_Y4r();
+    d.nout = 4;
+    d.dst_arr[0] = L.a_state(yn);
+    d.dst_arr[1] = L.a_state(yn) + L.F;
+    d.dst_arr[2] = L.a_Y2r();
+    d.dst_arr[3] = L.a_Y3r();
+    d.coef[0][0] = 1.0;
+    for (int j = 0; j < 4; ++j) d.coef[0][1 + j] = hp * c1[j];
     const double as[3] = {0.5, 0.5, 1.0};
     for (int s = 0; s < 3; ++s) {
       dense_coeffs(s + 2, theta, cs);
-      for (int j = 0; j < 4; ++j) a.coef[1 + s][1 + j] = 2.0 * (cs[j] - c1[j]) / as[s];  // h_p / (a_s dt) = 2 / a_s
+      for (int j = 0; j < 4; ++j) d.coef[1 + s][1 + j] = 2.0 * (cs[j] - c1[j]) / as[s];  // h_p / (a_s dt) = 2 / a_s
     }
-    if (theta != 0.0) {
-      a.nsrc = 7;
-      a.src[5] = h->arr(ip, L.a_state(pnew));
-      a.src[6] = h->arr(ip, L.a_state(pnew) + L.F);
-      a.nout = 6;
-      a.dst[4] = h->arr(ib, L.a_state(1 - yn));
-      a.dst[5] = h->arr(ib, L.a_state(1 - yn) + L.F);
-      a.coef[4][5] = 1.0;
-      a.coef[5][6] = 1.0;
+    if (theta != 0.0) {  // second problem: same-time prolongation of the parent's new state into y_{n+1}
+      a.nprob = 2;
+      GhostProblem& e = a.prob[1];
+      e.nsrc = e.nout = 2;
+      e.src_arr[0] = L.a_state(pnew);
+      e.src_arr[1] = L.a_state(pnew) + L.F;
+      e.dst_arr[0] = L.a_state(1 - yn);
+      e.dst_arr[1] = L.a_state(1 - yn) + L.F;
+      e.coef[0][0] = 1.0;
+      e.coef[1][1] = 1.0;
     }
     ghost_launch(q, ib, a);
   }
@@ -277,13 +301,14 @@ void fill_level_dense(Seq& q, int level, double theta, double dt) {
 void fill_level_same_time(Seq& q, int level, int n, const int* child_arrays, const int* parent_arrays) {
   sc_hierarchy* h = q.h;
   for (int ib : h->L.level_boxes[level]) {
-    const int ip = h->L.boxes[ib].parent;
     GhostArgs a{};
-    a.nsrc = a.nout = n;
+    a.nprob = 1;
+    GhostProblem& d = a.prob[0];
+    d.nsrc = d.nout = n;
     for (int s = 0; s < n; ++s) {
-      a.src[s] = h->arr(ip, parent_arrays[s]);
-      a.dst[s] = h->arr(ib, child_arrays[s]);
-      a.coef[s][s] = 1.0;
+      d.src_arr[s] = parent_arrays[s];
+      d.dst_arr[s] = child_arrays[s];
+      d.coef[s][s] = 1.0;
     }
     ghost_launch(q, ib, a);
   }
@@ -498,10 +523,15 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   h->tmaps.resize(h->L.boxes.size());
   h->tmap_ok.assign(h->L.boxes.size(), 0);
   h->rmaps.resize(h->L.boxes.size());
+  h->gmaps.resize(h->L.boxes.size());
+  h->gmap_ok.assign(h->L.boxes.size(), 0);
   for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
     const BoxInfo& b = h->L.boxes[ib];
     h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
+    h->gmap_ok[ib] = 1;
+    for (int ax = 0; ax < 3; ++ax)
+      if (!make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 2 + ax, h->gmaps[ib].m[ax].bytes)) h->gmap_ok[ib] = 0;
   }
   if ((ce = cudaStreamSynchronize(h->stream)) != cudaSuccess) return bail("sync", ce);
   h->cur.assign(h->L.nlevels, 0);
@@ -510,6 +540,8 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   select_kernels(env && !strcmp(env, "ref") ? 0 : 1);
   const char* eg = getenv("SC_GRAPH");
   h->use_graph = !(eg && !strcmp(eg, "0"));
+  const char* ed = getenv("SC_DEBUG_SYNC");
+  h->debug_sync = ed && !strcmp(ed, "1") && !h->use_graph;
   *out = h;
   return SC_OK;
 }

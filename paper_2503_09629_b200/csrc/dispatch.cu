@@ -1,4 +1,4 @@
-// dispatch.cu — picks the kernel set: the tuned sm_100a kernels (default: stage_tma.cu, ghost_tiled.cu,
+// dispatch.cu — picks the kernel set: the tuned sm_100a kernels (default: stage_tma.cu, ghost_tma.cu,
 // restrict_zmarch.cu) or the straightforward direct-load kernels of kernels_basic.cu (environment
 // SC_KERNELS=ref; A/B checks and debugging only). Both are CUDA; there is no CPU path.
 #include "kernels.h"
@@ -11,7 +11,9 @@ bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const un
 void stage_box_dims(unsigned box[4]);
 void restrict_box_dims(unsigned box[4]);
 void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
-void launch_ghost_fill_tiled(const GhostArgs& a, cudaStream_t st);
+void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st);
+bool ghost_tma_takes(const GhostArgs& a);
+void ghost_box_dims(int axis, unsigned box[4]);
 void launch_restrict_ref(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st);
 void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st);
 
@@ -24,8 +26,8 @@ void launch_stage(const StageArgs& a, cudaStream_t st) {
   else launch_stage_tma(a, st);
 }
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st) {
-  if (g_mode == 0 || a.ntiles == 0) launch_ghost_fill_direct(a, st);
-  else launch_ghost_fill_tiled(a, st);
+  if (g_mode == 0 || !ghost_tma_takes(a)) launch_ghost_fill_direct(a, st);
+  else launch_ghost_fill_tma(a, st);
 }
 void launch_restrict(const RestrictArgs& a, cudaStream_t st) {
   if (g_mode == 0) launch_restrict_ref(a.child, a.parent, a.V, a.ychild, a.yparent, st);
@@ -34,7 +36,8 @@ void launch_restrict(const RestrictArgs& a, cudaStream_t st) {
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128) {
   unsigned box[4];
   if (kind == 0) stage_box_dims(box);
-  else restrict_box_dims(box);
+  else if (kind == 1) restrict_box_dims(box);
+  else ghost_box_dims(kind - 2, box);
   return make_box_tensor_map_tma(b, narrays, base, box, out_map128);
 }
 

@@ -44,35 +44,48 @@ struct StageArgs {
 };
 void launch_stage(const StageArgs& a, cudaStream_t st);
 // 128-byte CUtensorMaps of a box: dims (px, py, pz, narrays), fp64, no swizzle; kind 0: box = the stage
-// kernels' halo tile, kind 1: box = the restriction kernel's pair of fine planes. Returns false (and leaves
+// kernels' halo tile, kind 1: box = the restriction kernel's pair of fine planes, kinds 2..4: the ghost
+// fill's parent footprint of a tile of an x- / y- / z-slab. Returns false (and leaves
 // the direct-load kernels in charge) when the driver entry point is unavailable or a TMA limit is violated.
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128);
 
 // ------------------------------------------------------------------------------------------------
-// a3: refinement-boundary ghost fill. For every ghost cell of a level >= 1 box and every output o:
-//     dst[o](ghost) = P[ sum_s coef[o][s] * src[s] ]     P = 5x5x5 tensor quartic Lagrange (S3)
-// over parent arrays src[s]. The dense-output time polynomial (eqs 10-18) is folded into coef by the
-// scheduler, which asks for all ghost shells one child level-step needs in ONE launch. Field f of every
-// src/dst is f arrays further (src[s] + f*parent.vol, dst[o] + f*child.vol).
+// a3: refinement-boundary ghost fill. One launch fills, for every ghost cell of a level >= 1 box, the shells
+// of up to GF_MAX_PROB independent PROBLEMS; problem p writes, for every output o,
+//     child array dst_arr[o] (ghost cell) = P[ sum_s coef[o][s] * parent array src_arr[s] ]
+// with P = 5x5x5 tensor quartic Lagrange (S3). The dense-output time polynomial (eqs 10-18) is folded into
+// coef by the scheduler, which asks for all ghost shells one child level-step needs in ONE launch: the
+// (5 sources -> 4 outputs) dense-output problem and, when the step ends at the parent's t_{n+1}, the
+// (2 -> 2) same-time prolongation of the parent's new state. Arrays are named by their index inside the
+// box (sc_internal.h); field f of every source / output is f arrays further.
 // ------------------------------------------------------------------------------------------------
-constexpr int GF_MAX_SRC = 7, GF_MAX_OUT = 6;
+constexpr int GF_MAX_SRC = 5, GF_MAX_OUT = 4, GF_MAX_PROB = 2;
 
 struct GhostTile {   // a piece of one ghost slab, box-local fine indices
   int lo[3];
   int n[3];
+  int org[3];        // origin of the tile grid cell this piece lies in (even; lo - org < tile size)
   int axis;          // the slab's thin axis: 0 = x-slab, 1 = y-slab, 2 = z-slab
-  int pad;
+};
+
+struct GhostProblem {
+  int nsrc, nout;
+  int src_arr[GF_MAX_SRC];
+  int dst_arr[GF_MAX_OUT];
+  double coef[GF_MAX_OUT][GF_MAX_SRC];
 };
 
 struct GhostArgs {
   BoxView child, parent;
   int F;
-  int nsrc, nout;
-  const double* src[GF_MAX_SRC];
-  double* dst[GF_MAX_OUT];
-  double coef[GF_MAX_OUT][GF_MAX_SRC];
-  const GhostTile* tiles;  // device; tile list of the child box (built once per box)
+  int nprob;
+  const double* parent_base;  // array 0 of the parent box
+  double* child_base;         // array 0 of the child box
+  GhostProblem prob[GF_MAX_PROB];
+  const GhostTile* tiles;     // device; tile list of the child box (built once per box)
   int ntiles;
+  const void* tmaps;          // host pointer to the parent's three footprint CUtensorMaps (thin axis x, y, z;
+                              // 128 bytes each, contiguous), or null -> direct-load kernel
 };
 void build_ghost_tiles(const BoxView& child, std::vector<GhostTile>& tiles);
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st);

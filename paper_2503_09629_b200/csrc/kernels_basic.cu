@@ -1,6 +1,6 @@
 // kernels_basic.cu — straightforward CUDA kernels of every step of the hot path (one thread per output
 // cell, gathers straight from global memory). They define the arithmetic of the CUDA path; the tuned
-// kernels (stage_tma.cu, ghost_tiled.cu, restrict_zmarch.cu) must agree with them to rounding. Selected
+// kernels (stage_tma.cu, ghost_tma.cu, restrict_zmarch.cu) must agree with them to rounding. Selected
 // with SC_KERNELS=ref; also the home of the periodic fill, pack/unpack and the ghost-map debug kernel.
 //
 // Index conventions: box-local cell (i,j,k), i fastest; level-global index I = lo + i; the parent cell
@@ -144,12 +144,13 @@ void launch_stage_direct(const StageArgs& a, cudaStream_t st) {
 // ------------------------------------------------------------------------------------------------
 // a3  ghost fill, direct version: one thread per (ghost cell, field), 125-point gather per source
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) ghost_fill_direct(GhostArgs a, long long nshell) {
+__global__ void __launch_bounds__(128) ghost_fill_direct(GhostArgs a, int ip, long long nshell) {
   const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int f = blockIdx.y;
   if (q >= nshell) return;
   int i, j, k;
   if (!shell_cell(a.child, q, i, j, k)) return;
+  const GhostProblem& pr = a.prob[ip];
   const int I[3] = {a.child.lo[0] + i, a.child.lo[1] + j, a.child.lo[2] + k};
   int J[3], p[3];
 #pragma unroll
@@ -157,41 +158,41 @@ __global__ void __launch_bounds__(128) ghost_fill_direct(GhostArgs a, long long 
     J[d] = (I[d] >> 1) - a.parent.lo[d];
     p[d] = I[d] & 1;
   }
-  const long long pv = (long long)f * a.parent.vol;
   double acc[GF_MAX_OUT];
 #pragma unroll
   for (int o = 0; o < GF_MAX_OUT; ++o) acc[o] = 0.0;
   for (int cc = -2; cc <= 2; ++cc)
     for (int bb = -2; bb <= 2; ++bb) {
-      const long long row = pv + cell_offset(a.parent, J[0], J[1] + bb, J[2] + cc);
+      const long long row = cell_offset(a.parent, J[0], J[1] + bb, J[2] + cc);
       const double wyz = c_wp[p[1]][bb + 2] * c_wp[p[2]][cc + 2];
       for (int aa = -2; aa <= 2; ++aa) {
         const double w = wyz * c_wp[p[0]][aa + 2];
         double v[GF_MAX_SRC];
 #pragma unroll
-        for (int s = 0; s < GF_MAX_SRC; ++s) v[s] = s < a.nsrc ? a.src[s][row + aa] : 0.0;
+        for (int s = 0; s < GF_MAX_SRC; ++s)
+          v[s] = s < pr.nsrc ? a.parent_base[(long long)(pr.src_arr[s] + f) * a.parent.vol + row + aa] : 0.0;
 #pragma unroll
         for (int o = 0; o < GF_MAX_OUT; ++o) {
-          if (o < a.nout) {
+          if (o < pr.nout) {
             double t = 0.0;
 #pragma unroll
             for (int s = 0; s < GF_MAX_SRC; ++s)
-              if (s < a.nsrc) t = fma(a.coef[o][s], v[s], t);
+              if (s < pr.nsrc) t = fma(pr.coef[o][s], v[s], t);
             acc[o] = fma(w, t, acc[o]);
           }
         }
       }
     }
-  const long long dofs = (long long)f * a.child.vol + cell_offset(a.child, i, j, k);
+  const long long dofs = cell_offset(a.child, i, j, k);
 #pragma unroll
   for (int o = 0; o < GF_MAX_OUT; ++o)
-    if (o < a.nout) a.dst[o][dofs] = acc[o];
+    if (o < pr.nout) a.child_base[(long long)(pr.dst_arr[o] + f) * a.child.vol + dofs] = acc[o];
 }
 
 void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st) {
   const long long ns = ghost_cell_count(a.child);
   dim3 grd((unsigned)((ns + 127) / 128), a.F, 1);
-  ghost_fill_direct<<<grd, 128, 0, st>>>(a, ns);
+  for (int ip = 0; ip < a.nprob; ++ip) ghost_fill_direct<<<grd, 128, 0, st>>>(a, ip, ns);
 }
 
 // ------------------------------------------------------------------------------------------------
