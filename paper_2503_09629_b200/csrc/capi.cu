@@ -201,11 +201,11 @@ void stage_level(Seq& q, int level, int mode, double dt) {
       a.inv12dx2[d] = 1.0 / (12.0 * dx * dx);
     }
     a.A = h->coupling();
+    a.S = a.A ? h->arr(ib, L.a_scratch()) : nullptr;
     a.tmap = h->tmap_ok[ib] ? h->tmaps[ib].bytes : nullptr;
     prof_begin(h, KIND_STAGE, stage_bytes(a.b, L.F, mode, a.write_Y4r));
-    launch_stage(a, h->stream);
+    q.n += launch_stage(a, h->stream);
     prof_end(h);
-    ++q.n;
   }
 }
 

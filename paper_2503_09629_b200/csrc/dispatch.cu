@@ -6,7 +6,7 @@
 namespace sc {
 
 void launch_stage_direct(const StageArgs& a, cudaStream_t st);
-void launch_stage_tma(const StageArgs& a, cudaStream_t st);
+int launch_stage_tma(const StageArgs& a, cudaStream_t st);
 bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned box[4], void* out_map128);
 void stage_box_dims(unsigned box[4]);
 void restrict_box_dims(unsigned box[4]);
@@ -21,9 +21,9 @@ static int g_mode = 1;
 void select_kernels(int mode) { g_mode = mode; }
 int selected_kernels() { return g_mode; }
 
-void launch_stage(const StageArgs& a, cudaStream_t st) {
-  if (g_mode == 0) launch_stage_direct(a, st);
-  else launch_stage_tma(a, st);
+int launch_stage(const StageArgs& a, cudaStream_t st) {
+  if (g_mode == 0) { launch_stage_direct(a, st); return 1; }
+  return launch_stage_tma(a, st);
 }
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st) {
   if (g_mode == 0 || !ghost_tma_takes(a)) launch_ghost_fill_direct(a, st);

@@ -38,11 +38,12 @@ struct StageArgs {
   double dt;
   double inv12dx2[3];  // 1 / (12 dx_a^2)
   const double* A;     // device F*F row-major coupling, or null
+  double* S;           // coupled systems: 2F scratch arrays for the coupling terms (A W) of the two operands
   // TMA path: tensor map of the box (all arrays as the 4th dimension) and the array indices of the roles
   const void* tmap;    // host pointer to the box's CUtensorMap, or null -> direct-load kernel
   int a_yn, a_Y2r, a_Y3r;
 };
-void launch_stage(const StageArgs& a, cudaStream_t st);
+int launch_stage(const StageArgs& a, cudaStream_t st);  // returns the number of kernels launched
 // 128-byte CUtensorMaps of a box: dims (px, py, pz, narrays), fp64, no swizzle; kind 0: box = the stage
 // kernels' halo tile, kind 1: box = the restriction kernel's pair of fine planes, kinds 2..4: the ghost
 // fill's parent footprint of a tile of an x- / y- / z-slab. Returns false (and leaves

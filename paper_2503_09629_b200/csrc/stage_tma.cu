@@ -71,6 +71,7 @@ struct TmaStageParams {
   double* ynew;
   double dt;
   double w[3];  // 1 / (12 dx_a^2)
+  const double* S;  // coupled systems: F arrays A*(first stage operand), then F arrays A*(second), from couple_matvec
 };
 
 // values of one array around the thread's two cells (x, x+1) in the current plane
@@ -125,7 +126,7 @@ __device__ __forceinline__ void scatter(double2 (&acc)[5], double2 centre_term, 
 
 }  // namespace
 
-template <int MODE>
+template <int MODE, bool COUPLED>
 __global__ void __launch_bounds__(NTHR, 2)
     stage_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ TmaStageParams p) {
   constexpr int NH = MODE == STAGE_12 ? 2 : 3;  // halo-read arrays per plane
@@ -179,6 +180,10 @@ __global__ void __launch_bounds__(NTHR, 2)
   const double* __restrict__ rho_g = p.yn + (long long)(p.F + f) * b.vol + cell0;
   double2 rho_nxt = make_double2(0.0, 0.0);
   (void)rho_g;
+  // coupling terms (A W)_f of the two stage operands at the centre cells, read like rho_n: one plane ahead
+  const double* __restrict__ s1_g = COUPLED ? p.S + (long long)f * b.vol + cell0 : nullptr;
+  const double* __restrict__ s2_g = COUPLED ? p.S + (long long)(p.F + f) * b.vol + cell0 : nullptr;
+  double2 s1_nxt = make_double2(0.0, 0.0), s2_nxt = s1_nxt;
 
   auto step = [&](auto Rc, int it) {
     constexpr int R = decltype(Rc)::value;
@@ -186,10 +191,18 @@ __global__ void __launch_bounds__(NTHR, 2)
     const bool inpl = it >= 2 && it < narr - 2;
     const int z = zs + dir * it;
     double2 rho_c = rho_nxt;
-    if (MODE == STAGE_34) {  // rho_n is read at the centre only: plain global load, one plane ahead
+    const double2 s1_c = s1_nxt, s2_c = s2_nxt;
+    {
       const int itn = it + 1;
-      if (active && itn >= 2 && itn < narr - 2)
-        rho_nxt = __ldg(reinterpret_cast<const double2*>(rho_g + (long long)(z + dir) * b.plane));
+      if (active && itn >= 2 && itn < narr - 2) {
+        const long long zo = (long long)(z + dir) * b.plane;
+        if (MODE == STAGE_34)  // rho_n is read at the centre only: plain global load, one plane ahead
+          rho_nxt = __ldg(reinterpret_cast<const double2*>(rho_g + zo));
+        if (COUPLED) {
+          s1_nxt = __ldg(reinterpret_cast<const double2*>(s1_g + zo));
+          s2_nxt = __ldg(reinterpret_cast<const double2*>(s2_g + zo));
+        }
+      }
     }
     mbar_wait(bar0 + 8 * st, (it / NST) & 1);
     const double* __restrict__ t0 = tiles + (st * NH) * TILE_DOUBLES;
@@ -201,6 +214,7 @@ __global__ void __launch_bounds__(NTHR, 2)
         const double2 iu = inplane(u, wxA, wyA, cA), iw = inplane(w, wxB, wyB, cB);
         ctA = make_double2(r.xb.x + iu.x, r.xb.y + iu.y);
         ctB = make_double2(r.xb.x + iw.x, r.xb.y + iw.y);
+        if (COUPLED) { ctA = fma2(hdt, s1_c, ctA); ctB = fma2(hdt, s2_c, ctB); }
         zcA = make_double2(wzA * u.xb.x, wzA * u.xb.y);
         zcB = make_double2(wzB * w.xb.x, wzB * w.xb.y);
       } else {
@@ -219,6 +233,7 @@ __global__ void __launch_bounds__(NTHR, 2)
         const double prx = rho_c.x + (third * (y2.xb.x - rho_c.x) + (2.0 * third) * (y3.xb.x - rho_c.x)) - third * rho_c.x;
         const double pry = rho_c.y + (third * (y2.xb.y - rho_c.y) + (2.0 * third) * (y3.xb.y - rho_c.y)) - third * rho_c.y;
         ctB = make_double2(prx + i4.x, pry + i4.y);
+        if (COUPLED) { ctA = fma2(dt, s1_c, ctA); ctB = fma2(dt6, s2_c, ctB); }
         Pu[R] = make_double2(fma(dt6, rho_c.x + 2.0 * (y2.xb.x + y3.xb.x), u.xb.x),
                              fma(dt6, rho_c.y + 2.0 * (y2.xb.y + y3.xb.y), u.xb.y));
         zcA = make_double2(wzA * w3.xb.x, wzA * w3.xb.y);
@@ -308,11 +323,12 @@ int pick_chunks(const BoxView& b, int F, int ctas_per_sm) {
   return best;
 }
 
-template <int MODE>
+template <int MODE, bool COUPLED>
 void launch_zmarch(const StageArgs& a, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    cudaFuncSetAttribute(stage_zmarch<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stage_smem<MODE>());
+    cudaFuncSetAttribute(stage_zmarch<MODE, COUPLED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)stage_smem<MODE>());
     configured = true;
   }
   TmaStageParams p{};
@@ -326,10 +342,87 @@ void launch_zmarch(const StageArgs& a, cudaStream_t st) {
   p.yn = a.yn; p.Y2r = a.Y2r; p.Y3r = a.Y3r; p.Y4r = a.Y4r; p.ynew = a.ynew;
   p.dt = a.dt;
   for (int d = 0; d < 3; ++d) p.w[d] = a.inv12dx2[d];
+  p.S = a.S;
   dim3 grd((a.b.n[0] + TX - 1) / TX, (a.b.n[1] + TY - 1) / TY, p.nchunks * a.F);
-  stage_zmarch<MODE><<<grd, NTHR, stage_smem<MODE>(), st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
+  stage_zmarch<MODE, COUPLED><<<grd, NTHR, stage_smem<MODE>(), st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
 }
 
+}  // namespace
+
+// ---- coupled systems: the pointwise F x F product -------------------------------------------------------
+// d_t rho_f = Lap u_f + sum_q A_fq u_q (PAPER.md:222-226 with BASELINE config 4's coupling, S21/S22). The
+// Laplacian acts field by field, the coupling cell by cell across ALL fields; they are split accordingly: this
+// kernel forms, at every interior cell, the coupling terms of the two stage operands W1, W2 of the following
+// z-march launch,
+//   STAGE_12:  W1 = u_n,               W2 = u_n + dt/2 rho_n
+//   STAGE_34:  W1 = u_n + dt/2 Y2r,    W2 = u_n + dt Y3r
+// S[f] = sum_q A_fq W1_q,  S[F + f] = sum_q A_fq W2_q, and the z-march kernel adds them at the centre cell.
+// One thread per cell: all F operand pairs in registers (every global load issued up front), A in shared
+// memory (broadcast reads). 2 F^2 FMA per cell against (2|3) F reads + 2 F writes.
+namespace {
+template <int MODE, int FB>
+__global__ void __launch_bounds__(128) couple_matvec(const TmaStageParams p, const double* __restrict__ A) {
+  __shared__ double sA[FB * FB];
+  const BoxView& b = p.b;
+  const int F = p.F;
+  for (int e = threadIdx.y * 32 + threadIdx.x; e < FB * FB; e += 128) {
+    const int r = e / FB, c = e % FB;
+    sA[e] = (r < F && c < F) ? A[r * F + c] : 0.0;
+  }
+  __syncthreads();
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z;
+  if (i >= b.n[0] || j >= b.n[1]) return;
+  const long long o = cell_offset(b, i, j, k);
+  const double hdt = 0.5 * p.dt;
+  double w1[FB], w2[FB];
+#pragma unroll
+  for (int q = 0; q < FB; ++q) {
+    if (q < F) {
+      const double u = __ldg(p.yn + (long long)q * b.vol + o);
+      if (MODE == STAGE_12) {
+        w1[q] = u;
+        w2[q] = fma(hdt, __ldg(p.yn + (long long)(F + q) * b.vol + o), u);
+      } else {
+        w1[q] = fma(hdt, __ldg(p.Y2r + (long long)q * b.vol + o), u);
+        w2[q] = fma(p.dt, __ldg(p.Y3r + (long long)q * b.vol + o), u);
+      }
+    } else {
+      w1[q] = w2[q] = 0.0;
+    }
+  }
+  double* __restrict__ S = const_cast<double*>(p.S);
+  for (int f = 0; f < F; ++f) {
+    double s1 = 0.0, s2 = 0.0;
+#pragma unroll
+    for (int q = 0; q < FB; ++q) {
+      const double aq = sA[f * FB + q];
+      s1 = fma(aq, w1[q], s1);
+      s2 = fma(aq, w2[q], s2);
+    }
+    S[(long long)f * b.vol + o] = s1;
+    S[(long long)(F + f) * b.vol + o] = s2;
+  }
+}
+
+template <int MODE>
+void launch_couple_mode(const TmaStageParams& p, const double* A, cudaStream_t st) {
+  dim3 blk(32, 4, 1), grd((p.b.n[0] + 31) / 32, (p.b.n[1] + 3) / 4, p.b.n[2]);
+  if (p.F <= 8) couple_matvec<MODE, 8><<<grd, blk, 0, st>>>(p, A);
+  else if (p.F <= 16) couple_matvec<MODE, 16><<<grd, blk, 0, st>>>(p, A);
+  else if (p.F <= 24) couple_matvec<MODE, 24><<<grd, blk, 0, st>>>(p, A);
+  else couple_matvec<MODE, 32><<<grd, blk, 0, st>>>(p, A);
+}
+
+void launch_couple_matvec(const StageArgs& a, cudaStream_t st) {
+  TmaStageParams p{};
+  p.b = a.b;
+  p.F = a.F;
+  p.yn = a.yn; p.Y2r = a.Y2r; p.Y3r = a.Y3r;
+  p.dt = a.dt;
+  p.S = a.S;
+  if (a.mode == STAGE_12) launch_couple_mode<STAGE_12>(p, a.A, st);
+  else launch_couple_mode<STAGE_34>(p, a.A, st);
+}
 }  // namespace
 
 void stage_box_dims(unsigned box[4]) { box[0] = HX; box[1] = HY; box[2] = 1; box[3] = 1; }
@@ -352,10 +445,17 @@ bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const un
   return true;
 }
 
-void launch_stage_tma(const StageArgs& a, cudaStream_t st) {
-  if (a.A || !a.tmap) { launch_stage_direct(a, st); return; }
-  if (a.mode == STAGE_12) launch_zmarch<STAGE_12>(a, st);
-  else launch_zmarch<STAGE_34>(a, st);
+int launch_stage_tma(const StageArgs& a, cudaStream_t st) {
+  if (!a.tmap || (a.A && !a.S)) { launch_stage_direct(a, st); return 1; }
+  if (a.A) {  // coupling terms first (pointwise F x F product over all fields), then the per-field z-march
+    launch_couple_matvec(a, st);
+    if (a.mode == STAGE_12) launch_zmarch<STAGE_12, true>(a, st);
+    else launch_zmarch<STAGE_34, true>(a, st);
+  } else {
+    if (a.mode == STAGE_12) launch_zmarch<STAGE_12, false>(a, st);
+    else launch_zmarch<STAGE_34, false>(a, st);
+  }
+  return a.A ? 2 : 1;
 }
 
 }  // namespace sc
