@@ -512,7 +512,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
     if (h->L.boxes[ib].level == 0) continue;
     std::vector<GhostTile> tl;
-    build_ghost_tiles(h->L.boxes[ib].v, tl);
+    build_ghost_tiles(h->L.boxes[ib].v, h->L.boxes[h->L.boxes[ib].parent].v, tl);
     sc_hierarchy::BoxTiles& bt = h->tiles[ib];
     bt.n = (int)tl.size();
     if (tl.empty()) continue;

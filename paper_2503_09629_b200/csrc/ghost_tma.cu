@@ -21,7 +21,6 @@
 // A ghost value costs 6 + 5 + 5 FMA instead of 125 and every parent value is fetched once per tile.
 #include <cuda.h>
 
-#include <cstdio>
 #include <cstdlib>
 
 #include "kernels.h"
@@ -87,42 +86,18 @@ __device__ __forceinline__ int raw_idx(int ia, int ib, int c) {
   return (ib * PA + ia) * PTX + c;               // box (PTX x, PA y, PB z); c counts from the even start
 }
 
-// geometry of one tile (box-local fine indices, parent-local footprint origin)
-struct TileGeo {
-  int axT, axA, axB;
-  int oA, oB;              // even tile origin along A, B
-  int vA0, vA1, vB0, vB1;  // valid tile-local fine range
-  int q[3];                // parent-local index of footprint cell 0 along x, y, z
-  int IT0, PT0, nt;        // level-global first thin cell, parent-global first footprint cell, thin cells
-};
-__device__ __forceinline__ int sel3(int ax, int x, int y, int z) { return ax == 0 ? x : (ax == 1 ? y : z); }
-__device__ __forceinline__ TileGeo tile_geo(const BoxView& ch, const BoxView& pa, const GhostTile& t) {
-  TileGeo g;  // (no dynamically indexed local arrays: they would live in local memory)
-  g.axT = t.axis;
-  g.axA = g.axT == 0 ? 1 : 0;
-  g.axB = g.axT == 2 ? 1 : 2;
-  const int tloA = sel3(g.axA, t.lo[0], t.lo[1], t.lo[2]), tloB = sel3(g.axB, t.lo[0], t.lo[1], t.lo[2]);
-  const int tloT = sel3(g.axT, t.lo[0], t.lo[1], t.lo[2]);
-  const int chA = sel3(g.axA, ch.lo[0], ch.lo[1], ch.lo[2]), chB = sel3(g.axB, ch.lo[0], ch.lo[1], ch.lo[2]);
-  const int paA = sel3(g.axA, pa.lo[0], pa.lo[1], pa.lo[2]), paB = sel3(g.axB, pa.lo[0], pa.lo[1], pa.lo[2]);
-  g.oA = sel3(g.axA, t.org[0], t.org[1], t.org[2]);
-  g.oB = sel3(g.axB, t.org[0], t.org[1], t.org[2]);
-  g.vA0 = tloA - g.oA; g.vA1 = g.vA0 + sel3(g.axA, t.n[0], t.n[1], t.n[2]);
-  g.vB0 = tloB - g.oB; g.vB1 = g.vB0 + sel3(g.axB, t.n[0], t.n[1], t.n[2]);
-  g.IT0 = sel3(g.axT, ch.lo[0], ch.lo[1], ch.lo[2]) + tloT;
-  g.PT0 = (g.IT0 >> 1) - 2;
-  g.nt = sel3(g.axT, t.n[0], t.n[1], t.n[2]);
-  const int qA = ((chA + g.oA) >> 1) - 2 - paA, qB = ((chB + g.oB) >> 1) - 2 - paB;
-  const int qT = g.PT0 - sel3(g.axT, pa.lo[0], pa.lo[1], pa.lo[2]);
-  // axT = 2: (A, B, T) = (x, y, z);  axT = 1: (x, z, y);  axT = 0: (y, z, x)
-  g.q[0] = g.axT == 0 ? qT : qA;
-  g.q[1] = g.axT == 0 ? qA : (g.axT == 1 ? qT : qB);
-  g.q[2] = g.axT == 2 ? qT : qB;
-  return g;
-}
-
 // ---- phase 1: thin-axis interpolation of every source, then the time combination ---------------------
-template <int AX, int NS, int NO>
+// 5-point thin-axis interpolation with immediate weights (P = parity of the fine cell), depth-3 tree
+template <int P>
+__device__ __forceinline__ double ip5(const double* L) {
+  constexpr double w0 = 35.0 / 2048.0, w1 = -252.0 / 2048.0, w2 = 1890.0 / 2048.0, w3 = 420.0 / 2048.0,
+                   w4 = -45.0 / 2048.0;
+  if (P) return fma(w4, L[4], fma(w1, L[1], w0 * L[0])) + fma(w3, L[3], w2 * L[2]);
+  return fma(w0, L[4], fma(w3, L[1], w4 * L[0])) + fma(w1, L[3], w2 * L[2]);
+}
+// PAR >= 0: ghost width 3 and PAR = parity of the first thin cell: the (parent cell, parity) pattern of the
+// three thin cells is known at compile time (no weight table, no barrier). PAR < 0: any width, weights in sWt.
+template <int AX, int NS, int NO, int PAR>
 __device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, int xoff, const double* __restrict__ raw,
                                        double* __restrict__ T, const double (*sWt)[PT], int tid) {
   constexpr int PA = Geo<AX>::PA;
@@ -139,29 +114,43 @@ __device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, int xoff,
 #pragma unroll
     for (int c = 0; c < PT; ++c) L[c] = raw[s * FOOTMAX + raw_idx<AX>(ia, ib, c) + (AX == 0 ? xoff : 0)];
     double v[4];
+    if (PAR == 0) {         // first thin cell even: (j, parity) = (2,0), (2,1), (3,0)
+      v[0] = ip5<0>(L); v[1] = ip5<1>(L); v[2] = ip5<0>(L + 1); v[3] = 0.0;
+    } else if (PAR == 1) {  // odd: (2,1), (3,0), (3,1)
+      v[0] = ip5<1>(L); v[1] = ip5<0>(L + 1); v[2] = ip5<1>(L + 1); v[3] = 0.0;
+    } else {
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      double r = 0.0;
-      if (k < nt) {
+      for (int k = 0; k < 4; ++k) {
+        double r = 0.0;
+        if (k < nt) {
 #pragma unroll
-        for (int c = 0; c < PT; ++c) r = fma(sWt[k][c], L[c], r);
+          for (int c = 0; c < PT; ++c) r = fma(sWt[k][c], L[c], r);
+        }
+        v[k] = r;
       }
-      v[k] = r;
     }
 #pragma unroll
     for (int o = 0; o < NO; ++o) {
       const double cf = pr.coef[o][s];
       if (cf != 0.0) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) acc[o][k] = fma(cf, v[k], acc[o][k]);
+        for (int k = 0; k < (PAR >= 0 ? 3 : 4); ++k) acc[o][k] = fma(cf, v[k], acc[o][k]);
       }
     }
   }
 #pragma unroll
   for (int o = 0; o < NO; ++o)
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (k < nt) T[((o * nt + k) * PB + ib) * PAMAX + ia] = acc[o][k];
+    for (int k = 0; k < (PAR >= 0 ? 3 : 4); ++k)
+      if (k < nt) T[((o * (PAR >= 0 ? 3 : nt) + k) * PB + ib) * PAMAX + ia] = acc[o][k];
+}
+template <int AX, int NS, int NO>
+__device__ __forceinline__ void phase1_par(int par, const GhostProblem& pr, int nt, int xoff,
+                                           const double* __restrict__ raw, double* __restrict__ T,
+                                           const double (*sWt)[PT], int tid) {
+  if (par == 0) phase1<AX, NS, NO, 0>(pr, nt, xoff, raw, T, sWt, tid);
+  else if (par == 1) phase1<AX, NS, NO, 1>(pr, nt, xoff, raw, T, sWt, tid);
+  else phase1<AX, NS, NO, -1>(pr, nt, xoff, raw, T, sWt, tid);
 }
 
 // ---- phase 2: interpolation along B, register-blocked ------------------------------------------------
@@ -186,76 +175,94 @@ __device__ __forceinline__ void phase2(int nplanes, const double* __restrict__ T
 }
 
 // ---- phase 3: interpolation along A and the store ----------------------------------------------------
+// Everything that can be a compile-time constant is one (NT = thin cells, 0 = runtime; NO = planes' output
+// count; FULL = the tile has no ragged edge), so a plane costs 5 shared loads, 10 FMA and one store.
 // z- and y-slabs (A = x): thread (a-pair ja, fb) walks the planes; the two children are one 16-byte store.
-template <int AX>
-__device__ __forceinline__ void phase3(const GhostArgs& a, const GhostProblem& pr, int NO, const GhostTile& t,
-                                       const TileGeo& g, int f, const double* __restrict__ U, int tid) {
+template <int AX, int NT, int NO, bool FULL>
+__device__ __forceinline__ void phase3(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
+                                       const double* __restrict__ U, int tid) {
   static_assert(AX != 0, "x-slabs have their own phase 3");
   const BoxView& ch = a.child;
   const int ja = tid % 16, fb = tid / 16, fa = 2 * ja;
-  const bool v0 = fa >= g.vA0 && fa < g.vA1, v1 = fa + 1 >= g.vA0 && fa + 1 < g.vA1;
-  if (fb < g.vB0 || fb >= g.vB1 || !(v0 || v1)) return;
-  const int nt = g.nt;
+  bool v0 = true, v1 = true;
+  if (!FULL) {
+    v0 = fa >= t.vA0 && fa < t.vA1;
+    v1 = fa + 1 >= t.vA0 && fa + 1 < t.vA1;
+    if (fb < t.vB0 || fb >= t.vB1 || !(v0 || v1)) return;
+  }
+  const int nt = NT ? NT : t.nt;
   const double* __restrict__ up = U + fb * PAMAX + ja + 2;
-  const int cA = g.oA + fa, cB = g.oB + fb;
-  const long long cell = AX == 2 ? cell_offset(ch, cA, cB, t.lo[2]) : cell_offset(ch, cA, t.lo[1], cB);
   const long long csT = AX == 1 ? ch.px : ch.plane;
+  const long long cell = t.cell0 + fa + (long long)fb * (AX == 1 ? ch.plane : ch.px);
+#pragma unroll
   for (int o = 0; o < NO; ++o) {
-    if (o >= pr.nout) break;
-    double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + cell;
-    double lo[4], hi[4];
+    if (o < pr.nout) {
+      double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + cell;
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (k < nt) children(up + (o * nt + k) * (TB * PAMAX), lo[k], hi[k]);
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (k < nt) {
-        if (v0 && v1) *reinterpret_cast<double2*>(d + k * csT) = make_double2(lo[k], hi[k]);
-        else if (v0) d[k * csT] = lo[k];
-        else d[k * csT + 1] = hi[k];
-      }
+      for (int k = 0; k < (NT ? NT : 4); ++k)
+        if (k < nt) {
+          double lo, hi;
+          children(up + (o * nt + k) * (TB * PAMAX), lo, hi);
+          if (FULL || (v0 && v1)) *reinterpret_cast<double2*>(d + k * csT) = make_double2(lo, hi);
+          else if (v0) d[k * csT] = lo;
+          else d[k * csT + 1] = hi;
+        }
+    }
   }
 }
 
 // x-slabs (thin = x, A = y): thread (fine row fa, fb) owns the g ghosts of one row and writes them as ONE
 // whole 32-byte sector when it can: with g = 3 the low ghosts sit at row positions 1..3 (position 0 is an
 // unused pad double), the high ghosts at XOFF+n .. XOFF+n+2 followed by a pad double when XOFF+n is a
-// multiple of 4 — no sector is written partially.
-__device__ __forceinline__ void phase3x(const GhostArgs& a, const GhostProblem& pr, int NO, const GhostTile& t,
-                                        const TileGeo& g, int f, const double* __restrict__ U, int tid) {
+// multiple of 4 — no sector is written partially (t.sector, decided on the host).
+template <int NT, int NO>
+__device__ __forceinline__ void phase3x(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
+                                        const double* __restrict__ U, int tid) {
   const BoxView& ch = a.child;
   const int fa = tid % 16, fb = tid / 16;
-  if (fb < g.vB0 || fb >= g.vB1 || fa < g.vA0 || fa >= g.vA1) return;
-  const int nt = g.nt;
+  if (fb < t.vB0 || fb >= t.vB1 || fa < t.vA0 || fa >= t.vA1) return;
+  const int nt = NT ? NT : t.nt;
   const double* __restrict__ up = U + fb * PAMAX + (fa >> 1) + 2;
   const bool odd = fa & 1;
-  const long long cell = cell_offset(ch, t.lo[0], g.oA + fa, g.oB + fb);
-  const bool lowside = t.lo[0] < 0;
-  const bool sector = ch.g == 3 && nt == 3 && (lowside || ((XOFF + ch.n[0]) & 3) == 0);
-  for (int o = 0; o < NO; ++o) {
-    if (o >= pr.nout) break;
-    double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + cell;
-    double v[4];
+  const long long cell = t.cell0 + (long long)fa * ch.px + (long long)fb * ch.plane;
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (k < nt) {
-        double lo, hi;
-        children(up + (o * nt + k) * (TB * PAMAX), lo, hi);
-        v[k] = odd ? hi : lo;
-      }
-    if (sector) {
-      if (lowside) {
+  for (int o = 0; o < NO; ++o) {
+    if (o < pr.nout) {
+      double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + cell;
+      double v[4];
+#pragma unroll
+      for (int k = 0; k < (NT ? NT : 4); ++k)
+        if (k < nt) {
+          double lo, hi;
+          children(up + (o * nt + k) * (TB * PAMAX), lo, hi);
+          v[k] = odd ? hi : lo;
+        }
+      if (NT == 3 && t.sector == 1) {
         *reinterpret_cast<double2*>(d - 1) = make_double2(0.0, v[0]);
         *reinterpret_cast<double2*>(d + 1) = make_double2(v[1], v[2]);
-      } else {
+      } else if (NT == 3 && t.sector == 2) {
         *reinterpret_cast<double2*>(d) = make_double2(v[0], v[1]);
         *reinterpret_cast<double2*>(d + 2) = make_double2(v[2], 0.0);
-      }
-    } else {
+      } else {
 #pragma unroll
-      for (int k = 0; k < 4; ++k)
-        if (k < nt) d[k] = v[k];
+        for (int k = 0; k < (NT ? NT : 4); ++k)
+          if (k < nt) d[k] = v[k];
+      }
     }
+  }
+}
+
+template <int NT, int NO>
+__device__ __forceinline__ void phase3_any(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
+                                           const double* __restrict__ U, int tid) {
+  const bool full = t.vA0 == 0 && t.vB0 == 0 && t.vB1 == TB && t.vA1 == (t.axis == 0 ? Geo<0>::TA : Geo<2>::TA);
+  if (t.axis == 0) phase3x<NT, NO>(a, pr, t, f, U, tid);
+  else if (t.axis == 1) {
+    if (full) phase3<1, NT, NO, true>(a, pr, t, f, U, tid);
+    else phase3<1, NT, NO, false>(a, pr, t, f, U, tid);
+  } else {
+    if (full) phase3<2, NT, NO, true>(a, pr, t, f, U, tid);
+    else phase3<2, NT, NO, false>(a, pr, t, f, U, tid);
   }
 }
 
@@ -267,8 +274,9 @@ __global__ void __launch_bounds__(NTHR, 2)
     ghost_fill_tma(const __grid_constant__ CUtensorMap mapx, const __grid_constant__ CUtensorMap mapy,
                    const __grid_constant__ CUtensorMap mapz, const __grid_constant__ GhostArgs a) {
   extern __shared__ unsigned char gsm_raw[];
-  __shared__ double sWt[4][PT];  // thin-axis weights: fine thin cell k <- footprint cell c
+  __shared__ double sWt[4][PT];  // thin-axis weights (ghost widths other than 3): thin cell k <- footprint cell c
   __shared__ __align__(8) unsigned long long sbar;
+  __shared__ __align__(16) GhostTile sTile[2];  // tile descriptors of the current and the next item
   const uint32_t s0 = (smem_u32g(gsm_raw) + 127u) & ~127u;
   double* const raw = reinterpret_cast<double*>(gsm_raw + (s0 - smem_u32g(gsm_raw)));
   const int maxplanes = GF_MAX_OUT * a.child.g;
@@ -279,77 +287,88 @@ __global__ void __launch_bounds__(NTHR, 2)
   const int per_prob = a.ntiles * a.F;
   const int nitems = a.nprob * per_prob;
 
-  // one thread: arm the barrier and request the source footprints of an item
-  auto issue = [&](int item) {
-    const int p = item / per_prob, rem = item - p * per_prob;
-    const int f = rem / a.ntiles, ti = rem - f * a.ntiles;
-    const GhostTile t = a.tiles[ti];
-    const TileGeo g = tile_geo(a.child, a.parent, t);
+  auto tile_index = [&](int item) { return (item % per_prob) % a.ntiles; };
+  // one thread: arm the barrier and request the source footprints of an item (descriptor already on chip)
+  auto issue = [&](int item, const GhostTile& t) {
+    const int p = item / per_prob, f = (item - p * per_prob) / a.ntiles;
     const GhostProblem& pr = a.prob[p];
-    const CUtensorMap* map = g.axT == 0 ? &mapx : (g.axT == 1 ? &mapy : &mapz);
-    const int foot = g.axT == 0 ? Geo<0>::FOOT : FOOTMAX;
+    const CUtensorMap* map = t.axis == 0 ? &mapx : (t.axis == 1 ? &mapy : &mapz);
+    const int foot = t.axis == 0 ? Geo<0>::FOOT : FOOTMAX;
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(pr.nsrc * foot * 8)
                  : "memory");
-    const int cx = g.axT == 0 ? (XOFF + g.q[0]) & ~1 : XOFF + g.q[0];  // x-slabs: even start (XOFF is even)
     for (int s = 0; s < pr.nsrc; ++s)
       asm volatile(
           "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, "
           "%4, %5}], [%6];" ::"r"(s0 + s * FOOTMAX * 8),
-          "l"(map), "r"(cx), "r"(a.parent.g + g.q[1]), "r"(a.parent.g + g.q[2]), "r"(pr.src_arr[s] + f),
-          "r"(bar)
+          "l"(map), "r"(t.cx), "r"(t.cy), "r"(t.cz), "r"(pr.src_arr[s] + f), "r"(bar)
           : "memory");
   };
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    if ((int)blockIdx.x < nitems) issue(blockIdx.x);
+    if ((int)blockIdx.x < nitems) {
+      sTile[0] = a.tiles[tile_index(blockIdx.x)];
+      issue(blockIdx.x, sTile[0]);
+    }
   }
   __syncthreads();
 
   int it = 0;
   for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
-    const int p = item / per_prob, rem = item - p * per_prob;
-    const int f = rem / a.ntiles, ti = rem - f * a.ntiles;
-    const GhostTile t = a.tiles[ti];
-    const TileGeo g = tile_geo(a.child, a.parent, t);
+    const int p = item / per_prob, f = (item - p * per_prob) / a.ntiles;
+    const GhostTile t = sTile[it & 1];
+    const bool more = item + (int)gridDim.x < nitems;
+    // next descriptor -> the other slot, asynchronously: no global load sits on any warp's path into a barrier
+    if (tid >= 32 && tid < 36 && more) {
+      const char* src = reinterpret_cast<const char*>(a.tiles + tile_index(item + gridDim.x)) + 16 * (tid - 32);
+      const uint32_t dst = smem_u32g(&sTile[(it + 1) & 1]) + 16 * (tid - 32);
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+    }
     const GhostProblem& pr = a.prob[p];
     const bool small = pr.nsrc <= 2 && pr.nout <= 2;
-    if (tid < 4 * PT) {
-      const int kt = tid / PT, c = tid % PT;
-      double w = 0.0;
-      if (kt < g.nt) {
-        const int Ig = g.IT0 + kt;
-        const int d = c - ((Ig >> 1) - g.PT0 - 2);  // offset from the first stencil cell of thin cell kt
-        if (d >= 0 && d < 5) w = wprol(Ig & 1, d);
+    if (t.par < 0) {  // ghost width != 3: weight table (CTA-uniform branch)
+      if (tid < 4 * PT) {
+        const int kt = tid / PT, c = tid % PT;
+        double w = 0.0;
+        if (kt < t.nt) {
+          const int Ig = t.IT0 + kt;
+          const int d = c - ((Ig >> 1) - (t.IT0 >> 1));  // offset from the first stencil cell of thin cell kt
+          if (d >= 0 && d < 5) w = wprol(Ig & 1, d);
+        }
+        sWt[kt][c] = w;
       }
-      sWt[kt][c] = w;
+      __syncthreads();
     }
-    __syncthreads();
     mbar_wait_g(bar, it & 1);
     // phase 1 (the footprints have landed)
-    const int xoff = g.q[0] & 1;  // x-slabs: footprint cell 0 sits at this offset of the loaded row
     if (small) {
-      if (g.axT == 2) phase1<2, 2, 2>(pr, g.nt, 0, raw, T, sWt, tid);
-      else if (g.axT == 1) phase1<1, 2, 2>(pr, g.nt, 0, raw, T, sWt, tid);
-      else phase1<0, 2, 2>(pr, g.nt, xoff, raw, T, sWt, tid);
+      if (t.axis == 2) phase1_par<2, 2, 2>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
+      else if (t.axis == 1) phase1_par<1, 2, 2>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
+      else phase1_par<0, 2, 2>(t.par, pr, t.nt, t.xoff, raw, T, sWt, tid);
     } else {
-      if (g.axT == 2) phase1<2, GF_MAX_SRC, GF_MAX_OUT>(pr, g.nt, 0, raw, T, sWt, tid);
-      else if (g.axT == 1) phase1<1, GF_MAX_SRC, GF_MAX_OUT>(pr, g.nt, 0, raw, T, sWt, tid);
-      else phase1<0, GF_MAX_SRC, GF_MAX_OUT>(pr, g.nt, xoff, raw, T, sWt, tid);
+      if (t.axis == 2) phase1_par<2, GF_MAX_SRC, GF_MAX_OUT>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
+      else if (t.axis == 1) phase1_par<1, GF_MAX_SRC, GF_MAX_OUT>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
+      else phase1_par<0, GF_MAX_SRC, GF_MAX_OUT>(t.par, pr, t.nt, t.xoff, raw, T, sWt, tid);
     }
-    __syncthreads();  // raw is free again, T is complete
-    if (tid == 0 && item + (int)gridDim.x < nitems) {
+    if (tid >= 32 && tid < 36) asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();  // raw is free again, T is complete, the next descriptor is in sTile
+    if (tid == 0 && more) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      issue(item + gridDim.x);
+      issue(item + gridDim.x, sTile[(it + 1) & 1]);
     }
-    const int NO = small ? 2 : GF_MAX_OUT;  // planes are laid out for NO outputs (unused ones hold zeros)
-    if (g.axT == 0) phase2<0>(NO * g.nt, T, U, tid);
-    else phase2<2>(NO * g.nt, T, U, tid);
+    // planes are laid out for NO = 2 or 4 outputs (unused ones hold zeros)
+    const int nplanes = (small ? 2 : GF_MAX_OUT) * t.nt;
+    if (t.axis == 0) phase2<0>(nplanes, T, U, tid);
+    else phase2<2>(nplanes, T, U, tid);
     __syncthreads();
-    if (g.axT == 0) phase3x(a, pr, NO, t, g, f, U, tid);
-    else if (g.axT == 1) phase3<1>(a, pr, NO, t, g, f, U, tid);
-    else phase3<2>(a, pr, NO, t, g, f, U, tid);
+    if (t.nt == 3) {
+      if (small) phase3_any<3, 2>(a, pr, t, f, U, tid);
+      else phase3_any<3, GF_MAX_OUT>(a, pr, t, f, U, tid);
+    } else {
+      if (small) phase3_any<0, 2>(a, pr, t, f, U, tid);
+      else phase3_any<0, GF_MAX_OUT>(a, pr, t, f, U, tid);
+    }
   }
 }
 
@@ -369,14 +388,49 @@ void cut(int r0, int r1, int T, int base, int align, std::vector<Piece>& out) {
 }
 }  // namespace
 
+namespace {
+// Descriptor of the piece [lo, lo + n) of the tile-grid cell at `org` (box-local fine indices) of a slab with
+// thin axis axT. Index maps: fine cell I (level-global) has parent I >> 1 (S1); the footprint starts 2 parent
+// cells before the first covered parent cell along every axis.
+GhostTile make_tile(const BoxView& ch, const BoxView& pa, int axT, const int lo[3], const int n[3], const int org[3]) {
+  const int axA = axT == 0 ? 1 : 0, axB = axT == 2 ? 1 : 2;  // (A, B, T) = (x,y,z) | (x,z,y) | (y,z,x)
+  GhostTile t{};
+  t.axis = axT;
+  t.nt = n[axT];
+  t.IT0 = ch.lo[axT] + lo[axT];
+  t.par = t.nt == 3 ? (t.IT0 & 1) : -1;
+  t.vA0 = lo[axA] - org[axA]; t.vA1 = t.vA0 + n[axA];
+  t.vB0 = lo[axB] - org[axB]; t.vB1 = t.vB0 + n[axB];
+  int q[3];  // parent-local index of footprint cell 0
+  q[axA] = ((ch.lo[axA] + org[axA]) >> 1) - 2 - pa.lo[axA];
+  q[axB] = ((ch.lo[axB] + org[axB]) >> 1) - 2 - pa.lo[axB];
+  q[axT] = (t.IT0 >> 1) - 2 - pa.lo[axT];
+  t.cx = XOFF + q[0];
+  t.xoff = 0;
+  if (axT == 0) { t.xoff = t.cx & 1; t.cx &= ~1; }  // x-slabs: 8-wide rows from an even start
+  t.cy = pa.g + q[1];
+  t.cz = pa.g + q[2];
+  const bool lowside = lo[0] < 0;
+  t.sector = (axT == 0 && ch.g == 3 && t.nt == 3) ? (lowside ? 1 : (((XOFF + ch.n[0]) & 3) == 0 ? 2 : 0)) : 0;
+  int c0[3];
+  c0[axT] = lo[axT]; c0[axA] = org[axA]; c0[axB] = org[axB];
+  t.cell0 = cell_offset(ch, c0[0], c0[1], c0[2]);
+  return t;
+}
+}  // namespace
+
 // Tile origins are even in y and z (so a tile covers whole parent cells) and a multiple of 4 in x in
 // LEVEL-GLOBAL index: the parent footprint of an x-extended tile then starts at an even parent x index,
-// i.e. on a 16-byte boundary (XOFF and lo are even) — TMA loads of 160-byte box rows from an odd fp64
-// coordinate fault on sm_100a ("illegal instruction", measured; 48-byte rows do not).
-void build_ghost_tiles(const BoxView& ch, std::vector<GhostTile>& tiles) {
+// i.e. on a 16-byte boundary (XOFF and lo are even) — a TMA tiled load whose innermost fp64 coordinate is
+// odd faults on sm_100a ("illegal instruction", measured).
+void build_ghost_tiles(const BoxView& ch, const BoxView& pa, std::vector<GhostTile>& tiles) {
   tiles.clear();
   const int g = ch.g;
   std::vector<Piece> as, bs;
+  auto push = [&](int ax, int l0, int l1, int l2, int n0, int n1, int n2, int o0, int o1, int o2) {
+    const int lo[3] = {l0, l1, l2}, n[3] = {n0, n1, n2}, org[3] = {o0, o1, o2};
+    tiles.push_back(make_tile(ch, pa, ax, lo, n, org));
+  };
   // z-slabs: A = x over the padded extent, B = y over the padded extent
   cut(-g, ch.n[0] + g, Geo<2>::TA, ch.lo[0], 4, as);
   cut(-g, ch.n[1] + g, TB, ch.lo[1], 2, bs);
@@ -384,7 +438,7 @@ void build_ghost_tiles(const BoxView& ch, std::vector<GhostTile>& tiles) {
     for (auto& b : bs)
       for (auto& x : as) {
         const int z = hi ? ch.n[2] : -g;
-        tiles.push_back(GhostTile{{x.lo, b.lo, z}, {x.n, b.n, g}, {x.org, b.org, z}, 2});
+        push(2, x.lo, b.lo, z, x.n, b.n, g, x.org, b.org, z);
       }
   // y-slabs: A = x padded, B = z interior
   cut(0, ch.n[2], TB, ch.lo[2], 2, bs);
@@ -392,7 +446,7 @@ void build_ghost_tiles(const BoxView& ch, std::vector<GhostTile>& tiles) {
     for (auto& b : bs)
       for (auto& x : as) {
         const int y = hi ? ch.n[1] : -g;
-        tiles.push_back(GhostTile{{x.lo, y, b.lo}, {x.n, g, b.n}, {x.org, y, b.org}, 1});
+        push(1, x.lo, y, b.lo, x.n, g, b.n, x.org, y, b.org);
       }
   // x-slabs: A = y interior, B = z interior
   cut(0, ch.n[1], Geo<0>::TA, ch.lo[1], 2, as);
@@ -400,15 +454,8 @@ void build_ghost_tiles(const BoxView& ch, std::vector<GhostTile>& tiles) {
     for (auto& b : bs)
       for (auto& y : as) {
         const int x = hi ? ch.n[0] : -g;
-        tiles.push_back(GhostTile{{x, y.lo, b.lo}, {g, y.n, b.n}, {x, y.org, b.org}, 0});
+        push(0, x, y.lo, b.lo, g, y.n, b.n, x, y.org, b.org);
       }
-  if (const char* e = getenv("SC_DBG_TILE")) {  // DEBUG
-    int lo = 0, hi = 1 << 30;
-    sscanf(e, "%d:%d", &lo, &hi);
-    std::vector<GhostTile> keep;
-    for (int i = 0; i < (int)tiles.size(); ++i) if (i >= lo && i < hi) keep.push_back(tiles[i]);
-    tiles = keep;
-  }
 }
 
 void ghost_box_dims(int axis, unsigned box[4]) {

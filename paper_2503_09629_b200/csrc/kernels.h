@@ -62,12 +62,19 @@ bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, vo
 // ------------------------------------------------------------------------------------------------
 constexpr int GF_MAX_SRC = 5, GF_MAX_OUT = 4, GF_MAX_PROB = 2;
 
-struct GhostTile {   // a piece of one ghost slab, box-local fine indices
-  int lo[3];
-  int n[3];
-  int org[3];        // origin of the tile grid cell this piece lies in (even; lo - org < tile size)
-  int axis;          // the slab's thin axis: 0 = x-slab, 1 = y-slab, 2 = z-slab
+struct GhostTile {   // one work tile of a ghost slab; everything the kernel needs is precomputed on the host
+  int axis;                // the slab's thin axis: 0 = x-slab, 1 = y-slab, 2 = z-slab
+  int nt;                  // thin cells (= ghost width)
+  int par;                 // ghost width 3: parity of the first thin cell's level-global index; else -1
+  int vA0, vA1, vB0, vB1;  // valid tile-local fine range along the transverse axes A (more contiguous), B
+  int cx, cy, cz;          // start of the parent footprint in the parent's tensor map (cx even)
+  int xoff;                // x-slabs: position of footprint cell 0 inside the loaded 8-wide row
+  int sector;              // x-slabs: 0 = scalar stores, 1 / 2 = whole-sector stores on the low / high side
+  int IT0;                 // level-global index of the first thin cell (weight table for widths != 3)
+  int pad;
+  long long cell0;         // offset inside a child array of tile-local (a = 0, b = 0, thin cell 0)
 };
+static_assert(sizeof(GhostTile) == 64, "the kernel fetches descriptors as four 16-byte copies");
 
 struct GhostProblem {
   int nsrc, nout;
@@ -88,7 +95,7 @@ struct GhostArgs {
   const void* tmaps;          // host pointer to the parent's three footprint CUtensorMaps (thin axis x, y, z;
                               // 128 bytes each, contiguous), or null -> direct-load kernel
 };
-void build_ghost_tiles(const BoxView& child, std::vector<GhostTile>& tiles);
+void build_ghost_tiles(const BoxView& child, const BoxView& parent, std::vector<GhostTile>& tiles);
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st);
 
 // a4: periodic ghost fill of `narrays` consecutive arrays of the level-0 box (reading S9).
