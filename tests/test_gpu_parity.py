@@ -208,3 +208,29 @@ def test_error_paths_on_device():
         G.sc_debug_ghost_map(0, 0)
     G.sc_step(w.dt_coarse)  # still usable afterwards
     G.close()
+
+
+@pytest.mark.parametrize("g", [2, 3, 4])
+def test_ghost_fill_geometry_sweep(g):
+    """Child boxes at every offset class (lo mod 4 per axis decides tile origins, footprint parity and the
+    alignment of every TMA coordinate), sizes that are not multiples of any tile, inside parents whose padded
+    extent the last footprints overrun: one subcycled + one uniform step each, every ghost and interior value."""
+    B = wl.Box
+    cases = [
+        ((40, 24, 28), (10, 8, 12), (32, 32, 26)),   # odd parent x index of the first footprint cell
+        ((64, 64, 64), (22, 20, 20), (44, 28, 26)),
+        ((64, 64, 64), (20, 22, 26), (30, 46, 18)),
+        ((48, 40, 36), (8, 8, 8), (66, 50, 42)),     # child reaches the nesting margin on the high sides
+        ((36, 36, 36), (14, 18, 10), (20, 14, 34)),
+        ((32, 32, 32), (8, 8, 8), (48, 48, 48)),
+    ]
+    for dom, lo, n in cases:
+        w = wl.Workload(f"sweep {dom} {lo} {n} g={g}", [B(0, (0, 0, 0), dom), B(1, lo, n)], dom, ghost=g,
+                        init=wl.multi_gaussian_init(3))
+        G, O = _pair(w)
+        for sub in (True, False):
+            G.sc_step(w.dt_coarse, sub)
+            O.step(w.dt_coarse, sub)
+            _compare_state(G, O, w, what=w.name + f" sub={sub}")
+        assert np.array_equal(G.sc_debug_ghost_map(1, 0), O.ghost_map(1, 0))
+        G.close()
