@@ -1,13 +1,16 @@
 // dispatch.cu — picks the kernel set: the tuned sm_100a kernels (default: stage_tma.cu, ghost_tma.cu,
 // restrict_zmarch.cu) or the straightforward direct-load kernels of kernels_basic.cu (environment
 // SC_KERNELS=ref; A/B checks and debugging only). Both are CUDA; there is no CPU path.
+#include <cstdlib>
+
 #include "kernels.h"
 
 namespace sc {
 
 void launch_stage_direct(const StageArgs& a, cudaStream_t st);
 int launch_stage_tma(const StageArgs& a, cudaStream_t st);
-bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned box[4], void* out_map128);
+bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned box[4], int l2_promotion,
+                             void* out_map128);
 void stage_box_dims(unsigned box[4]);
 void restrict_box_dims(unsigned box[4]);
 void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
@@ -38,7 +41,9 @@ bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, vo
   if (kind == 0) stage_box_dims(box);
   else if (kind == 1) restrict_box_dims(box);
   else ghost_box_dims(kind - 2, box);
-  return make_box_tensor_map_tma(b, narrays, base, box, out_map128);
+  // streaming tiles (stage, restriction) promote misses to 256-byte fetches; the ghost fill's footprint rows are
+  // 64-160 bytes and isolated: promotion there only multiplies the DRAM traffic
+  return make_box_tensor_map_tma(b, narrays, base, box, kind <= 1 ? 256 : 0, out_map128);
 }
 
 }  // namespace sc

@@ -492,7 +492,8 @@ void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st) {
   }
   const long long nitems = (long long)a.nprob * a.ntiles * a.F;
   const int per_sm = smem <= 112 * 1024 ? 2 : 1;
-  const unsigned grid = (unsigned)(nitems < (long long)nsm * per_sm ? nitems : (long long)nsm * per_sm);
+  const long long want = (long long)nsm * per_sm;
+  const unsigned grid = (unsigned)(nitems < want ? nitems : want);
   const CUtensorMap* m = static_cast<const CUtensorMap*>(a.tmaps);
   ghost_fill_tma<<<grid, NTHR, smem, st>>>(m[0], m[1], m[2], a);
 }
