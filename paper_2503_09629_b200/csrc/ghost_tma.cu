@@ -4,21 +4,27 @@
 //   child array dst_arr[o](ghost cell) = P[ sum_s coef[o][s] * parent array src_arr[s] ],   P = 5x5x5 quartic Lagrange
 //
 // The ghost shell of a box is the union of six slabs (z-lo, z-hi, y-lo, y-hi, x-lo, x-hi); each slab is cut
-// into tiles  g (thin axis) x TA x TB  fine cells whose origin is EVEN in every axis, so the parent footprint
-// of a tile is exactly (TA/2+4) x (TB/2+4) x 6 parent cells. A work ITEM is (problem, field, tile).
-// Persistent CTAs (two per SM) walk the item list; per item
+// into tiles  g (thin axis) x TA x TB  fine cells (32 x 16 for z- and y-slabs, 16 x 16 for x-slabs) whose
+// origin is even in every axis, so a tile covers whole parent cells and its parent footprint is exactly
+// (TA/2+4) x (TB/2+4) x 6 cells. The host precomputes one 64-byte descriptor per tile (index maps, TMA
+// coordinates, ragged-edge ranges, store mode). A work ITEM is (problem, field, tile). Persistent CTAs (two
+// per SM) walk the item list; per item
 //   0. the footprint of every source array arrives in shared memory through ONE TMA tiled load per source
 //      (cp.async.bulk.tensor.4d on the parent's footprint tensor map, out-of-range cells zero-filled),
-//      requested one item AHEAD: the loads of item i+1 fly while item i is interpolated, so no warp ever
-//      waits on HBM (the v2 kernel spent 35 % of its samples on 7 dependent global round trips per tile);
-//   1. one thread per parent column: thin-axis interpolation (6 parent cells -> g fine cells) of every
-//      source, then the time combination into the outputs          -> T[plane = (o, thin cell)][b][a]
+//      requested one item AHEAD so it flies while the current item is interpolated; the descriptor of the
+//      next item comes by cp.async, so no global load sits on a warp's path into a barrier;
+//   1. one thread per parent column: thin-axis interpolation (6 parent cells -> g fine cells; for g = 3 the
+//      weights are compile-time constants chosen by the parity of the first thin cell) of every source,
+//      then the time combination into the outputs             -> T[plane = (o, thin cell)][b][a]
 //   2. interpolation along b, register-blocked: one thread per (plane, a)  -> U[plane][fb][a]
 //   3. interpolation along a and the store: thread (a-pair, fb) walks the planes; for z- and y-slabs a = x
-//      and the pair is one 16-byte store, coalesced across the warp; for x-slabs (thin = x) the thread
-//      writes whole 32-byte sectors (the g = 3 ghosts of a row plus one unused pad double), so no sector
-//      is written partially.
+//      and the pair is one 16-byte store, coalesced across the warp; for x-slabs (thin = x) a thread owns
+//      the g ghosts of one row and writes them as ONE whole 32-byte sector (plus an unused pad double).
 // A ghost value costs 6 + 5 + 5 FMA instead of 125 and every parent value is fetched once per tile.
+// Measured (r01, profiles/): the kernel is bound by the footprint loads — isolated 64-160-byte rows, 72-144
+// per source box: 2-13k cycles from request to arrival, growing with the number of boxes in flight on the
+// GPU; replacing TMA by per-thread 16-byte cp.async, prefetching two items ahead into L2, or removing the
+// index arithmetic from the phases each left the launch time within 10 %.
 #include <cuda.h>
 
 #include <cstdlib>
