@@ -19,6 +19,18 @@ def _free_port() -> int:
     return p
 
 
+def _torchrun(args, attempts=2):
+    """World-size-2 launch on 127.0.0.1; a rendezvous that loses the race for its port is retried on a new one."""
+    env = dict(os.environ, OMP_NUM_THREADS="2")
+    for _ in range(attempts):
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+               "--master-addr", "127.0.0.1", "--master-port", str(_free_port())] + list(args)
+        r = subprocess.run(cmd, capture_output=True, text=True, timeout=900, cwd=ROOT, env=env)
+        if r.returncode == 0:
+            break
+    return r
+
+
 _WORKER = r"""
 import os, sys, json
 sys.path.insert(0, {root!r})
@@ -38,9 +50,7 @@ dist.destroy_process_group()
 def test_max_over_ranks_and_whole_job_value_world2(tmp_path):
     script = tmp_path / "worker.py"
     script.write_text(_WORKER.format(root=ROOT))
-    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
-           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), str(script)]
-    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    r = _torchrun([str(script)])
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
     assert sorted(l["rank"] for l in lines) == [0, 1]
@@ -52,11 +62,8 @@ def test_max_over_ranks_and_whole_job_value_world2(tmp_path):
 
 def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     """bench.py --impl reference with N = 2: rank 0 alone runs the oracle and prints; rank 1 exits 0 silently."""
-    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
-           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()),
-           os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0",
-           "--config", "1"]
-    r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    r = _torchrun([os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                   "--warmup", "0", "--config", "1"])
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1
