@@ -46,6 +46,7 @@ struct sc_hierarchy {
   bool own_stream = false;
   double* staging = nullptr;      // device, largest padded dense box
   size_t staging_bytes = 0;
+  std::vector<double> coupling_host;  // F*F, host copy of the coupling matrix
   std::vector<int> cur;           // per level: state slot (0 or 1) that holds the current state y
   bool l0_ghosts_valid = false;   // level 0: ghosts of y hold the periodic copies (no set_state since)
   double time = 0.0;
@@ -201,6 +202,7 @@ void stage_level(Seq& q, int level, int mode, double dt) {
       a.inv12dx2[d] = 1.0 / (12.0 * dx * dx);
     }
     a.A = h->coupling();
+    a.A_host = a.A ? h->coupling_host.data() : nullptr;
     a.S = a.A ? h->arr(ib, L.a_scratch()) : nullptr;
     a.tmap = h->tmap_ok[ib] ? h->tmaps[ib].bytes : nullptr;
     prof_begin(h, KIND_STAGE, stage_bytes(a.b, L.F, mode, a.write_Y4r));
@@ -505,6 +507,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   if ((ce = cudaMalloc(&h->staging, smax)) != cudaSuccess) return bail("cudaMalloc(staging)", ce);
   if ((ce = cudaMemsetAsync(h->arena, 0, h->L.arena_bytes, h->stream)) != cudaSuccess) return bail("memset", ce);
   if (h->L.has_coupling) {
+    h->coupling_host.assign(desc->coupling, desc->coupling + (size_t)h->L.F * h->L.F);
     ce = cudaMemcpyAsync(h->arena + h->L.coupling_offset, desc->coupling, sizeof(double) * h->L.F * h->L.F,
                          cudaMemcpyHostToDevice, h->stream);
     if (ce != cudaSuccess) return bail("copy coupling", ce);

@@ -38,6 +38,7 @@ struct StageArgs {
   double dt;
   double inv12dx2[3];  // 1 / (12 dx_a^2)
   const double* A;     // device F*F row-major coupling, or null
+  const double* A_host; // the same matrix in host memory (kernel-parameter copy for couple_matvec)
   double* S;           // coupled systems: 2F scratch arrays for the coupling terms (A W) of the two operands
   // TMA path: tensor map of the box (all arrays as the 4th dimension) and the array indices of the roles
   const void* tmap;    // host pointer to the box's CUtensorMap, or null -> direct-load kernel

@@ -357,19 +357,19 @@ void launch_zmarch(const StageArgs& a, cudaStream_t st) {
 //   STAGE_12:  W1 = u_n,               W2 = u_n + dt/2 rho_n
 //   STAGE_34:  W1 = u_n + dt/2 Y2r,    W2 = u_n + dt Y3r
 // S[f] = sum_q A_fq W1_q,  S[F + f] = sum_q A_fq W2_q, and the z-march kernel adds them at the centre cell.
-// One thread per cell: all F operand pairs in registers (every global load issued up front), A in shared
-// memory (broadcast reads). 2 F^2 FMA per cell against (2|3) F reads + 2 F writes.
+// One thread per cell: all F operand pairs in registers (every global load issued up front), A in the
+// constant bank (kernel parameter). 2 F^2 FMA per cell against (2|3) F reads + 2 F writes.
 namespace {
+template <int FB> struct CoupleMatrix { double a[FB * FB]; };  // row-major, zero-padded to FB x FB
+
+// The matrix travels as a KERNEL PARAMETER (up to 8 KB; parameters may be 32 KB since CUDA 12.1): with both
+// loops unrolled every A_fq is an immediate constant-bank operand of its FMA — no shared-memory traffic at
+// all (the shared-memory version spent one broadcast LDS per FMA pair and ran at 40-53 % of DRAM peak).
 template <int MODE, int FB>
-__global__ void __launch_bounds__(128) couple_matvec(const TmaStageParams p, const double* __restrict__ A) {
-  __shared__ double sA[FB * FB];
+__global__ void __launch_bounds__(128)
+    couple_matvec(const __grid_constant__ TmaStageParams p, const __grid_constant__ CoupleMatrix<FB> A) {
   const BoxView& b = p.b;
   const int F = p.F;
-  for (int e = threadIdx.y * 32 + threadIdx.x; e < FB * FB; e += 128) {
-    const int r = e / FB, c = e % FB;
-    sA[e] = (r < F && c < F) ? A[r * F + c] : 0.0;
-  }
-  __syncthreads();
   const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z;
   if (i >= b.n[0] || j >= b.n[1]) return;
   const long long o = cell_offset(b, i, j, k);
@@ -391,26 +391,36 @@ __global__ void __launch_bounds__(128) couple_matvec(const TmaStageParams p, con
     }
   }
   double* __restrict__ S = const_cast<double*>(p.S);
-  for (int f = 0; f < F; ++f) {
-    double s1 = 0.0, s2 = 0.0;
 #pragma unroll
-    for (int q = 0; q < FB; ++q) {
-      const double aq = sA[f * FB + q];
-      s1 = fma(aq, w1[q], s1);
-      s2 = fma(aq, w2[q], s2);
+  for (int f = 0; f < FB; ++f) {
+    if (f < F) {
+      double s1 = 0.0, s2 = 0.0;
+#pragma unroll
+      for (int q = 0; q < FB; ++q) {
+        s1 = fma(A.a[f * FB + q], w1[q], s1);
+        s2 = fma(A.a[f * FB + q], w2[q], s2);
+      }
+      S[(long long)f * b.vol + o] = s1;
+      S[(long long)(F + f) * b.vol + o] = s2;
     }
-    S[(long long)f * b.vol + o] = s1;
-    S[(long long)(F + f) * b.vol + o] = s2;
   }
 }
 
-template <int MODE>
-void launch_couple_mode(const TmaStageParams& p, const double* A, cudaStream_t st) {
+template <int MODE, int FB>
+void launch_couple_fb(const TmaStageParams& p, const double* A_host, cudaStream_t st) {
+  CoupleMatrix<FB> m;
+  for (int r = 0; r < FB; ++r)
+    for (int c = 0; c < FB; ++c) m.a[r * FB + c] = (r < p.F && c < p.F) ? A_host[r * p.F + c] : 0.0;
   dim3 blk(32, 4, 1), grd((p.b.n[0] + 31) / 32, (p.b.n[1] + 3) / 4, p.b.n[2]);
-  if (p.F <= 8) couple_matvec<MODE, 8><<<grd, blk, 0, st>>>(p, A);
-  else if (p.F <= 16) couple_matvec<MODE, 16><<<grd, blk, 0, st>>>(p, A);
-  else if (p.F <= 24) couple_matvec<MODE, 24><<<grd, blk, 0, st>>>(p, A);
-  else couple_matvec<MODE, 32><<<grd, blk, 0, st>>>(p, A);
+  couple_matvec<MODE, FB><<<grd, blk, 0, st>>>(p, m);
+}
+
+template <int MODE>
+void launch_couple_mode(const TmaStageParams& p, const double* A_host, cudaStream_t st) {
+  if (p.F <= 8) launch_couple_fb<MODE, 8>(p, A_host, st);
+  else if (p.F <= 16) launch_couple_fb<MODE, 16>(p, A_host, st);
+  else if (p.F <= 24) launch_couple_fb<MODE, 24>(p, A_host, st);
+  else launch_couple_fb<MODE, 32>(p, A_host, st);
 }
 
 void launch_couple_matvec(const StageArgs& a, cudaStream_t st) {
@@ -420,8 +430,8 @@ void launch_couple_matvec(const StageArgs& a, cudaStream_t st) {
   p.yn = a.yn; p.Y2r = a.Y2r; p.Y3r = a.Y3r;
   p.dt = a.dt;
   p.S = a.S;
-  if (a.mode == STAGE_12) launch_couple_mode<STAGE_12>(p, a.A, st);
-  else launch_couple_mode<STAGE_34>(p, a.A, st);
+  if (a.mode == STAGE_12) launch_couple_mode<STAGE_12>(p, a.A_host, st);
+  else launch_couple_mode<STAGE_34>(p, a.A_host, st);
 }
 }  // namespace
 
@@ -450,7 +460,7 @@ bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const un
 }
 
 int launch_stage_tma(const StageArgs& a, cudaStream_t st) {
-  if (!a.tmap || (a.A && !a.S)) { launch_stage_direct(a, st); return 1; }
+  if (!a.tmap || (a.A && !(a.S && a.A_host))) { launch_stage_direct(a, st); return 1; }
   if (a.A) {  // coupling terms first (pointwise F x F product over all fields), then the per-field z-march
     launch_couple_matvec(a, st);
     if (a.mode == STAGE_12) launch_zmarch<STAGE_12, true>(a, st);
