@@ -290,7 +290,7 @@ def run_gpu(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of the
 # dominant kernel (profiles/): filled in per round; None until a capture exists.
-TRAFFIC = {}
+TRAFFIC = {"rk_stage": 678.0e6}  # profiles/r01_v3.md: (298+228 + 589+240)/2 MB per 256^3 launch (cfg 5)
 
 
 def main():
