@@ -233,7 +233,7 @@ def run_gpu(args):
     dom = max(kinds, key=lambda k: kinds[k]["ms_total"])
     ksum = sum(k["ms_total"] for k in kinds.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["algorithmic_GBps"], "peak": peak,
-                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom),
+                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom) if args.config == 5 else None,
                 "peak_source": peak_src, "share_of_step": kinds[dom]["ms_total"] / ksum,
                 "bytes_per_launch": kinds[dom]["bytes_per_launch"], "avg_launch_us": kinds[dom]["avg_us"]}
 
