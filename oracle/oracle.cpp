@@ -22,9 +22,12 @@
 // Pins (tests/test_oracle_*.py, run with -m "not gpu"): dense-output invariants and the rational
 // coefficient table; scalar-ODE stage-order test; closed-form single-level amplification matrix;
 // polynomial exactness of prolongation / restriction / Laplacian; brute-force ghost index map;
-// plane-wave convergence ladder (order ~4); subcycled-vs-uniform agreement; linearity.
-// PARITY UNPINNED: bit-level values of the composite multi-level scheme have no closed form — the
-// oracle is the definition there ("Oracle pins").
+// plane-wave convergence ladder (order ~4); subcycled-vs-uniform agreement; linearity; and the COMPOSITE
+// multi-level step (dense-output fills at theta = 0 and 1/2, stage formulas, restrictions, both modes) against
+// the exact solution u = r^2 + 3 t^2, rho = 6 t, which every operator reproduces to rounding
+// (test_composite_scheme_exact_for_quadratic_solution). What stays unpinned at bit level is only the
+// composite step on data the operators do NOT reproduce exactly; there the oracle is the definition and the
+// convergence ladder bounds it.
 
 #include <cmath>
 #include <cstdint>

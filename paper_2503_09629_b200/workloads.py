@@ -194,6 +194,19 @@ def plane_wave_init(w: Workload, level: int, ibox: int, comp: int) -> np.ndarray
     return plane_wave_exact(w, level, ibox, comp, 0.0)
 
 
+def quadratic_exact(w: Workload, level: int, ibox: int, comp: int, t: float, pad: int = 0) -> np.ndarray:
+    """u = x^2 + y^2 + z^2 + 3 t^2, rho = 6 t: an exact solution of the wave equation (u_tt = 6 = Lap u) that
+    every operator of the scheme reproduces exactly (away from the periodic seam of level 0)."""
+    x, y, z = w.centres(level, ibox, pad)
+    if comp < w.nfields:
+        return z[:, None, None] ** 2 + y[None, :, None] ** 2 + x[None, None, :] ** 2 + 3.0 * t * t
+    return np.full((len(z), len(y), len(x)), 6.0 * t)
+
+
+def quadratic_init(w: Workload, level: int, ibox: int, comp: int) -> np.ndarray:
+    return quadratic_exact(w, level, ibox, comp, 0.0)
+
+
 def multi_gaussian_init(ngauss: int = 8):
     """u_f = sum_m a exp(-|x-c|^2/(2 w^2)), a~U(-1,1), c~U(-.5,.5)^3, w~U(.05,.3); rho_f = 0 (S23)."""
     def f(w: Workload, level: int, ibox: int, comp: int) -> np.ndarray:

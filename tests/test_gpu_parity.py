@@ -234,3 +234,24 @@ def test_ghost_fill_geometry_sweep(g):
             _compare_state(G, O, w, what=w.name + f" sub={sub}")
         assert np.array_equal(G.sc_debug_ghost_map(1, 0), O.ghost_map(1, 0))
         G.close()
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_exact_quadratic_solution_without_the_oracle(sub):
+    """The CUDA path against a closed form, no oracle involved: u = x^2+y^2+z^2+3t^2, rho = 6t is reproduced
+    exactly by every operator of the scheme (see tests/test_oracle_scheme.py), so after one coarse step of a
+    3-level hierarchy every level must hold it to rounding away from level 0's periodic seam."""
+    n = 64
+    w = wl.Workload("quadratic", wl.nested_cubes(3, n), (n, n, n), init=wl.quadratic_init)
+    G = sc.Hierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, sub)
+    t = w.dt_coarse
+    for l in (1, 2):
+        for c in (0, 1):
+            got = G.sc_debug_read_padded(l, 0, c)
+            want = wl.quadratic_exact(w, l, 0, c, t, pad=w.ghost)
+            assert np.max(np.abs(got - want)) < 2e-12, (sub, l, c, float(np.max(np.abs(got - want))))
+    m = slice(10, n - 10)
+    for c in (0, 1):
+        assert np.max(np.abs(G.sc_read_level(0, 0, c)[m, m, m] - wl.quadratic_exact(w, 0, 0, c, t)[m, m, m])) < 2e-12
+    G.close()

@@ -321,3 +321,29 @@ def test_convergence_ladder_and_sub_vs_uniform(oracle_mod):
     d64 = max(np.max(np.abs(a - b)) for a, b in zip(u64s, u64u))
     assert d32 < 0.2 * max(e32s) and d64 < 0.3 * max(e64s)
     assert 2.5 < math.log2(d32 / d64) < 3.6  # the difference itself converges at ~3rd order (S12)
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_composite_scheme_exact_for_quadratic_solution(oracle_mod, sub):
+    """Pins the COMPOSITE multi-level scheme to a closed form: u = x^2+y^2+z^2+3t^2, rho = 6t solves the wave
+    equation, the 4th-order Laplacian, the quartic prolongation and the quintic restriction are exact on it,
+    RK4 is exact for solutions quadratic in t, and so are eq (10) and the stage formulas (15)-(18) for a linear
+    autonomous system (d3y/dt3 = f_y d2y/dt2 and 4 (k_3 - k_2) / h_p^2 = f_y d2y/dt2 hold exactly; with the
+    child's h in place of the parent's, S5, the h^3 terms would not cancel). One coarse step of a 3-level
+    hierarchy (2 and 4 subcycled fine steps, theta = 0 and 1/2 fills, both restrictions) must therefore
+    reproduce the polynomial to rounding wherever the periodic seam of level 0 (8 cells per step) has not reached."""
+    n = 64
+    w = wl.Workload("quadratic", wl.nested_cubes(3, n), (n, n, n), init=wl.quadratic_init)
+    H = oracle_mod.OracleHierarchy.from_workload(w)
+    H.step(w.dt_coarse, sub)
+    t = w.dt_coarse
+    for l in (1, 2):
+        for c in (0, 1):
+            got = H.read(l, 0, c, padded=True)
+            want = wl.quadratic_exact(w, l, 0, c, t, pad=w.ghost)
+            assert np.max(np.abs(got - want)) < 2e-12, (sub, l, c, float(np.max(np.abs(got - want))))
+    m = slice(10, n - 10)
+    for c in (0, 1):
+        got = H.read(0, 0, c)[m, m, m]
+        want = wl.quadratic_exact(w, 0, 0, c, t)[m, m, m]
+        assert np.max(np.abs(got - want)) < 2e-12, (sub, 0, c)
