@@ -155,6 +155,7 @@ struct Hier {
   int domain[3] = {0, 0, 0};
   double xlo[3], xhi[3];
   std::vector<double> A;  // F*F coupling or empty
+  double sigma = 0.0;     // Kreiss-Oliger dissipation strength (eqs 35-36); 0 = none
   std::vector<BoxData> boxes;
   std::vector<std::vector<int>> level_boxes;
   double time = 0.0;
@@ -163,6 +164,35 @@ struct Hier {
 
 inline bool is_interior(const BoxData& b, int i, int j, int k) {
   return i >= 0 && i < b.n[0] && j >= 0 && j < b.n[1] && k >= 0 && k < b.n[2];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Kreiss-Oliger dissipation: d_t y -> RHS + Q y for EVERY evolved variable (eq 35),
+//   Q y = (-1)^{r/2} sigma / 2^{r+2} sum_i h_i^{r+1} D_{i+}^{r/2+1} D_{i-}^{r/2+1} y          (eq 36)
+// with r = 4 the order of the finite differences of the RHS (S2): (D+ D-)^3 y = delta^6 y / h^6,
+//   delta^6 y = y[-3] - 6 y[-2] + 15 y[-1] - 20 y[0] + 15 y[+1] - 6 y[+2] + y[+3],
+// so Q y = sigma / 64 sum_i delta_i^6 y / h_i. Uses all 3 ghost layers.
+// ---------------------------------------------------------------------------------------------
+void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vector<Field>& kout) {
+  const int V = 2 * H.F;
+  double c[3];
+  for (int a = 0; a < 3; ++a) c[a] = H.sigma / (64.0 * H.dx(b.level, a));
+  for (int v = 0; v < V; ++v) {
+    const Field& y = Y[v];
+    Field& kv = kout[v];
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < b.n[2]; ++k)
+      for (int j = 0; j < b.n[1]; ++j)
+        for (int i = 0; i < b.n[0]; ++i) {
+          const double d6x = y.at(i - 3, j, k) - 6.0 * y.at(i - 2, j, k) + 15.0 * y.at(i - 1, j, k) - 20.0 * y.at(i, j, k) +
+                             15.0 * y.at(i + 1, j, k) - 6.0 * y.at(i + 2, j, k) + y.at(i + 3, j, k);
+          const double d6y = y.at(i, j - 3, k) - 6.0 * y.at(i, j - 2, k) + 15.0 * y.at(i, j - 1, k) - 20.0 * y.at(i, j, k) +
+                             15.0 * y.at(i, j + 1, k) - 6.0 * y.at(i, j + 2, k) + y.at(i, j + 3, k);
+          const double d6z = y.at(i, j, k - 3) - 6.0 * y.at(i, j, k - 2) + 15.0 * y.at(i, j, k - 1) - 20.0 * y.at(i, j, k) +
+                             15.0 * y.at(i, j, k + 1) - 6.0 * y.at(i, j, k + 2) + y.at(i, j, k + 3);
+          kv.at(i, j, k) += c[0] * d6x + c[1] * d6y + c[2] * d6z;
+        }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -198,6 +228,7 @@ void rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vect
           kr.at(i, j, k) = dxx + dyy + dzz + src;
         }
   }
+  if (H.sigma != 0.0) add_dissipation(H, b, Y, kout);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -533,6 +564,17 @@ void* oc_create(int nlevels, int nboxes, const int* box_level, const int* box_lo
 }
 
 void oc_destroy(void* h) { delete static_cast<Hier*>(h); }
+
+// Kreiss-Oliger strength sigma of eq (36); needs ghost width >= 3. Returns 0, or -1 with oc_last_error set.
+int oc_set_dissipation(void* h, double sigma) {
+  Hier* H = static_cast<Hier*>(h);
+  if (!H || !(sigma >= 0.0) || (sigma != 0.0 && H->g < 3)) {
+    snprintf(g_err, sizeof g_err, "dissipation needs sigma >= 0 and ghost width >= 3");
+    return -1;
+  }
+  H->sigma = sigma;
+  return 0;
+}
 
 int oc_set_state(void* h, int level, int box, int comp, const double* src) {
   Hier* H = static_cast<Hier*>(h);

@@ -83,6 +83,7 @@ class Workload:
     coarse_steps: int = 1
     init: Optional[Callable[["Workload", int, int, int], np.ndarray]] = None
     note: str = ""
+    ko_sigma: float = 0.0                      # Kreiss-Oliger strength (eqs 35-36); 0 = none
 
     @property
     def nlevels(self) -> int:

@@ -347,3 +347,73 @@ def test_composite_scheme_exact_for_quadratic_solution(oracle_mod, sub):
         got = H.read(0, 0, c)[m, m, m]
         want = wl.quadratic_exact(w, 0, 0, c, t)[m, m, m]
         assert np.max(np.abs(got - want)) < 2e-12, (sub, 0, c)
+
+
+def test_kreiss_oliger_closed_form_amplification(oracle_mod):
+    """Eqs (35)-(36) on one periodic level: on a Fourier mode Q acts as the number
+    q = sigma/64 sum_axis (2 cos 3kh - 12 cos 2kh + 30 cos kh - 20)/h  (<= 0: dissipative), on u AND rho, so
+    M = [[q, 1], [-kappa^2, q]] and n steps apply R(dt M)^n. A wrong sign, a dropped variable, a wrong power of h
+    or a transposed stencil weight changes q."""
+    n, sigma = 16, 0.3
+    w = wl.Workload("t", [wl.Box(0, (0, 0, 0), (n, n, n))], (n, n, n), ko_sigma=sigma)
+    H = oracle_mod.OracleHierarchy.from_workload(
+        wl.Workload("t", w.boxes, w.domain_cells, ko_sigma=sigma, init=lambda *a: np.zeros((n, n, n))))
+    x, y, z = w.centres(0, 0)
+    kv = math.pi * np.array([3, -2, 5])
+    ph = kv[2] * z[:, None, None] + kv[1] * y[None, :, None] + kv[0] * x[None, None, :]
+    s, c = np.sin(ph), np.cos(ph)
+    H.set_state(0, 0, 0, 0.7 * s - 0.2 * c)
+    H.set_state(0, 0, 1, 1.1 * s + 0.4 * c)
+    h = w.dx(0)
+    kappa2 = sum((30 - 32 * math.cos(k * h) + 2 * math.cos(2 * k * h)) / (12 * h * h) for k in kv)
+    q = sigma / 64.0 * sum((2 * math.cos(3 * k * h) - 12 * math.cos(2 * k * h) + 30 * math.cos(k * h) - 20) / h for k in kv)
+    assert q < 0
+    dt, nsteps = 0.25 * h, 25
+    Z = dt * np.array([[q, 1.0], [-kappa2, q]])
+    R = np.linalg.matrix_power(np.eye(2) + Z + Z @ Z / 2 + Z @ Z @ Z / 6 + Z @ Z @ Z @ Z / 24, nsteps)
+    for _ in range(nsteps):
+        H.step(dt, True)
+    a, b = R @ np.array([0.7, 1.1])
+    cc, d = R @ np.array([-0.2, 0.4])
+    assert np.max(np.abs(H.read_level(0, 0, 0) - (a * s + cc * c))) < 2e-13
+    assert np.max(np.abs(H.read_level(0, 0, 1) - (b * s + d * c))) < 2e-12
+    # the undamped scheme gives a different answer at this mode by far more than the tolerance
+    R0 = np.linalg.matrix_power(_amp_matrix(kappa2, dt), nsteps)
+    assert abs((R0 @ np.array([0.7, 1.1]))[0] - a) > 1e-3
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_composite_scheme_with_dissipation_exact_for_quadratic_solution(oracle_mod, sub):
+    """Q annihilates polynomials of degree <= 5, so the exact quadratic solution must survive the composite
+    3-level step with dissipation switched on exactly as without it (every ghost layer the 7-point stencil
+    reads, at every stage, must hold the polynomial)."""
+    n = 64
+    w = wl.Workload("quadratic+KO", wl.nested_cubes(3, n), (n, n, n), init=wl.quadratic_init, ko_sigma=0.2)
+    H = oracle_mod.OracleHierarchy.from_workload(w)
+    H.step(w.dt_coarse, sub)
+    t = w.dt_coarse
+    for l in (1, 2):
+        for c in (0, 1):
+            got = H.read(l, 0, c, padded=True)
+            assert np.max(np.abs(got - wl.quadratic_exact(w, l, 0, c, t, pad=w.ghost))) < 5e-12, (sub, l, c)
+    m = slice(14, n - 14)  # the seam now travels 3 cells per stage
+    for c in (0, 1):
+        assert np.max(np.abs(H.read(0, 0, c)[m, m, m] - wl.quadratic_exact(w, 0, 0, c, t)[m, m, m])) < 5e-12
+
+
+def test_dissipation_damps_grid_noise_and_keeps_smooth_data(oracle_mod):
+    """Nyquist-scale noise decays under Q (one level: |amplification| < 1 for the highest mode), while a smooth
+    mode changes by O(h^5)."""
+    n = 16
+    box = [wl.Box(0, (0, 0, 0), (n, n, n))]
+    i = np.arange(n)
+    checker = ((-1.0) ** (i[:, None, None] + i[None, :, None] + i[None, None, :]))
+    out = {}
+    for sigma in (0.0, 0.5):
+        H = oracle_mod.OracleHierarchy(box, (n, n, n), ko_sigma=sigma)
+        H.set_state(0, 0, 0, np.zeros((n, n, n)))
+        H.set_state(0, 0, 1, 1e-3 * checker)      # rho at the Nyquist mode: Lap u = 0 keeps u = t * rho only
+        for _ in range(10):
+            H.step(0.25 * 2.0 / n, True)
+        out[sigma] = np.max(np.abs(H.read_level(0, 0, 1)))
+    assert out[0.5] < 0.2 * out[0.0]
