@@ -58,6 +58,10 @@ typedef struct {
  *                   comp = nfields+f -> rho_f            (V = 2*nfields arrays per box)
  * coupling: HOST pointer to nfields*nfields doubles, row-major A[f][j], or NULL for A = 0:
  *   d_t u_f = rho_f,   d_t rho_f = Lap_h u_f + sum_j A[f][j] u_j       (BASELINE cfg 4)
+ * ko_sigma: strength of the Kreiss-Oliger dissipation added to the time derivative of EVERY evolved variable,
+ *   d_t y -> RHS + Q y,  Q y = sigma/64 sum_i delta_i^6 y / h_i  (eqs 35-36 with r = 4);
+ *   needs ghost >= 3. With sigma > 0 the step runs the general stage-by-stage kernels (the stage vectors' u parts
+ *   are stored: 5 more arrays per field), with sigma = 0 the two-launch formulation of DESIGN.md section 6.
  * arena: optional DEVICE memory of at least sc_arena_bytes() bytes, 256-byte aligned, owned by the
  *   caller, who keeps it alive and does not touch it until sc_destroy; NULL -> the library allocates.
  * cuda_stream: a cudaStream_t (as void*) on which all work of this hierarchy is enqueued (must not be
@@ -76,6 +80,7 @@ typedef struct {
   void* arena;             /* DEVICE or NULL                                                */
   uint64_t arena_bytes;
   void* cuda_stream;
+  double ko_sigma;         /* Kreiss-Oliger strength sigma >= 0; 0 = none */
 } sc_hierarchy_desc;
 
 typedef struct sc_hierarchy sc_hierarchy; /* opaque; created by sc_create_hierarchy, freed by sc_destroy */

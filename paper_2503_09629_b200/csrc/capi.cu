@@ -335,9 +335,157 @@ void restrict_level(Seq& q, int level) {  // level -> level-1, into the parents'
   }
 }
 
+// ---- NEXT-1: the general stage-by-stage path, used with Kreiss-Oliger dissipation (stage_ko.cu) -----------
+// Arrays of stage s: U_s = a_U(s), R_s = a_R(s) for s = 2..4; Y_1 = y_n lives in the state slot.
+void stage_ko_level(Seq& q, int level, int s, double dt) {
+  sc_hierarchy* h = q.h;
+  const Layout& L = h->L;
+  const int yn = q.cur[level], ynew = 1 - yn, F = L.F;
+  const bool keep_k4 = s == 4 && q.sub && level + 1 < L.nlevels;
+  for (int ib : L.level_boxes[level]) {
+    StageKOArgs a{};
+    a.b = L.boxes[ib].v;
+    a.F = F;
+    a.stage = s;
+    a.yn_u = h->arr(ib, L.a_state(yn));
+    a.yn_r = h->arr(ib, L.a_state(yn) + F);
+    a.Yu = s == 1 ? a.yn_u : h->arr(ib, L.a_U(s));
+    a.Yr = s == 1 ? a.yn_r : h->arr(ib, L.a_R(s));
+    a.outU = s < 4 ? h->arr(ib, L.a_U(s + 1)) : h->arr(ib, L.a_state(ynew));
+    a.outR = s < 4 ? h->arr(ib, L.a_R(s + 1)) : h->arr(ib, L.a_state(ynew) + F);
+    a.U2 = h->arr(ib, L.a_U(2)); a.U3 = h->arr(ib, L.a_U(3));
+    a.R2 = h->arr(ib, L.a_R(2)); a.R3 = h->arr(ib, L.a_R(3));
+    a.K4u = keep_k4 ? h->arr(ib, L.a_K4()) : nullptr;
+    a.K4r = keep_k4 ? h->arr(ib, L.a_K4() + F) : nullptr;
+    a.dt = dt;
+    for (int d = 0; d < 3; ++d) {
+      const double dx = L.dx(level, d);
+      a.inv12dx2[d] = 1.0 / (12.0 * dx * dx);
+      a.ko[d] = L.ko_sigma / (64.0 * dx);
+    }
+    a.A = h->coupling();
+    // reads: Y_s (2 arrays); + y_n (2) for s >= 2; + Y_2, Y_3 (4) for s = 4.  writes: 2 (+ 2 for k_4)
+    const double per = s == 1 ? 4.0 : (s < 4 ? 6.0 : (keep_k4 ? 12.0 : 10.0));
+    prof_begin(h, KIND_STAGE, 8.0 * per * F * cells(a.b));
+    launch_stage_ko(a, h->stream);
+    prof_end(h);
+    ++q.n;
+  }
+}
+
+// ghosts of one stage's output arrays on level 0
+void periodic_stage_ko(Seq& q, int s) {
+  const Layout& L = q.h->L;
+  periodic_level0(q, L.a_U(s), L.F);
+  periodic_level0(q, L.a_R(s), L.F);
+}
+
+// Dense-output ghosts of ALL stage vectors of one level-step of `level` >= 1, one launch
+// per box. The parent stores (y_n, Y_2, Y_3, Y_4, k_4) per variable; with K_j = (Y_{j+1} - y_n)/(a_j h_p) for
+// j = 1..3 the value of eqs (15)-(18) at stage s,  y_n^p + h_p sum_j c^(s)_j K_j,  is the combination
+//   (1 - sum_{j<=3} c_j/a_j) y_n^p + sum_{j<=3} (c_j/a_j) Y_{j+1}^p + h_p c_4 k_4^p
+// — one (5 -> 4) problem for the u variables and one for the rho variables. At theta = 1/2 a third problem
+// prolongs the parent's new state into the shells of y_{n+1} (eq (10) at theta + 1/2 = 1, S8).
+void fill_level_dense_ko(Seq& q, int level, double theta, double dt) {
+  sc_hierarchy* h = q.h;
+  const Layout& L = h->L;
+  const double hp = 2.0 * dt;
+  const int yn = q.cur[level], F = L.F;
+  const int pnew = q.cur[level - 1], pold = 1 - pnew;
+  const double as[3] = {0.5, 0.5, 1.0};
+  for (int ib : L.level_boxes[level]) {
+    GhostArgs a{};
+    a.nprob = 2;
+    for (int v = 0; v < 2; ++v) {  // v = 0: u variables, v = 1: rho variables
+      GhostProblem& d = a.prob[v];
+      d.nsrc = 5;
+      d.nout = 4;
+      d.src_arr[0] = L.a_state(pold) + v * F;
+      d.dst_arr[0] = L.a_state(yn) + v * F;
+      for (int s = 2; s <= 4; ++s) {
+        d.src_arr[s - 1] = v ? L.a_R(s) : L.a_U(s);
+        d.dst_arr[s - 1] = v ? L.a_R(s) : L.a_U(s);
+      }
+      d.src_arr[4] = L.a_K4() + v * F;
+      for (int s = 1; s <= 4; ++s) {
+        double c[4];
+        dense_coeffs(s, theta, c);
+        double c0 = 1.0;
+        for (int j = 0; j < 3; ++j) {
+          d.coef[s - 1][1 + j] = c[j] / as[j];
+          c0 -= c[j] / as[j];
+        }
+        d.coef[s - 1][0] = c0;
+        d.coef[s - 1][4] = hp * c[3];
+      }
+    }
+    if (theta != 0.0) {
+      a.nprob = 3;
+      GhostProblem& e = a.prob[2];
+      e.nsrc = e.nout = 2;
+      e.src_arr[0] = L.a_state(pnew);
+      e.src_arr[1] = L.a_state(pnew) + F;
+      e.dst_arr[0] = L.a_state(1 - yn);
+      e.dst_arr[1] = L.a_state(1 - yn) + F;
+      e.coef[0][0] = 1.0;
+      e.coef[1][1] = 1.0;
+    }
+    ghost_launch(q, ib, a);
+  }
+}
+
+void level_step_ko(Seq& q, int level, double dt, double theta) {
+  const Layout& L = q.h->L;
+  const int yn = q.cur[level];
+  if (level == 0) {
+    if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
+  } else {
+    fill_level_dense_ko(q, level, theta, dt);
+  }
+  for (int s = 1; s <= 4; ++s) {
+    stage_ko_level(q, level, s, dt);
+    if (level == 0) {
+      if (s < 4) periodic_stage_ko(q, s + 1);
+      else periodic_level0(q, L.a_state(1 - yn), L.V);
+    }
+  }
+  if (level == 0) q.l0_valid = true;
+  q.cur[level] = 1 - yn;
+}
+
+// non-subcycled step with dissipation (S11/S15): same-time prolongation of the parent's same stage vector
+void uniform_step_ko(Seq& q, double dt) {
+  const Layout& L = q.h->L;
+  const int Lv = L.nlevels, F = L.F;
+  if (!q.l0_valid) periodic_level0(q, L.a_state(q.cur[0]), L.V);
+  for (int l = 1; l < Lv; ++l) {
+    const int ca[2] = {L.a_state(q.cur[l]), L.a_state(q.cur[l]) + F};
+    const int pa[2] = {L.a_state(q.cur[l - 1]), L.a_state(q.cur[l - 1]) + F};
+    fill_level_same_time(q, l, 2, ca, pa);
+  }
+  for (int s = 1; s <= 4; ++s) {
+    for (int l = 0; l < Lv; ++l) stage_ko_level(q, l, s, dt);
+    if (s < 4) {
+      periodic_stage_ko(q, s + 1);
+      const int ca[2] = {L.a_U(s + 1), L.a_R(s + 1)};
+      for (int l = 1; l < Lv; ++l) fill_level_same_time(q, l, 2, ca, ca);
+    }
+  }
+  periodic_level0(q, L.a_state(1 - q.cur[0]), L.V);
+  q.l0_valid = true;
+  for (int l = 1; l < Lv; ++l) {
+    const int ca[2] = {L.a_state(1 - q.cur[l]), L.a_state(1 - q.cur[l]) + F};
+    const int pa[2] = {L.a_state(1 - q.cur[l - 1]), L.a_state(1 - q.cur[l - 1]) + F};
+    fill_level_same_time(q, l, 2, ca, pa);
+  }
+  for (int l = 0; l < Lv; ++l) q.cur[l] = 1 - q.cur[l];
+  for (int l = Lv - 1; l >= 1; --l) restrict_level(q, l);
+}
+
 // One RK4 step of one level (eqs 1-9) with its ghost fills. theta: start of this step inside the parent's.
 void level_step(Seq& q, int level, double dt, double theta) {
   const Layout& L = q.h->L;
+  if (L.ko_sigma > 0.0) { level_step_ko(q, level, dt, theta); return; }
   const int yn = q.cur[level];
   if (level == 0) {
     if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
@@ -367,6 +515,7 @@ void advance(Seq& q, int level, double dt, double theta) {
 // non-subcycled step of all levels (reading S11/S15)
 void uniform_step(Seq& q, double dt) {
   const Layout& L = q.h->L;
+  if (L.ko_sigma > 0.0) { uniform_step_ko(q, dt); return; }
   const int Lv = L.nlevels, F = L.F;
   // ghosts of y_n = (u_n, rho_n): from the parent's y_n after the last restriction
   if (!q.l0_valid) periodic_level0(q, L.a_state(q.cur[0]), L.V);

@@ -44,7 +44,13 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
     for (int q = 0; q < d->nfields * d->nfields; ++q)
       if (!std::isfinite(d->coupling[q])) return fail(err, SC_ERR_INVALID_ARG, "non-finite coupling entry %d", q);
 
+  if (!(d->ko_sigma >= 0.0) || !std::isfinite(d->ko_sigma))
+    return fail(err, SC_ERR_INVALID_ARG, "ko_sigma must be finite and >= 0");
+  if (d->ko_sigma > 0.0 && d->ghost < 3)
+    return fail(err, SC_ERR_UNSUPPORTED, "Kreiss-Oliger dissipation reads 3 ghost layers (ghost = %d)", d->ghost);
+
   L->nlevels = d->nlevels;
+  L->ko_sigma = d->ko_sigma;
   L->g = d->ghost;
   L->F = d->nfields;
   L->V = 2 * d->nfields;
@@ -121,7 +127,7 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
   // of 32 doubles, so every array starts on a 256-byte boundary
   unsigned long long off = 0;
   for (BoxInfo& b : L->boxes) {
-    b.narrays = 2 * L->V + 3 * L->F + (L->has_coupling ? 2 * L->F : 0);
+    b.narrays = 2 * L->V + 3 * L->F + (L->has_coupling ? 2 * L->F : 0) + (L->ko_sigma > 0.0 ? 3 * L->F + L->V : 0);
     b.arena_offset = off;
     off += (unsigned long long)b.narrays * (unsigned long long)b.v.vol * sizeof(double);
   }

@@ -52,6 +52,33 @@ int launch_stage(const StageArgs& a, cudaStream_t st);  // returns the number of
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128);
 
 // ------------------------------------------------------------------------------------------------
+// NEXT-1: one RK4 stage of the general formulation with Kreiss-Oliger dissipation (stage_ko.cu).
+// All pointers are field-0 arrays of one box; field f is f arrays further.
+// ------------------------------------------------------------------------------------------------
+struct StageKOArgs {
+  BoxView b;
+  int F;
+  int stage;             // 1..4
+  const double* Yu;      // u- and rho-part of the stage vector Y_s (stage 1: the state y_n), read with 3 ghost layers
+  const double* Yr;
+  const double* yn_u;    // y_n, centre only
+  const double* yn_r;
+  double* outU;          // stage < 4: Y_{s+1};  stage 4: y_{n+1}
+  double* outR;
+  const double* U2;      // stage 4, centre only: Y_2, Y_3 (Y_4 is Yu, Yr)
+  const double* U3;
+  const double* R2;
+  const double* R3;
+  double* K4u;           // stage 4: k_4, or null where no child reads it
+  double* K4r;
+  double dt;
+  double inv12dx2[3];    // 1 / (12 dx_a^2)
+  double ko[3];          // sigma / (64 dx_a)
+  const double* A;       // device F*F coupling, or null
+};
+void launch_stage_ko(const StageKOArgs& a, cudaStream_t st);
+
+// ------------------------------------------------------------------------------------------------
 // a3: refinement-boundary ghost fill. One launch fills, for every ghost cell of a level >= 1 box, the shells
 // of up to GF_MAX_PROB independent PROBLEMS; problem p writes, for every output o,
 //     child array dst_arr[o] (ghost cell) = P[ sum_s coef[o][s] * parent array src_arr[s] ]
@@ -61,7 +88,7 @@ bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, vo
 // (2 -> 2) same-time prolongation of the parent's new state. Arrays are named by their index inside the
 // box (sc_internal.h); field f of every source / output is f arrays further.
 // ------------------------------------------------------------------------------------------------
-constexpr int GF_MAX_SRC = 5, GF_MAX_OUT = 4, GF_MAX_PROB = 2;
+constexpr int GF_MAX_SRC = 5, GF_MAX_OUT = 4, GF_MAX_PROB = 3;
 
 struct GhostTile {   // one work tile of a ghost slab; everything the kernel needs is precomputed on the host
   int axis;                // the slab's thin axis: 0 = x-slab, 1 = y-slab, 2 = z-slab

@@ -12,6 +12,8 @@
 //     [2V+F, 2V+2F)     Y3r = rho-part of Y_3 (eq 8)
 //     [2V+2F, 2V+3F)    Y4r = rho-part of Y_4 (eq 9)
 //     [2V+3F, 2V+5F)    only if a coupling matrix is set: scratch for A*u_n and A*R of the current stage
+//     then, only with Kreiss-Oliger dissipation (ko_sigma > 0): U2, U3, U4 (F each: u-parts of the stage
+//                       vectors) and K4 (V: the slope k_4), see stage_ko.cu
 // The u-parts of the stage vectors and the slopes k_1..k_4 are never materialised (S26): for
 // d_t u = rho the slope k_{s,u} IS Y_{s,rho}, so Y_{s+1,u} = u_n + a_s dt Y_{s,rho} is rebuilt where it is
 // needed, and k_{s,rho} = (Y_{s+1,rho} - rho_n)/(a_s dt). After a level-step the child level reads
@@ -73,6 +75,7 @@ struct Layout {
   unsigned long long coupling_offset = 0;   // bytes into the arena (F*F doubles) if has_coupling
   unsigned long long arena_bytes = 0;
   bool has_coupling = false;
+  double ko_sigma = 0.0;                    // > 0: Kreiss-Oliger dissipation, general stage-by-stage path
   double dx(int level, int a) const { return (xhi[a] - xlo[a]) / ((double)domain[a] * (double)(1u << level)); }
   // first array index of each role
   int a_state(int slot) const { return slot * V; }
@@ -80,6 +83,11 @@ struct Layout {
   int a_Y3r() const { return 2 * V + F; }
   int a_Y4r() const { return 2 * V + 2 * F; }
   int a_scratch() const { return 2 * V + 3 * F; }
+  // dissipation path only: u-parts of Y_2..Y_4 (the rho-parts are Y2r..Y4r) and the slope k_4 (u, then rho)
+  int a_extra() const { return 2 * V + 3 * F + (has_coupling ? 2 * F : 0); }
+  int a_U(int s) const { return a_extra() + (s - 2) * F; }   // s = 2, 3, 4
+  int a_R(int s) const { return 2 * V + (s - 2) * F; }       // = Y2r, Y3r, Y4r
+  int a_K4() const { return a_extra() + 3 * F; }             // V arrays
 };
 
 // Validate a description and compute the layout. Host only, no CUDA calls.

@@ -255,3 +255,70 @@ def test_exact_quadratic_solution_without_the_oracle(sub):
     for c in (0, 1):
         assert np.max(np.abs(G.sc_read_level(0, 0, c)[m, m, m] - wl.quadratic_exact(w, 0, 0, c, t)[m, m, m])) < 2e-12
     G.close()
+
+
+# ---- NEXT-1: Kreiss-Oliger dissipation (eqs 35-36), general stage-by-stage path -------------------
+def _with_ko(w, sigma=0.25):
+    w.ko_sigma = sigma
+    w.name += f" + KO sigma={sigma}"
+    return w
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_ko_cfg1_full_run(sub):
+    w = _with_ko(wl.cfg1())
+    G, O = _pair(w)
+    for _ in range(w.coarse_steps):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+    rel = _compare_state(G, O, w, what=f"KO cfg1 sub={sub}")
+    print(f"KO cfg1 sub={sub}: max rel diff {rel:.2e}")
+    # the dissipation did something: the undamped run differs by far more than the tolerance
+    G0 = sc.Hierarchy.from_workload(wl.cfg1())
+    for _ in range(w.coarse_steps):
+        G0.sc_step(w.dt_coarse, sub)
+    assert np.max(np.abs(G0.sc_read_level(1, 0, 0) - G.sc_read_level(1, 0, 0))) > 1e-8
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_ko_ragged_multibox_coupled(sub):
+    w = _with_ko(wl.ragged_small(), 0.1)
+    G, O = _pair(w)
+    for _ in range(3):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+        _compare_state(G, O, w, what=f"KO ragged sub={sub}")
+
+
+def test_ko_four_levels_and_mode_switch():
+    w = _with_ko(wl.cfg3(n=48, nlevels=4), 0.3)
+    G, O = _pair(w)
+    for sub in (True, False, True):
+        G.sc_step(w.dt_coarse, sub)
+        O.step(w.dt_coarse, sub)
+    _compare_state(G, O, w, what="KO cfg3/48")
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_ko_exact_quadratic_solution_without_the_oracle(sub):
+    n = 64
+    w = wl.Workload("quadratic+KO", wl.nested_cubes(3, n), (n, n, n), init=wl.quadratic_init, ko_sigma=0.2)
+    G = sc.Hierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, sub)
+    t = w.dt_coarse
+    for l in (1, 2):
+        for c in (0, 1):
+            got = G.sc_debug_read_padded(l, 0, c)
+            assert np.max(np.abs(got - wl.quadratic_exact(w, l, 0, c, t, pad=w.ghost))) < 5e-12, (sub, l, c)
+    m = slice(14, n - 14)
+    for c in (0, 1):
+        assert np.max(np.abs(G.sc_read_level(0, 0, c)[m, m, m] - wl.quadratic_exact(w, 0, 0, c, t)[m, m, m])) < 5e-12
+    G.close()
+
+
+def test_ko_needs_three_ghost_layers():
+    w = wl.cfg1()
+    w.ghost = 2
+    w.ko_sigma = 0.1
+    with pytest.raises(sc.SubcycleError):
+        sc.Hierarchy.from_workload(w)
