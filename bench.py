@@ -33,8 +33,12 @@ METRIC = "grid-point updates/s (all levels, fp64 RK4)"
 UNIT = "updates/s"
 
 
-def pick_workload(idx: int):
-    return {1: wl.cfg1, 2: lambda: wl.cfg2(128), 3: wl.cfg3, 4: wl.cfg4, 5: wl.cfg5}[idx]()
+def pick_workload(idx: int, sigma: float = 0.0):
+    w = {1: wl.cfg1, 2: lambda: wl.cfg2(128), 3: wl.cfg3, 4: wl.cfg4, 5: wl.cfg5}[idx]()
+    if sigma:
+        w.ko_sigma = sigma
+        w.name += f" + Kreiss-Oliger sigma={sigma}"
+    return w
 
 
 def measured_peaks():
@@ -56,7 +60,7 @@ def oracle_sample(w, max_levels: int):
         return w, f"all {w.nlevels} levels"
     boxes = [b for b in w.boxes if b.level < max_levels]
     s = wl.Workload(w.name + f" [levels 0..{max_levels - 1}]", boxes, w.domain_cells, w.nfields, w.ghost,
-                    w.xlo, w.xhi, w.coupling, w.coarse_steps, w.init)
+                    w.xlo, w.xhi, w.coupling, w.coarse_steps, w.init, ko_sigma=w.ko_sigma)
     return s, f"levels 0..{max_levels - 1} of {w.nlevels} ({'+'.join(str(b.n[0]) + '^3' for b in boxes)})"
 
 
@@ -82,7 +86,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    w = pick_workload(args.config)
+    w = pick_workload(args.config, args.sigma)
     sub = args.mode == "sub"
     r = time_oracle(w, max(1, args.steps), min(args.warmup, 1), sub, max_levels=args.oracle_levels)
     ms = 1e3 * r.pop("_seconds") / r.pop("_steps")
@@ -177,10 +181,11 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    w = pick_workload(args.config)
+    w = pick_workload(args.config, args.sigma)
     sub = args.mode == "sub"
     dt = w.dt_coarse
-    H = sc.Hierarchy(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling, device=f"cuda:{local}")
+    H = sc.Hierarchy(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling, device=f"cuda:{local}",
+                     ko_sigma=w.ko_sigma)
 
     # inputs: seeded synthetic state, staged in pinned host memory (also the e2e source buffers)
     host_in, host_out = {}, {}
@@ -233,7 +238,7 @@ def run_gpu(args):
     dom = max(kinds, key=lambda k: kinds[k]["ms_total"])
     ksum = sum(k["ms_total"] for k in kinds.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["algorithmic_GBps"], "peak": peak,
-                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom) if args.config == 5 else None,
+                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom) if args.config == 5 and not args.sigma else None,
                 "peak_source": peak_src, "share_of_step": kinds[dom]["ms_total"] / ksum,
                 "bytes_per_launch": kinds[dom]["bytes_per_launch"], "avg_launch_us": kinds[dom]["avg_us"]}
 
@@ -273,7 +278,7 @@ def run_gpu(args):
             "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "mode": "subcycled" if sub else "uniform", "ghost": w.ghost,
-                       "nfields": w.nfields, "dt_coarse": dt, "updates_per_step": upd_step,
+                       "nfields": w.nfields, "ko_sigma": w.ko_sigma, "dt_coarse": dt, "updates_per_step": upd_step,
                        "zone_cycles_per_step": w.zone_cycles_per_coarse_step(),
                        "l2": "inputs larger than L2 (state + stage buffers %.1f GB)" % (H.arena_bytes / 1e9),
                        "parallelism": "replicas only" if world > 1 else "1 GPU"},
@@ -300,6 +305,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--mode", default="sub", choices=["sub", "uniform"])
+    ap.add_argument("--sigma", type=float, default=0.0,
+                    help="Kreiss-Oliger dissipation strength (PAPER.md eqs 35-36); 0 = the configs as BASELINE states them")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--oracle-levels", type=int, default=2,
                     help="levels of the workload the CPU oracle is timed on (bounded sample)")

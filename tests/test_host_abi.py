@@ -107,3 +107,18 @@ def test_null_and_range_errors_do_not_abort(built):
     assert L.sc_read_level(None, 0, 0, 0, None, 0) == SC_ERR_INVALID_ARG
     assert L.sc_destroy(None) == 0
     assert L.sc_time(None) == 0.0
+
+
+def test_dissipation_in_the_description(built):
+    """ko_sigma (eqs 35-36): validated on the host, and it buys 5 more arrays per field (U2..U4, k_4)."""
+    w = wl.cfg3(n=32, nlevels=3)
+    base = _bytes(w)
+    d, keep = sc.make_desc(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling, ko_sigma=0.2)
+    with_ko = sc.sc_arena_bytes(d)
+    assert with_ko > base and abs(with_ko / base - 12.0 / 7.0) < 0.01
+    for bad in (-0.1, float("nan"), float("inf")):
+        d, keep = sc.make_desc(w.boxes, w.domain_cells, ko_sigma=bad)
+        assert sc.lib().sc_arena_bytes(d) == 0
+    d, keep = sc.make_desc(w.boxes, w.domain_cells, ghost=2, ko_sigma=0.1)   # Q reads 3 ghost layers
+    assert sc.lib().sc_arena_bytes(d) == 0
+    assert b"ghost" in sc.lib().sc_last_error()
