@@ -66,6 +66,8 @@ struct sc_hierarchy {
   struct GMaps { TMap m[3]; };
   std::vector<GMaps> gmaps;       // per box: ghost-fill footprint maps of the box as PARENT (thin axis x, y, z)
   std::vector<char> gmap_ok;
+  std::vector<TMap> kmaps;        // per box: halo-3 tile of the dissipative stage kernel (ko_sigma > 0)
+  std::vector<char> kmap_ok;
   // per-launch CUDA-event timing (sc_profile): eager launches, one event pair per kernel
   bool profiling = false;
   struct ProfRec { int kind; double bytes; cudaEvent_t e0, e1; };
@@ -364,6 +366,9 @@ void stage_ko_level(Seq& q, int level, int s, double dt) {
       a.ko[d] = L.ko_sigma / (64.0 * dx);
     }
     a.A = h->coupling();
+    a.tmap = h->kmap_ok[ib] ? h->kmaps[ib].bytes : nullptr;
+    a.a_Yu = s == 1 ? L.a_state(yn) : L.a_U(s);
+    a.a_Yr = s == 1 ? L.a_state(yn) + F : L.a_R(s);
     // reads: Y_s (2 arrays); + y_n (2) for s >= 2; + Y_2, Y_3 (4) for s = 4.  writes: 2 (+ 2 for k_4)
     const double per = s == 1 ? 4.0 : (s < 4 ? 6.0 : (keep_k4 ? 12.0 : 10.0));
     prof_begin(h, KIND_STAGE, 8.0 * per * F * cells(a.b));
@@ -676,11 +681,15 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   h->tmap_ok.assign(h->L.boxes.size(), 0);
   h->rmaps.resize(h->L.boxes.size());
   h->gmaps.resize(h->L.boxes.size());
+  h->kmaps.resize(h->L.boxes.size());
+  h->kmap_ok.assign(h->L.boxes.size(), 0);
   h->gmap_ok.assign(h->L.boxes.size(), 0);
   for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
     const BoxInfo& b = h->L.boxes[ib];
     h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
+    h->kmap_ok[ib] = h->L.ko_sigma > 0.0 &&
+                     make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 5, h->kmaps[ib].bytes);
     h->gmap_ok[ib] = 1;
     for (int ax = 0; ax < 3; ++ax)
       if (!make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 2 + ax, h->gmaps[ib].m[ax].bytes)) h->gmap_ok[ib] = 0;

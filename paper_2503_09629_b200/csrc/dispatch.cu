@@ -19,6 +19,10 @@ bool ghost_tma_takes(const GhostArgs& a);
 void ghost_box_dims(int axis, unsigned box[4]);
 void launch_restrict_ref(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st);
 void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st);
+void launch_stage_ko_direct(const StageKOArgs& a, cudaStream_t st);
+void launch_stage_ko_tma(const StageKOArgs& a, cudaStream_t st);
+bool stage_ko_tma_takes(const StageKOArgs& a);
+void stageko_box_dims(unsigned box[4]);
 
 static int g_mode = 1;
 void select_kernels(int mode) { g_mode = mode; }
@@ -27,6 +31,10 @@ int selected_kernels() { return g_mode; }
 int launch_stage(const StageArgs& a, cudaStream_t st) {
   if (g_mode == 0) { launch_stage_direct(a, st); return 1; }
   return launch_stage_tma(a, st);
+}
+void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {
+  if (g_mode == 0 || !stage_ko_tma_takes(a)) launch_stage_ko_direct(a, st);
+  else launch_stage_ko_tma(a, st);
 }
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st) {
   if (g_mode == 0 || !ghost_tma_takes(a)) launch_ghost_fill_direct(a, st);
@@ -40,10 +48,11 @@ bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, vo
   unsigned box[4];
   if (kind == 0) stage_box_dims(box);
   else if (kind == 1) restrict_box_dims(box);
-  else ghost_box_dims(kind - 2, box);
+  else if (kind <= 4) ghost_box_dims(kind - 2, box);
+  else stageko_box_dims(box);
   // streaming tiles (stage, restriction) promote misses to 256-byte fetches; the ghost fill's footprint rows are
   // 64-160 bytes and isolated: promotion there only multiplies the DRAM traffic
-  return make_box_tensor_map_tma(b, narrays, base, box, kind <= 1 ? 256 : 0, out_map128);
+  return make_box_tensor_map_tma(b, narrays, base, box, (kind <= 1 || kind == 5) ? 256 : 0, out_map128);
 }
 
 }  // namespace sc

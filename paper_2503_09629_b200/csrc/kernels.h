@@ -47,7 +47,7 @@ struct StageArgs {
 int launch_stage(const StageArgs& a, cudaStream_t st);  // returns the number of kernels launched
 // 128-byte CUtensorMaps of a box: dims (px, py, pz, narrays), fp64, no swizzle; kind 0: box = the stage
 // kernels' halo tile, kind 1: box = the restriction kernel's pair of fine planes, kinds 2..4: the ghost
-// fill's parent footprint of a tile of an x- / y- / z-slab. Returns false (and leaves
+// fill's parent footprint of a tile of an x- / y- / z-slab, kind 5: the dissipative stage kernel's halo-3 tile. Returns false (and leaves
 // the direct-load kernels in charge) when the driver entry point is unavailable or a TMA limit is violated.
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128);
 
@@ -75,6 +75,8 @@ struct StageKOArgs {
   double inv12dx2[3];    // 1 / (12 dx_a^2)
   double ko[3];          // sigma / (64 dx_a)
   const double* A;       // device F*F coupling, or null
+  const void* tmap;      // host pointer to the box's stage_ko CUtensorMap (kind 5), or null -> direct-load kernel
+  int a_Yu, a_Yr;        // array indices of Yu, Yr (field 0) in the tensor map
 };
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st);
 

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) stage_ko(const __grid_constant__ StageKOA
   }
 }
 
-void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {
+void launch_stage_ko_direct(const StageKOArgs& a, cudaStream_t st) {
   dim3 blk(64, 4, 1);
   dim3 grd((a.b.n[0] + 63) / 64, (a.b.n[1] + 3) / 4, a.b.n[2] * a.F);
   stage_ko<<<grd, blk, 0, st>>>(a);

@@ -300,7 +300,7 @@ template <int MODE>
 size_t stage_smem() { return (size_t)NST * (MODE == STAGE_12 ? 2 : 3) * TILE_DOUBLES * 8 + NST * 8 + 128; }
 
 // z-chunks per column: enough CTAs to fill the machine in whole waves, as few halo planes as possible
-int pick_chunks(const BoxView& b, int F, int ctas_per_sm) {
+int pick_chunks_impl(const BoxView& b, int F, int ctas_per_sm, int halo_planes) {
   static const int forced = [] { const char* e = getenv("SC_ZCHUNKS"); return e ? atoi(e) : 0; }();
   static const int nsm = [] {
     int dev = 0, n = 148;
@@ -317,11 +317,13 @@ int pick_chunks(const BoxView& b, int F, int ctas_per_sm) {
     const int ch = (b.n[2] + nch - 1) / nch;
     const long long ctas = cols * ((b.n[2] + ch - 1) / ch);
     const long long waves = (ctas + slots - 1) / slots;
-    const double cost = (double)waves * (ch + 4 + 6);  // time ~ waves x (planes marched + pipeline fill)
+    const double cost = (double)waves * (ch + halo_planes + 6);  // time ~ waves x (planes marched + pipeline fill)
     if (cost < best_cost - 1e-9) { best_cost = cost; best = nch; }
   }
   return best;
 }
+
+int pick_chunks(const BoxView& b, int F, int ctas_per_sm) { return pick_chunks_impl(b, F, ctas_per_sm, 4); }
 
 template <int MODE, bool COUPLED>
 void launch_zmarch(const StageArgs& a, cudaStream_t st) {
@@ -434,6 +436,10 @@ void launch_couple_matvec(const StageArgs& a, cudaStream_t st) {
   else launch_couple_mode<STAGE_34>(p, a.A_host, st);
 }
 }  // namespace
+
+int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes) {
+  return pick_chunks_impl(b, F, ctas_per_sm, halo_planes);
+}
 
 void stage_box_dims(unsigned box[4]) { box[0] = HX; box[1] = HY; box[2] = 1; box[3] = 1; }
 
