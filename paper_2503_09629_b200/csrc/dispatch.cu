@@ -10,7 +10,7 @@ namespace sc {
 void launch_stage_direct(const StageArgs& a, cudaStream_t st);
 int launch_stage_tma(const StageArgs& a, cudaStream_t st);
 bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned box[4], int l2_promotion,
-                             void* out_map128);
+                             bool swizzle64, void* out_map128);
 void stage_box_dims(unsigned box[4]);
 void restrict_box_dims(unsigned box[4]);
 void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
@@ -51,8 +51,9 @@ bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, vo
   else if (kind <= 4) ghost_box_dims(kind - 2, box);
   else stageko_box_dims(box);
   // streaming tiles (stage, restriction) promote misses to 256-byte fetches; the ghost fill's footprint rows are
-  // 64-160 bytes and isolated: promotion there only multiplies the DRAM traffic
-  return make_box_tensor_map_tma(b, narrays, base, box, (kind <= 1 || kind == 5) ? 256 : 0, out_map128);
+  // 64-160 bytes and isolated: promotion there only multiplies the DRAM traffic. The x-slab footprint (kind 2,
+  // 64-byte rows) is swizzled so that one-thread-per-row reads are bank-conflict free (ghost_tma.cu).
+  return make_box_tensor_map_tma(b, narrays, base, box, (kind <= 1 || kind == 5) ? 256 : 0, kind == 2, out_map128);
 }
 
 }  // namespace sc

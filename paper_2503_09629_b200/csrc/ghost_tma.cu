@@ -37,24 +37,27 @@ void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
 
 namespace {
 
-// Tile geometry per thin axis AX. z- and y-slabs (A = x): 32 x 16 fine cells. x-slabs (A = y, thin = x):
-// 16 x 16, and the footprint's x extent is loaded as 8 doubles from an EVEN x coordinate — a TMA tiled load
-// whose innermost fp64 coordinate is odd (start not 16-byte aligned) faults on sm_100a (measured).
-constexpr int TB = 16, PB = TB / 2 + 4;          // fine cells / parent footprint along B
+// Tile geometry per thin axis AX: 32 x 16 fine cells along (A, B). x-slabs (A = y, thin = x): the footprint's
+// x extent is loaded as 8 doubles from an EVEN x coordinate — a TMA tiled load whose innermost fp64
+// coordinate is odd (start not 16-byte aligned) faults on sm_100a (measured) — through a SWIZZLE_64B tensor
+// map: the 64-byte rows land with their 16-byte chunks XOR-ed by bits 1-2 of the row index, so that phase 1's
+// one-thread-per-row 16-byte loads are bank-conflict free.
+constexpr int TA = 32, PA = TA / 2 + 4;          // fine cells / parent footprint along A (2-cell halo each side)
+constexpr int TB = 16, PB = TB / 2 + 4;          // ... along B
 constexpr int PT = 6;                            // parent cells along the thin axis (ghost width <= 4)
 constexpr int PTX = 8;                           // ... as loaded for x-slabs (even start, 64-byte rows)
-constexpr int PAMAX = 20;                        // pitch of T and U rows
+constexpr int PAMAX = PA;                        // pitch of a T row
+constexpr int TPLANE = PB * PAMAX + 4;           // pitch of a T plane: 8 banks past a multiple of 32 (x-slab lanes)
 template <int AX> struct Geo {
-  static constexpr int TA = AX == 0 ? 16 : 32;   // fine cells along A
-  static constexpr int PA = TA / 2 + 4;          // parent footprint along A (2-cell halo each side)
   static constexpr int FOOT = AX == 0 ? PTX * PA * PB : PA * PB * PT;  // doubles per source footprint
 };
-constexpr int FOOTMAX = Geo<2>::FOOT;            // 1440 doubles = 11520 B: stride between sources in smem
+constexpr int FOOTMAX = Geo<0>::FOOT;            // 1920 doubles = 15360 B: stride between sources in smem
 constexpr int NTHR = 256;
-static_assert(Geo<0>::FOOT <= FOOTMAX && Geo<1>::FOOT == FOOTMAX, "source slots are FOOTMAX doubles");
-static_assert(Geo<2>::PA * PB <= NTHR && Geo<2>::PA <= PAMAX, "phase 1: one thread per parent column");
-static_assert(TB * (Geo<2>::TA / 2) == NTHR && TB * Geo<0>::TA == NTHR, "phase 3 thread maps");
-static_assert((FOOTMAX * 8) % 128 == 0 && (Geo<0>::FOOT * 8) % 16 == 0, "TMA destination alignment");
+static_assert(Geo<1>::FOOT <= FOOTMAX && Geo<2>::FOOT <= FOOTMAX, "source slots are FOOTMAX doubles");
+static_assert(PA * PB <= NTHR, "phase 1: one thread per parent column");
+static_assert((TA / 2) * GF_MAX_OUT * 4 == NTHR, "phase 2: thread = (output, thin cell, parent column)");
+static_assert((FOOTMAX * 8) % 1024 == 0, "TMA destination alignment (swizzle atom)");
+static_assert((TPLANE * 2) % 32 == 8, "x-slab phase 2: the four thin-cell lanes of a column hit distinct banks");
 
 __device__ __forceinline__ uint32_t smem_u32g(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_wait_g(uint32_t bar, uint32_t parity) {
@@ -82,14 +85,13 @@ __device__ __forceinline__ void children(const double* p, double& lo, double& hi
   lo = w4 * a + w3 * b + w2 * c + w1 * d + w0 * e;  // parity 0: -1/4
 }
 
-// shared-memory index of footprint cell (ia, ib, c) of a tile whose thin axis is AX: the layout the TMA box
-// of that axis produces (x fastest)
+// shared-memory index of footprint cell (ia, ib, c) of a tile whose thin axis is AX (1 or 2): the layout the
+// TMA box of that axis produces (x fastest)
 template <int AX>
 __device__ __forceinline__ int raw_idx(int ia, int ib, int c) {
-  constexpr int PA = Geo<AX>::PA;
+  static_assert(AX != 0, "x-slab rows are read as swizzled 16-byte chunks");
   if (AX == 2) return (c * PB + ib) * PA + ia;   // box (PA x, PB y, PT z)
-  if (AX == 1) return (ib * PT + c) * PA + ia;   // box (PA x, PT y, PB z)
-  return (ib * PA + ia) * PTX + c;               // box (PTX x, PA y, PB z); c counts from the even start
+  return (ib * PT + c) * PA + ia;                // box (PA x, PT y, PB z)
 }
 
 // ---- phase 1: thin-axis interpolation of every source, then the time combination ---------------------
@@ -103,10 +105,10 @@ __device__ __forceinline__ double ip5(const double* L) {
 }
 // PAR >= 0: ghost width 3 and PAR = parity of the first thin cell: the (parent cell, parity) pattern of the
 // three thin cells is known at compile time (no weight table, no barrier). PAR < 0: any width, weights in sWt.
-template <int AX, int NS, int NO, int PAR>
-__device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, int xoff, const double* __restrict__ raw,
+// XO (x-slabs): position of footprint cell 0 inside the loaded 8-wide row.
+template <int AX, int NS, int NO, int PAR, int XO>
+__device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, const double* __restrict__ raw,
                                        double* __restrict__ T, const double (*sWt)[PT], int tid) {
-  constexpr int PA = Geo<AX>::PA;
   if (tid >= PA * PB) return;
   const int ia = tid % PA, ib = tid / PA;
   double acc[NO][4];
@@ -117,8 +119,22 @@ __device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, int xoff,
 #pragma unroll
   for (int s = 0; s < NS; ++s) {
     double L[PT];
+    if (AX == 0) {  // row tid of the (PTX x, PA y, PB z) box; chunk q sits at q ^ bits 1-2 of the row (SWIZZLE_64B)
+      const double2* __restrict__ row = reinterpret_cast<const double2*>(raw + s * FOOTMAX) + tid * 4;
+      const int sw = (tid >> 1) & 3;
+      double d[PTX];
 #pragma unroll
-    for (int c = 0; c < PT; ++c) L[c] = raw[s * FOOTMAX + raw_idx<AX>(ia, ib, c) + (AX == 0 ? xoff : 0)];
+      for (int q = 0; q < (XO ? 4 : 3); ++q) {
+        const double2 t2 = row[q ^ sw];
+        d[2 * q] = t2.x;
+        d[2 * q + 1] = t2.y;
+      }
+#pragma unroll
+      for (int c = 0; c < PT; ++c) L[c] = d[c + XO];
+    } else {
+#pragma unroll
+      for (int c = 0; c < PT; ++c) L[c] = raw[s * FOOTMAX + raw_idx<AX == 0 ? 1 : AX>(ia, ib, c)];
+    }
     double v[4];
     if (PAR == 0) {         // first thin cell even: (j, parity) = (2,0), (2,1), (3,0)
       v[0] = ip5<0>(L); v[1] = ip5<1>(L); v[2] = ip5<0>(L + 1); v[3] = 0.0;
@@ -148,134 +164,133 @@ __device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, int xoff,
   for (int o = 0; o < NO; ++o)
 #pragma unroll
     for (int k = 0; k < (PAR >= 0 ? 3 : 4); ++k)
-      if (k < nt) T[((o * (PAR >= 0 ? 3 : nt) + k) * PB + ib) * PAMAX + ia] = acc[o][k];
+      if (k < nt) T[(o * (PAR >= 0 ? 3 : nt) + k) * TPLANE + ib * PAMAX + ia] = acc[o][k];
 }
-template <int AX, int NS, int NO>
-__device__ __forceinline__ void phase1_par(int par, const GhostProblem& pr, int nt, int xoff,
-                                           const double* __restrict__ raw, double* __restrict__ T,
-                                           const double (*sWt)[PT], int tid) {
-  if (par == 0) phase1<AX, NS, NO, 0>(pr, nt, xoff, raw, T, sWt, tid);
-  else if (par == 1) phase1<AX, NS, NO, 1>(pr, nt, xoff, raw, T, sWt, tid);
-  else phase1<AX, NS, NO, -1>(pr, nt, xoff, raw, T, sWt, tid);
+template <int AX, int NS, int NO, int XO>
+__device__ __forceinline__ void phase1_par(int par, const GhostProblem& pr, int nt, const double* __restrict__ raw,
+                                           double* __restrict__ T, const double (*sWt)[PT], int tid) {
+  if (par == 0) phase1<AX, NS, NO, 0, XO>(pr, nt, raw, T, sWt, tid);
+  else if (par == 1) phase1<AX, NS, NO, 1, XO>(pr, nt, raw, T, sWt, tid);
+  else phase1<AX, NS, NO, -1, XO>(pr, nt, raw, T, sWt, tid);
 }
-
-// ---- phase 2: interpolation along B, register-blocked ------------------------------------------------
-template <int AX>
-__device__ __forceinline__ void phase2(int nplanes, const double* __restrict__ T, double* __restrict__ U, int tid) {
-  constexpr int PA = Geo<AX>::PA;
-  for (int w = tid; w < nplanes * PA; w += NTHR) {
-    const int ia = w % PA, pl = w / PA;
-    const double* __restrict__ in = T + pl * (PB * PAMAX) + ia;
-    double* __restrict__ out = U + pl * (TB * PAMAX) + ia;
-    double v[PB];
-#pragma unroll
-    for (int j = 0; j < PB; ++j) v[j] = in[j * PAMAX];
-#pragma unroll
-    for (int j = 0; j < TB / 2; ++j) {
-      double lo, hi;
-      children(&v[j + 2], lo, hi);
-      out[(2 * j) * PAMAX] = lo;
-      out[(2 * j + 1) * PAMAX] = hi;
-    }
-  }
+template <int NS, int NO>
+__device__ __forceinline__ void phase1_any(const GhostTile& t, const GhostProblem& pr, const double* __restrict__ raw,
+                                           double* __restrict__ T, const double (*sWt)[PT], int tid) {
+  if (t.axis == 2) phase1_par<2, NS, NO, 0>(t.par, pr, t.nt, raw, T, sWt, tid);
+  else if (t.axis == 1) phase1_par<1, NS, NO, 0>(t.par, pr, t.nt, raw, T, sWt, tid);
+  else if (t.xoff) phase1_par<0, NS, NO, 1>(t.par, pr, t.nt, raw, T, sWt, tid);
+  else phase1_par<0, NS, NO, 0>(t.par, pr, t.nt, raw, T, sWt, tid);
 }
 
-// ---- phase 3: interpolation along A and the store ----------------------------------------------------
-// Everything that can be a compile-time constant is one (NT = thin cells, 0 = runtime; NO = planes' output
-// count; FULL = the tile has no ragged edge), so a plane costs 5 shared loads, 10 FMA and one store.
-// z- and y-slabs (A = x): thread (a-pair ja, fb) walks the planes; the two children are one 16-byte store.
-template <int AX, int NT, int NO, bool FULL>
-__device__ __forceinline__ void phase3(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
-                                       const double* __restrict__ U, int tid) {
-  static_assert(AX != 0, "x-slabs have their own phase 3");
+// ---- phase 2: the two transverse interpolations and the store, marching along B in registers ----------
+// children of the centre of a 5-value window held in registers
+__device__ __forceinline__ void children5(const double (&w)[5], double& lo, double& hi) {
+  constexpr double w0 = 35.0 / 2048.0, w1 = -252.0 / 2048.0, w2 = 1890.0 / 2048.0, w3 = 420.0 / 2048.0,
+                   w4 = -45.0 / 2048.0;
+  hi = fma(w4, w[4], fma(w1, w[1], w0 * w[0])) + fma(w3, w[3], w2 * w[2]);
+  lo = fma(w0, w[4], fma(w3, w[1], w4 * w[0])) + fma(w1, w[3], w2 * w[2]);
+}
+// z- and y-slabs (A = x): thread = (plane = (output, thin cell), parent column ja). It walks the PB parent rows of
+// its plane of T: each row is interpolated along A to the column's two children (5 shared loads, 10 FMA) and
+// pushed into a 5-row register window; once the window is full every new row yields two fine rows (20 FMA), each
+// stored as one 16-byte pair — 512 contiguous bytes per warp and store. Nothing goes back through shared memory.
+// The march is a rolled loop on purpose: unrolled, the phase is 12 KB of straight-line code per variant and the
+// kernel stalls on instruction fetch (measured: stall_no_inst 35-50 % of the samples).
+__device__ __forceinline__ void push_row(const double* __restrict__ p, double (&wl)[5], double (&wh)[5]) {
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { wl[i] = wl[i + 1]; wh[i] = wh[i + 1]; }
+  children(p, wl[4], wh[4]);
+}
+__device__ __forceinline__ void phase2(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
+                                       const double* __restrict__ T, int tid) {
   const BoxView& ch = a.child;
-  const int ja = tid % 16, fb = tid / 16, fa = 2 * ja;
-  bool v0 = true, v1 = true;
-  if (!FULL) {
-    v0 = fa >= t.vA0 && fa < t.vA1;
-    v1 = fa + 1 >= t.vA0 && fa + 1 < t.vA1;
-    if (fb < t.vB0 || fb >= t.vB1 || !(v0 || v1)) return;
-  }
-  const int nt = NT ? NT : t.nt;
-  const double* __restrict__ up = U + fb * PAMAX + ja + 2;
-  const long long csT = AX == 1 ? ch.px : ch.plane;
-  const long long cell = t.cell0 + fa + (long long)fb * (AX == 1 ? ch.plane : ch.px);
+  const int ja = tid & 15, pl = tid >> 4, nt = t.nt;
+  if (pl >= pr.nout * nt) return;
+  const int o = pl / nt, k = pl - o * nt, fa = 2 * ja;
+  const bool full = t.vA0 == 0 && t.vB0 == 0 && t.vB1 == TB && t.vA1 == TA;
+  const bool v0 = fa >= t.vA0 && fa < t.vA1, v1 = fa + 1 >= t.vA0 && fa + 1 < t.vA1;
+  if (!(v0 || v1)) return;
+  const long long csT = t.axis == 1 ? ch.px : ch.plane, csB = t.axis == 1 ? ch.plane : ch.px;
+  double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + t.cell0 + fa + k * csT;
+  const double* __restrict__ tp = T + pl * TPLANE + ja + 2;
+  double wl[5], wh[5];
 #pragma unroll
-  for (int o = 0; o < NO; ++o) {
-    if (o < pr.nout) {
-      double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + cell;
-#pragma unroll
-      for (int k = 0; k < (NT ? NT : 4); ++k)
-        if (k < nt) {
-          double lo, hi;
-          children(up + (o * nt + k) * (TB * PAMAX), lo, hi);
-          if (FULL || (v0 && v1)) *reinterpret_cast<double2*>(d + k * csT) = make_double2(lo, hi);
-          else if (v0) d[k * csT] = lo;
-          else d[k * csT + 1] = hi;
-        }
-    }
-  }
-}
-
-// x-slabs (thin = x, A = y): thread (fine row fa, fb) owns the g ghosts of one row and writes them as ONE
-// whole 32-byte sector when it can: with g = 3 the low ghosts sit at row positions 1..3 (position 0 is an
-// unused pad double), the high ghosts at XOFF+n .. XOFF+n+2 followed by a pad double when XOFF+n is a
-// multiple of 4 — no sector is written partially (t.sector, decided on the host).
-template <int NT, int NO>
-__device__ __forceinline__ void phase3x(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
-                                        const double* __restrict__ U, int tid) {
-  const BoxView& ch = a.child;
-  const int fa = tid % 16, fb = tid / 16;
-  if (fb < t.vB0 || fb >= t.vB1 || fa < t.vA0 || fa >= t.vA1) return;
-  const int nt = NT ? NT : t.nt;
-  const double* __restrict__ up = U + fb * PAMAX + (fa >> 1) + 2;
-  const bool odd = fa & 1;
-  const long long cell = t.cell0 + (long long)fa * ch.px + (long long)fb * ch.plane;
-#pragma unroll
-  for (int o = 0; o < NO; ++o) {
-    if (o < pr.nout) {
-      double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + cell;
-      double v[4];
-#pragma unroll
-      for (int k = 0; k < (NT ? NT : 4); ++k)
-        if (k < nt) {
-          double lo, hi;
-          children(up + (o * nt + k) * (TB * PAMAX), lo, hi);
-          v[k] = odd ? hi : lo;
-        }
-      if (NT == 3 && t.sector == 1) {
-        *reinterpret_cast<double2*>(d - 1) = make_double2(0.0, v[0]);
-        *reinterpret_cast<double2*>(d + 1) = make_double2(v[1], v[2]);
-      } else if (NT == 3 && t.sector == 2) {
-        *reinterpret_cast<double2*>(d) = make_double2(v[0], v[1]);
-        *reinterpret_cast<double2*>(d + 2) = make_double2(v[2], 0.0);
-      } else {
-#pragma unroll
-        for (int k = 0; k < (NT ? NT : 4); ++k)
-          if (k < nt) d[k] = v[k];
+  for (int i = 0; i < 5; ++i) wl[i] = wh[i] = 0.0;
+#pragma unroll 1
+  for (int jb = 0; jb < 4; ++jb, tp += PAMAX) push_row(tp, wl, wh);
+#pragma unroll 1
+  for (int fb = 0; fb < TB; fb += 2, tp += PAMAX, d += 2 * csB) {
+    push_row(tp, wl, wh);
+    double l0, l1, h0, h1;
+    children5(wl, l0, l1);  // fine rows fb (l0), fb + 1 (l1) of fine column fa
+    children5(wh, h0, h1);  // ... of fine column fa + 1
+    double* __restrict__ r1 = d + csB;
+    if (full) {
+      *reinterpret_cast<double2*>(d) = make_double2(l0, h0);
+      *reinterpret_cast<double2*>(r1) = make_double2(l1, h1);
+    } else {
+      if (fb >= t.vB0 && fb < t.vB1) {
+        if (v0 && v1) *reinterpret_cast<double2*>(d) = make_double2(l0, h0);
+        else if (v0) d[0] = l0;
+        else d[1] = h0;
+      }
+      if (fb + 1 >= t.vB0 && fb + 1 < t.vB1) {
+        if (v0 && v1) *reinterpret_cast<double2*>(r1) = make_double2(l1, h1);
+        else if (v0) r1[0] = l1;
+        else r1[1] = h1;
       }
     }
   }
 }
 
-template <int NT, int NO>
-__device__ __forceinline__ void phase3_any(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
-                                           const double* __restrict__ U, int tid) {
-  const bool full = t.vA0 == 0 && t.vB0 == 0 && t.vB1 == TB && t.vA1 == (t.axis == 0 ? Geo<0>::TA : Geo<2>::TA);
-  if (t.axis == 0) phase3x<NT, NO>(a, pr, t, f, U, tid);
-  else if (t.axis == 1) {
-    if (full) phase3<1, NT, NO, true>(a, pr, t, f, U, tid);
-    else phase3<1, NT, NO, false>(a, pr, t, f, U, tid);
-  } else {
-    if (full) phase3<2, NT, NO, true>(a, pr, t, f, U, tid);
-    else phase3<2, NT, NO, false>(a, pr, t, f, U, tid);
+// x-slabs (thin = x, A = y, B = z): thread = (output, parent column ja, lane kk of four); the four kk lanes of a
+// column are adjacent lanes of a warp and own the four doubles of the 32-byte sector that holds the g = 3
+// ghosts of a row plus one unused pad double (low side: pad first; high side: pad last, when XOFF + n is a
+// multiple of 4 — t.sector, decided on the host), so every store instruction writes whole sectors. The pad lane
+// computes nothing and stores 0. Other widths (t.sector = 0): lane kk stores thin cell kk.
+__device__ __forceinline__ void phase2x(const GhostArgs& a, const GhostProblem& pr, const GhostTile& t, int f,
+                                        const double* __restrict__ T, int tid) {
+  const BoxView& ch = a.child;
+  const int kk = tid & 3, ja = (tid >> 2) & 15, o = tid >> 6, nt = t.nt, fa = 2 * ja;
+  if (o >= pr.nout) return;
+  const int kt = kk - (t.sector == 1);  // thin cell of this lane
+  const bool comp = kt >= 0 && kt < nt;
+  if (!comp && t.sector == 0) return;
+  const bool v0 = fa >= t.vA0 && fa < t.vA1, v1 = fa + 1 >= t.vA0 && fa + 1 < t.vA1;
+  if (!(v0 || v1)) return;
+  double* __restrict__ d = a.child_base + (long long)(pr.dst_arr[o] + f) * ch.vol + t.cell0 + (long long)fa * ch.px + kt;
+  const double* __restrict__ tp = T + (o * nt + (comp ? kt : 0)) * TPLANE + ja + 2;
+  double wl[5], wh[5];
+#pragma unroll
+  for (int i = 0; i < 5; ++i) wl[i] = wh[i] = 0.0;
+  if (comp) {
+#pragma unroll 1
+    for (int jb = 0; jb < 4; ++jb, tp += PAMAX) push_row(tp, wl, wh);
+  }
+#pragma unroll 1
+  for (int fb = 0; fb < TB; fb += 2, tp += PAMAX, d += 2 * ch.plane) {
+    double l0 = 0.0, l1 = 0.0, h0 = 0.0, h1 = 0.0;
+    if (comp) {
+      push_row(tp, wl, wh);
+      children5(wl, l0, l1);  // fine z rows fb, fb + 1 of fine y row fa
+      children5(wh, h0, h1);  // ... of fine y row fa + 1
+    }
+    double* __restrict__ r1 = d + ch.plane;
+    if (fb >= t.vB0 && fb < t.vB1) {
+      if (v0) d[0] = l0;
+      if (v1) d[ch.px] = h0;
+    }
+    if (fb + 1 >= t.vB0 && fb + 1 < t.vB1) {
+      if (v0) r1[0] = l1;
+      if (v1) r1[ch.px] = h1;
+    }
   }
 }
 
 }  // namespace
 
 // ---- the kernel ----------------------------------------------------------------------------------------
-// dynamic shared memory: raw[GF_MAX_SRC][FOOTMAX] | T[GF_MAX_OUT * g][PB][PAMAX] | U[GF_MAX_OUT * g][TB][PAMAX]
+// dynamic shared memory (1024-byte aligned): raw[GF_MAX_SRC][FOOTMAX] | T[GF_MAX_OUT * g][TPLANE]
 __global__ void __launch_bounds__(NTHR, 2)
     ghost_fill_tma(const __grid_constant__ CUtensorMap mapx, const __grid_constant__ CUtensorMap mapy,
                    const __grid_constant__ CUtensorMap mapz, const __grid_constant__ GhostArgs a) {
@@ -283,11 +298,9 @@ __global__ void __launch_bounds__(NTHR, 2)
   __shared__ double sWt[4][PT];  // thin-axis weights (ghost widths other than 3): thin cell k <- footprint cell c
   __shared__ __align__(8) unsigned long long sbar;
   __shared__ __align__(16) GhostTile sTile[2];  // tile descriptors of the current and the next item
-  const uint32_t s0 = (smem_u32g(gsm_raw) + 127u) & ~127u;
+  const uint32_t s0 = (smem_u32g(gsm_raw) + 1023u) & ~1023u;
   double* const raw = reinterpret_cast<double*>(gsm_raw + (s0 - smem_u32g(gsm_raw)));
-  const int maxplanes = GF_MAX_OUT * a.child.g;
   double* const T = raw + GF_MAX_SRC * FOOTMAX;
-  double* const U = T + maxplanes * PB * PAMAX;
   const uint32_t bar = smem_u32g(&sbar);
   const int tid = threadIdx.x;
   const int per_prob = a.ntiles * a.F;
@@ -299,7 +312,7 @@ __global__ void __launch_bounds__(NTHR, 2)
     const int p = item / per_prob, f = (item - p * per_prob) / a.ntiles;
     const GhostProblem& pr = a.prob[p];
     const CUtensorMap* map = t.axis == 0 ? &mapx : (t.axis == 1 ? &mapy : &mapz);
-    const int foot = t.axis == 0 ? Geo<0>::FOOT : FOOTMAX;
+    const int foot = t.axis == 0 ? Geo<0>::FOOT : Geo<2>::FOOT;
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(pr.nsrc * foot * 8)
                  : "memory");
     for (int s = 0; s < pr.nsrc; ++s)
@@ -347,34 +360,18 @@ __global__ void __launch_bounds__(NTHR, 2)
       __syncthreads();
     }
     mbar_wait_g(bar, it & 1);
-    // phase 1 (the footprints have landed)
-    if (small) {
-      if (t.axis == 2) phase1_par<2, 2, 2>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
-      else if (t.axis == 1) phase1_par<1, 2, 2>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
-      else phase1_par<0, 2, 2>(t.par, pr, t.nt, t.xoff, raw, T, sWt, tid);
-    } else {
-      if (t.axis == 2) phase1_par<2, GF_MAX_SRC, GF_MAX_OUT>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
-      else if (t.axis == 1) phase1_par<1, GF_MAX_SRC, GF_MAX_OUT>(t.par, pr, t.nt, 0, raw, T, sWt, tid);
-      else phase1_par<0, GF_MAX_SRC, GF_MAX_OUT>(t.par, pr, t.nt, t.xoff, raw, T, sWt, tid);
-    }
+    // phase 1 (the footprints have landed); T planes are laid out per output (o * nt + k)
+    if (small) phase1_any<2, 2>(t, pr, raw, T, sWt, tid);
+    else phase1_any<GF_MAX_SRC, GF_MAX_OUT>(t, pr, raw, T, sWt, tid);
     if (tid >= 32 && tid < 36) asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();  // raw is free again, T is complete, the next descriptor is in sTile
     if (tid == 0 && more) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       issue(item + gridDim.x, sTile[(it + 1) & 1]);
     }
-    // planes are laid out for NO = 2 or 4 outputs (unused ones hold zeros)
-    const int nplanes = (small ? 2 : GF_MAX_OUT) * t.nt;
-    if (t.axis == 0) phase2<0>(nplanes, T, U, tid);
-    else phase2<2>(nplanes, T, U, tid);
-    __syncthreads();
-    if (t.nt == 3) {
-      if (small) phase3_any<3, 2>(a, pr, t, f, U, tid);
-      else phase3_any<3, GF_MAX_OUT>(a, pr, t, f, U, tid);
-    } else {
-      if (small) phase3_any<0, 2>(a, pr, t, f, U, tid);
-      else phase3_any<0, GF_MAX_OUT>(a, pr, t, f, U, tid);
-    }
+    if (t.axis == 0) phase2x(a, pr, t, f, T, tid);
+    else phase2(a, pr, t, f, T, tid);
+    __syncthreads();  // T may be overwritten by the next item's phase 1
   }
 }
 
@@ -438,7 +435,7 @@ void build_ghost_tiles(const BoxView& ch, const BoxView& pa, std::vector<GhostTi
     tiles.push_back(make_tile(ch, pa, ax, lo, n, org));
   };
   // z-slabs: A = x over the padded extent, B = y over the padded extent
-  cut(-g, ch.n[0] + g, Geo<2>::TA, ch.lo[0], 4, as);
+  cut(-g, ch.n[0] + g, TA, ch.lo[0], 4, as);
   cut(-g, ch.n[1] + g, TB, ch.lo[1], 2, bs);
   for (int hi = 0; hi < 2; ++hi)
     for (auto& b : bs)
@@ -455,7 +452,7 @@ void build_ghost_tiles(const BoxView& ch, const BoxView& pa, std::vector<GhostTi
         push(1, x.lo, y, b.lo, x.n, g, b.n, x.org, y, b.org);
       }
   // x-slabs: A = y interior, B = z interior
-  cut(0, ch.n[1], Geo<0>::TA, ch.lo[1], 2, as);
+  cut(0, ch.n[1], TA, ch.lo[1], 2, as);
   for (int hi = 0; hi < 2; ++hi)
     for (auto& b : bs)
       for (auto& y : as) {
@@ -465,8 +462,8 @@ void build_ghost_tiles(const BoxView& ch, const BoxView& pa, std::vector<GhostTi
 }
 
 void ghost_box_dims(int axis, unsigned box[4]) {
-  box[0] = axis == 0 ? PTX : Geo<2>::PA;
-  box[1] = axis == 0 ? Geo<0>::PA : (axis == 1 ? PT : PB);
+  box[0] = axis == 0 ? PTX : PA;
+  box[1] = axis == 0 ? PA : (axis == 1 ? PT : PB);
   box[2] = axis == 2 ? PT : PB;
   box[3] = 1;
 }
@@ -490,7 +487,7 @@ void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st) {
     return n > 0 ? n : 148;
   }();
   const int maxplanes = GF_MAX_OUT * a.child.g;
-  const size_t smem = 128 + sizeof(double) * ((size_t)GF_MAX_SRC * FOOTMAX + (size_t)maxplanes * (PB * PAMAX + TB * PAMAX));
+  const size_t smem = 1024 + sizeof(double) * ((size_t)GF_MAX_SRC * FOOTMAX + (size_t)maxplanes * TPLANE);
   static size_t configured = 0;
   if (smem > configured) {
     cudaFuncSetAttribute(ghost_fill_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -444,7 +444,7 @@ int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes)
 void stage_box_dims(unsigned box[4]) { box[0] = HX; box[1] = HY; box[2] = 1; box[3] = 1; }
 
 bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned bx[4], int l2_promotion,
-                             void* out_map128) {
+                             bool swizzle64, void* out_map128) {
   EncodeTiledFn enc = encode_tiled();
   if (!enc) return false;
   if (b.px > (1 << 30) || (reinterpret_cast<uintptr_t>(base) & 15)) return false;
@@ -454,7 +454,8 @@ bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const un
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   CUtensorMap m;
   const CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
                          l2_promotion == 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
                                              : (l2_promotion == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
                                                                     : CU_TENSOR_MAP_L2_PROMOTION_NONE),
