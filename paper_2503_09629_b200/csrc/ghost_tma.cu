@@ -116,8 +116,8 @@ __device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, const dou
   for (int o = 0; o < NO; ++o)
 #pragma unroll
     for (int k = 0; k < 4; ++k) acc[o][k] = 0.0;
-#pragma unroll
-  for (int s = 0; s < NS; ++s) {
+#pragma unroll 1
+  for (int s = 0; s < NS; ++s) {  // rolled: the kernel is sensitive to instruction fetch (see phase 2)
     double L[PT];
     if (AX == 0) {  // row tid of the (PTX x, PA y, PB z) box; chunk q sits at q ^ bits 1-2 of the row (SWIZZLE_64B)
       const double2* __restrict__ row = reinterpret_cast<const double2*>(raw + s * FOOTMAX) + tid * 4;
@@ -154,7 +154,8 @@ __device__ __forceinline__ void phase1(const GhostProblem& pr, int nt, const dou
 #pragma unroll
     for (int o = 0; o < NO; ++o) {
       const double cf = pr.coef[o][s];
-      if (cf != 0.0) {
+      // small shape: a slot beyond nsrc holds stale data (possibly NaN) and has coefficient 0 -> skip it
+      if (NS == GF_MAX_SRC || cf != 0.0) {
 #pragma unroll
         for (int k = 0; k < (PAR >= 0 ? 3 : 4); ++k) acc[o][k] = fma(cf, v[k], acc[o][k]);
       }
