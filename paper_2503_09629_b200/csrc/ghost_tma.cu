@@ -4,11 +4,11 @@
 //   child array dst_arr[o](ghost cell) = P[ sum_s coef[o][s] * parent array src_arr[s] ],   P = 5x5x5 quartic Lagrange
 //
 // The ghost shell of a box is the union of six slabs (z-lo, z-hi, y-lo, y-hi, x-lo, x-hi); each slab is cut
-// into tiles  g (thin axis) x TA x TB  fine cells (32 x 16 for z- and y-slabs, 16 x 16 for x-slabs) whose
-// origin is even in every axis, so a tile covers whole parent cells and its parent footprint is exactly
-// (TA/2+4) x (TB/2+4) x 6 cells. The host precomputes one 64-byte descriptor per tile (index maps, TMA
-// coordinates, ragged-edge ranges, store mode). A work ITEM is (problem, field, tile). Persistent CTAs (two
-// per SM) walk the item list; per item
+// into tiles  g (thin axis) x 32 (A) x 16 (B)  fine cells whose origin is even in every axis, so a tile covers
+// whole parent cells and its parent footprint is exactly 20 x 12 x 6 cells (x-slabs: rows of 8, see below). The
+// host precomputes one 64-byte descriptor per tile (index maps, TMA coordinates, ragged-edge ranges, store
+// mode). A work ITEM is (problem, field, tile). Persistent CTAs (two per SM, equal item counts) walk the item
+// list; per item
 //   0. the footprint of every source array arrives in shared memory through ONE TMA tiled load per source
 //      (cp.async.bulk.tensor.4d on the parent's footprint tensor map, out-of-range cells zero-filled),
 //      requested one item AHEAD so it flies while the current item is interpolated; the descriptor of the
@@ -16,15 +16,23 @@
 //   1. one thread per parent column: thin-axis interpolation (6 parent cells -> g fine cells; for g = 3 the
 //      weights are compile-time constants chosen by the parity of the first thin cell) of every source,
 //      then the time combination into the outputs             -> T[plane = (o, thin cell)][b][a]
-//   2. interpolation along b, register-blocked: one thread per (plane, a)  -> U[plane][fb][a]
-//   3. interpolation along a and the store: thread (a-pair, fb) walks the planes; for z- and y-slabs a = x
-//      and the pair is one 16-byte store, coalesced across the warp; for x-slabs (thin = x) a thread owns
-//      the g ghosts of one row and writes them as ONE whole 32-byte sector (plus an unused pad double).
+//   2. both transverse interpolations and the store in ONE pass that never returns to shared memory: thread
+//      (plane, parent column) marches along b; each T row is interpolated along a to the column's two children
+//      and pushed into a 5-row register window, from which every step produces two fine rows. z- and y-slabs
+//      (a = x): a row pair is one 16-byte store, 512 contiguous bytes per warp. x-slabs (thin = x): the four
+//      lanes (3 ghosts + 1 pad double) of a row are adjacent lanes and write ONE whole 32-byte sector.
 // A ghost value costs 6 + 5 + 5 FMA instead of 125 and every parent value is fetched once per tile.
-// Measured (r01, profiles/): the kernel is bound by the footprint loads — isolated 64-160-byte rows, 72-144
-// per source box: 2-13k cycles from request to arrival, growing with the number of boxes in flight on the
-// GPU; replacing TMA by per-thread 16-byte cp.async, prefetching two items ahead into L2, or removing the
-// index arithmetic from the phases each left the launch time within 10 %.
+// Measured (r01, profiles/r01_v4.md): 256^3 child box, (5 -> 4) problem 25 us, with the (2 -> 2) problem 38 us
+// (v3 with separate b- and a-passes through shared memory: 31 / 42 us). What the profiles showed on the way:
+//   * an empty launch of this grid already costs 6 us between its two events;
+//   * the kernel is sensitive to instruction fetch: with phase 2's 12-step march unrolled (12 KB of straight-
+//     line code per variant) 35-50 % of the stall samples were stall_no_inst and the launch took 44 us; rolled
+//     (20 register moves per step) 40 us; with phase 1's source loop rolled as well 35.6 us; a 5-way unrolled
+//     rotating window without moves was slower again (43.7 us);
+//   * the x-slab footprint rows (64 B each) are read by one thread per row: unswizzled that is a 16-way bank
+//     conflict (2.7 M conflict wavefronts per launch), hence the SWIZZLE_64B tensor map;
+//   * doubling the CTA to 512 threads (half the outputs per thread) and programmatic dependent launch of the
+//     whole kernel chain both made the step slower (48.8 us per launch; 22.0 -> 22.8 ms per coarse step).
 #include <cuda.h>
 
 #include <cstdlib>
@@ -497,7 +505,9 @@ void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st) {
   const long long nitems = (long long)a.nprob * a.ntiles * a.F;
   const int per_sm = smem <= 112 * 1024 ? 2 : 1;
   const long long want = (long long)nsm * per_sm;
-  const unsigned grid = (unsigned)(nitems < want ? nitems : want);
+  // equal item counts per CTA: with R = ceil(nitems / want) rounds, ceil(nitems / R) CTAs all do R items (+-1)
+  const long long rounds = (nitems + want - 1) / want;
+  const unsigned grid = (unsigned)(nitems <= want ? nitems : (nitems + rounds - 1) / rounds);
   const CUtensorMap* m = static_cast<const CUtensorMap*>(a.tmaps);
   ghost_fill_tma<<<grid, NTHR, smem, st>>>(m[0], m[1], m[2], a);
 }
