@@ -29,6 +29,7 @@
 // composite step on data the operators do NOT reproduce exactly; there the oracle is the definition and the
 // convergence ladder bounds it.
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
@@ -338,6 +339,35 @@ void restrict_to_parent(const Hier& H, const BoxData& child, BoxData& par) {
   }
 }
 
+// Same-level ghost exchange (NEXT-2; the ghost zones at a refinement boundary are the same
+// zones an inter-process boundary uses). Boxes of one level may abut or sit closer than a ghost width: every
+// ghost cell of a box that lies in the INTERIOR of a sibling box takes the sibling's value of the same array
+// (the same stage vector at the same time), replacing whatever the refinement-boundary fill wrote there. A
+// level cut into abutting boxes therefore computes exactly what the uncut level computes.
+void sibling_exchange(Hier& H, int level, std::vector<Field> BoxData::*which) {
+  const int g = H.g;
+  for (int ia : H.level_boxes[level])
+    for (int ib : H.level_boxes[level]) {
+      if (ia == ib) continue;
+      BoxData& A = H.boxes[ia];
+      const BoxData& B = H.boxes[ib];
+      int lo[3], hi[3];  // level-global index range of  padded(A) n interior(B)
+      bool empty = false;
+      for (int a = 0; a < 3; ++a) {
+        lo[a] = std::max(A.lo[a] - g, B.lo[a]);
+        hi[a] = std::min(A.lo[a] + A.n[a] + g, B.lo[a] + B.n[a]);
+        if (hi[a] <= lo[a]) empty = true;
+      }
+      if (empty) continue;
+      for (size_t c = 0; c < (A.*which).size(); ++c)
+        for (int k = lo[2]; k < hi[2]; ++k)
+          for (int j = lo[1]; j < hi[1]; ++j)
+            for (int i = lo[0]; i < hi[0]; ++i)
+              (A.*which)[c].at(i - A.lo[0], j - A.lo[1], k - A.lo[2]) =
+                  (B.*which)[c].at(i - B.lo[0], j - B.lo[1], k - B.lo[2]);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // time stepping
 // ---------------------------------------------------------------------------------------------
@@ -357,6 +387,7 @@ void fill(Hier& H, int level, std::vector<Field> BoxData::*which, int stage, dou
     if (level == 0) periodic_fill(b, b.*which);
     else dense_ghost_fill(H, b, H.boxes[b.parent], b.*which, stage, theta, 2.0 * dt);
   }
+  sibling_exchange(H, level, which);
 }
 
 // One RK4 step of all boxes of one level (eqs 1-9), ghosts by fill(); theta = where this step starts
@@ -413,6 +444,7 @@ void same_time_fill(Hier& H, int level, std::vector<Field> BoxData::*which) {
     const BoxData& par = H.boxes[b.parent];
     for (int c = 0; c < 2 * H.F; ++c) prolong_into_ghosts(b, par, (par.*which)[c], (b.*which)[c]);
   }
+  sibling_exchange(H, level, which);
 }
 
 void uniform_step(Hier& H, double dt) {
@@ -472,10 +504,10 @@ bool validate(Hier& H, char* msg, size_t cap) {
       for (int jb : H.level_boxes[l]) {
         if (jb == ib) continue;
         const BoxData& o = H.boxes[jb];
-        bool apart = false;
+        bool disjoint = false;  // interiors must not overlap; any distance (abutting included) is fine
         for (int a = 0; a < 3; ++a)
-          if (b.lo[a] >= o.lo[a] + o.n[a] + 2 * margin || o.lo[a] >= b.lo[a] + b.n[a] + 2 * margin) apart = true;
-        if (!apart) return fail("sibling boxes too close");
+          if (b.lo[a] >= o.lo[a] + o.n[a] || o.lo[a] >= b.lo[a] + b.n[a]) disjoint = true;
+        if (!disjoint) return fail("sibling boxes overlap");
       }
     }
   }
