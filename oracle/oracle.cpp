@@ -13,6 +13,8 @@
 //   ghost stage vectors, eqs (15)-(18) ..... PAPER.md:98-109    -> dense_stage()
 //   recursion, steps 1-7 ................... PAPER.md:111-119   -> advance()
 //   wave system, eqs (39)-(40) ............. PAPER.md:222-226   -> rhs()
+//   Kreiss-Oliger dissipation, eqs (35)-(36) PAPER.md:194-204   -> add_dissipation()
+//   same-level ghost exchange .............. PAPER.md:20, 347   -> sibling_exchange()
 //
 // Where the paper is silent the readings S1..S24 of DESIGN.md apply (cell-centred grids S1, 4th-order
 // centred Laplacian S2, quartic Lagrange prolongation S3, quintic Lagrange restriction S4, parent-step
@@ -25,7 +27,9 @@
 // plane-wave convergence ladder (order ~4); subcycled-vs-uniform agreement; linearity; and the COMPOSITE
 // multi-level step (dense-output fills at theta = 0 and 1/2, stage formulas, restrictions, both modes) against
 // the exact solution u = r^2 + 3 t^2, rho = 6 t, which every operator reproduces to rounding
-// (test_composite_scheme_exact_for_quadratic_solution). What stays unpinned at bit level is only the
+// (test_composite_scheme_exact_for_quadratic_solution); the same-level ghost exchange by decomposition
+// invariance (a level cut into abutting boxes reproduces the uncut level bit for bit) and the same exact
+// solution through abutting / edge-touching / near siblings (tests/test_oracle_siblings.py). What stays unpinned at bit level is only the
 // composite step on data the operators do NOT reproduce exactly; there the oracle is the definition and the
 // convergence ladder bounds it.
 
