@@ -52,7 +52,11 @@ typedef struct {
  *   - every level >= 1 box: lo and n even on every axis (it covers whole parent cells), n >= 8;
  *     it lies inside ONE box of level-1 with at least 4 parent cells of margin to that box's
  *     interior edge (reading S13: the 5-point prolongation footprint never touches parent ghosts);
- *   - boxes of one level are disjoint and at least 4 parent cells (8 own cells) apart.
+ *   - the interiors of the boxes of one level are disjoint. Boxes may abut or sit at any distance: every ghost
+ *     cell of a box that lies in the interior of a box of the same level takes that box's value of the same
+ *     stage vector (same-level ghost exchange after every fill and stage; a refinement
+ *     boundary uses the same ghost zones as an inter-process boundary), so a level cut into abutting boxes
+ *     computes what the uncut level computes. A child box must still nest in ONE parent box.
  * The state has nfields second-order fields u_f with first-order partners rho_f = d_t u_f:
  *   component index comp = f        -> u_f
  *                   comp = nfields+f -> rho_f            (V = 2*nfields arrays per box)

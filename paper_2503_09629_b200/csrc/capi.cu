@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <algorithm>
 #include <cstring>
 #include <map>
 #include <string>
@@ -68,6 +69,8 @@ struct sc_hierarchy {
   std::vector<char> gmap_ok;
   std::vector<TMap> kmaps;        // per box: halo-3 tile of the dissipative stage kernel (ko_sigma > 0)
   std::vector<char> kmap_ok;
+  struct LevelSiblings { SiblingPair* dev = nullptr; int n = 0; long long maxcells = 0; double cells = 0.0; };
+  std::vector<LevelSiblings> sib; // per level: ordered pairs of boxes that exchange ghosts (kernels.h a7)
   // per-launch CUDA-event timing (sc_profile): eager launches, one event pair per kernel
   bool profiling = false;
   struct ProfRec { int kind; double bytes; cudaEvent_t e0, e1; };
@@ -219,6 +222,20 @@ void periodic_level0(Seq& q, int first_array, int narrays) {
   const BoxView& v = h->L.boxes[ib].v;
   prof_begin(h, KIND_PERIODIC, 16.0 * narrays * shell_cells(v));
   launch_periodic_fill(v, narrays, h->arr(ib, first_array), h->stream);
+  prof_end(h);
+  ++q.n;
+}
+
+// Same-level ghost exchange of arrays [first_array, first_array + narrays) between the boxes of `level`
+// (kernels.h a7). Called after every refinement-boundary fill and after every kernel that produced a
+// stage vector, for exactly the arrays written: a ghost cell inside a sibling's interior ends up with the
+// sibling's value of the same stage vector, as on an uncut level. No launch when no two boxes are in reach.
+void sibling_level(Seq& q, int level, int first_array, int narrays) {
+  sc_hierarchy* h = q.h;
+  const sc_hierarchy::LevelSiblings& s = h->sib[level];
+  if (s.n == 0) return;
+  prof_begin(h, KIND_PERIODIC, 16.0 * narrays * s.cells);
+  launch_sibling_copy(s.dev, s.n, s.maxcells, reinterpret_cast<double*>(h->arena), first_array, narrays, h->stream);
   prof_end(h);
   ++q.n;
 }
@@ -446,12 +463,18 @@ void level_step_ko(Seq& q, int level, double dt, double theta) {
     if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
   } else {
     fill_level_dense_ko(q, level, theta, dt);
+    sibling_level(q, level, L.a_state(yn), L.V);
   }
   for (int s = 1; s <= 4; ++s) {
     stage_ko_level(q, level, s, dt);
     if (level == 0) {
       if (s < 4) periodic_stage_ko(q, s + 1);
       else periodic_level0(q, L.a_state(1 - yn), L.V);
+    } else if (s < 4) {  // the stage vector just produced: ghosts inside a sibling take the sibling's Y_{s+1}
+      sibling_level(q, level, L.a_U(s + 1), L.F);
+      sibling_level(q, level, L.a_R(s + 1), L.F);
+    } else {
+      sibling_level(q, level, L.a_state(1 - yn), L.V);
     }
   }
   if (level == 0) q.l0_valid = true;
@@ -467,13 +490,18 @@ void uniform_step_ko(Seq& q, double dt) {
     const int ca[2] = {L.a_state(q.cur[l]), L.a_state(q.cur[l]) + F};
     const int pa[2] = {L.a_state(q.cur[l - 1]), L.a_state(q.cur[l - 1]) + F};
     fill_level_same_time(q, l, 2, ca, pa);
+    sibling_level(q, l, ca[0], L.V);
   }
   for (int s = 1; s <= 4; ++s) {
     for (int l = 0; l < Lv; ++l) stage_ko_level(q, l, s, dt);
     if (s < 4) {
       periodic_stage_ko(q, s + 1);
       const int ca[2] = {L.a_U(s + 1), L.a_R(s + 1)};
-      for (int l = 1; l < Lv; ++l) fill_level_same_time(q, l, 2, ca, ca);
+      for (int l = 1; l < Lv; ++l) {
+        fill_level_same_time(q, l, 2, ca, ca);
+        sibling_level(q, l, ca[0], F);
+        sibling_level(q, l, ca[1], F);
+      }
     }
   }
   periodic_level0(q, L.a_state(1 - q.cur[0]), L.V);
@@ -482,6 +510,7 @@ void uniform_step_ko(Seq& q, double dt) {
     const int ca[2] = {L.a_state(1 - q.cur[l]), L.a_state(1 - q.cur[l]) + F};
     const int pa[2] = {L.a_state(1 - q.cur[l - 1]), L.a_state(1 - q.cur[l - 1]) + F};
     fill_level_same_time(q, l, 2, ca, pa);
+    sibling_level(q, l, ca[0], L.V);
   }
   for (int l = 0; l < Lv; ++l) q.cur[l] = 1 - q.cur[l];
   for (int l = Lv - 1; l >= 1; --l) restrict_level(q, l);
@@ -496,13 +525,17 @@ void level_step(Seq& q, int level, double dt, double theta) {
     if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
   } else {
     fill_level_dense(q, level, theta, dt);
+    sibling_level(q, level, L.a_state(yn), L.V);  // u_n, rho_n: on a sibling's interior u_n + a_1 dt rho_n IS Y_{2,u}
   }
   stage_level(q, level, STAGE_12, dt);
   if (level == 0) periodic_level0(q, L.a_Y2r(), 2 * L.F);  // Y2r and Y3r are adjacent
+  else sibling_level(q, level, L.a_Y2r(), 2 * L.F);
   stage_level(q, level, STAGE_34, dt);
   if (level == 0) {
     periodic_level0(q, L.a_state(1 - yn), L.V);
     q.l0_valid = true;
+  } else {
+    sibling_level(q, level, L.a_state(1 - yn), L.V);  // y_{n+1}: read by the restriction and sc_debug_read_padded
   }
   q.cur[level] = 1 - yn;
 }
@@ -528,6 +561,7 @@ void uniform_step(Seq& q, double dt) {
     const int ca[2] = {L.a_state(q.cur[l]), L.a_state(q.cur[l]) + F};
     const int pa[2] = {L.a_state(q.cur[l - 1]), L.a_state(q.cur[l - 1]) + F};
     fill_level_same_time(q, l, 2, ca, pa);
+    sibling_level(q, l, ca[0], L.V);
   }
   for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_12, dt);
   // ghosts of Y_{3,u}, Y_{4,u} = P[parent's Y_{3,u}, Y_{4,u}]  <=>  shells of Y2r, Y3r = P[parent's Y2r, Y3r]
@@ -535,6 +569,7 @@ void uniform_step(Seq& q, double dt) {
   for (int l = 1; l < Lv; ++l) {
     const int ca[2] = {L.a_Y2r(), L.a_Y3r()};
     fill_level_same_time(q, l, 2, ca, ca);
+    sibling_level(q, l, ca[0], 2 * F);
   }
   for (int l = 0; l < Lv; ++l) stage_level(q, l, STAGE_34, dt);
   // ghosts of y_{n+1} from the parent's y_{n+1} before the restriction
@@ -544,6 +579,7 @@ void uniform_step(Seq& q, double dt) {
     const int ca[2] = {L.a_state(1 - q.cur[l]), L.a_state(1 - q.cur[l]) + F};
     const int pa[2] = {L.a_state(1 - q.cur[l - 1]), L.a_state(1 - q.cur[l - 1]) + F};
     fill_level_same_time(q, l, 2, ca, pa);
+    sibling_level(q, l, ca[0], L.V);
   }
   for (int l = 0; l < Lv; ++l) q.cur[l] = 1 - q.cur[l];
   for (int l = Lv - 1; l >= 1; --l) restrict_level(q, l);
@@ -653,6 +689,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     set_error(std::string(what) + ": " + cudaGetErrorString(e));
     if (h->staging) cudaFree(h->staging);
     for (auto& bt : h->tiles) if (bt.dev) cudaFree(bt.dev);
+    for (auto& s : h->sib) if (s.dev) cudaFree(s.dev);
     if (h->own_arena) cudaFree(h->arena);
     if (h->own_stream) cudaStreamDestroy(h->stream);
     delete h;
@@ -676,6 +713,38 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     if ((ce = cudaMalloc(&bt.dev, sizeof(GhostTile) * tl.size())) != cudaSuccess) return bail("cudaMalloc(tiles)", ce);
     if ((ce = cudaMemcpy(bt.dev, tl.data(), sizeof(GhostTile) * tl.size(), cudaMemcpyHostToDevice)) != cudaSuccess)
       return bail("copy tiles", ce);
+  }
+  h->sib.assign(h->L.nlevels, {});
+  for (int l = 1; l < h->L.nlevels; ++l) {
+    std::vector<SiblingPair> pr;
+    sc_hierarchy::LevelSiblings& s = h->sib[l];
+    for (int ia : h->L.level_boxes[l])
+      for (int ib : h->L.level_boxes[l]) {
+        if (ia == ib) continue;
+        const BoxInfo &A = h->L.boxes[ia], &B = h->L.boxes[ib];
+        SiblingPair p{};
+        long long nc = 1;
+        for (int a = 0; a < 3; ++a) {  // padded(A) n interior(B), level-global indices
+          const int lo = std::max(A.v.lo[a] - A.v.g, B.v.lo[a]);
+          const int hi = std::min(A.v.lo[a] + A.v.n[a] + A.v.g, B.v.lo[a] + B.v.n[a]);
+          p.lo[a] = lo;
+          p.n[a] = hi - lo;
+          nc *= hi > lo ? hi - lo : 0;
+        }
+        if (nc == 0) continue;
+        p.dst = A.v;
+        p.src = B.v;
+        p.dst_off = (long long)(A.arena_offset / sizeof(double));
+        p.src_off = (long long)(B.arena_offset / sizeof(double));
+        pr.push_back(p);
+        s.maxcells = std::max(s.maxcells, nc);
+        s.cells += (double)nc;
+      }
+    s.n = (int)pr.size();
+    if (pr.empty()) continue;
+    if ((ce = cudaMalloc(&s.dev, sizeof(SiblingPair) * pr.size())) != cudaSuccess) return bail("cudaMalloc(sibling pairs)", ce);
+    if ((ce = cudaMemcpy(s.dev, pr.data(), sizeof(SiblingPair) * pr.size(), cudaMemcpyHostToDevice)) != cudaSuccess)
+      return bail("copy sibling pairs", ce);
   }
   h->tmaps.resize(h->L.boxes.size());
   h->tmap_ok.assign(h->L.boxes.size(), 0);
@@ -866,6 +935,7 @@ int32_t sc_destroy(sc_hierarchy* h) {
     if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
   if (h->staging) cudaFree(h->staging);
   for (auto& bt : h->tiles) if (bt.dev) cudaFree(bt.dev);
+  for (auto& s : h->sib) if (s.dev) cudaFree(s.dev);
   if (h->own_arena && h->arena) cudaFree(h->arena);
   if (h->own_stream) cudaStreamDestroy(h->stream);
   delete h;

@@ -115,11 +115,10 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
       for (int jb : L->level_boxes[l]) {
         if (jb == ib) continue;
         const BoxInfo& o = L->boxes[jb];
-        bool apart = false;
+        bool disjoint = false;  // any distance is fine (abutting boxes exchange ghosts, kernels.h a7)
         for (int a = 0; a < 3; ++a)
-          if (b.v.lo[a] >= o.v.lo[a] + o.v.n[a] + 2 * margin || o.v.lo[a] >= b.v.lo[a] + b.v.n[a] + 2 * margin)
-            apart = true;
-        if (!apart) return fail(err, SC_ERR_NESTING, "boxes %d and %d overlap or are closer than %d parent cells", ib, jb, margin);
+          if (b.v.lo[a] >= o.v.lo[a] + o.v.n[a] || o.v.lo[a] >= b.v.lo[a] + b.v.n[a]) disjoint = true;
+        if (!disjoint) return fail(err, SC_ERR_NESTING, "boxes %d and %d overlap", ib, jb);
       }
     }
   }

@@ -142,6 +142,19 @@ struct RestrictArgs {
 };
 void launch_restrict(const RestrictArgs& a, cudaStream_t st);
 
+// a7: same-level ghost exchange. Boxes of one level may abut or sit closer
+// than a ghost width; every ghost cell of a box that lies in the INTERIOR of a sibling takes the sibling's value
+// of the same array, after the refinement-boundary fill wrote its (prolonged) value there. One record per
+// ordered pair (dst, src) whose  padded(dst) n interior(src)  is not empty; the region is a box.
+struct SiblingPair {
+  BoxView dst, src;
+  long long dst_off, src_off;  // doubles from the arena base to array 0 of the two boxes
+  int lo[3], n[3];             // the region: first cell (level-global index) and extent
+};
+// copies arrays [first_array, first_array + narrays) of every pair; `maxcells` = largest region
+void launch_sibling_copy(const SiblingPair* pairs_dev, int npairs, long long maxcells, double* arena, int first_array,
+                         int narrays, cudaStream_t st);
+
 // interior-only <-> padded copies for sc_set_state / sc_read_level (device src/dst, dense [k][j][i])
 void launch_pack(const BoxView& b, const double* padded, double* dense, int with_ghosts, cudaStream_t st);
 void launch_unpack(const BoxView& b, const double* dense, double* padded, cudaStream_t st);

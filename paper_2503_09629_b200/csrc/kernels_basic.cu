@@ -216,6 +216,28 @@ void launch_periodic_fill(const BoxView& b, int V, double* y, cudaStream_t st) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// a7  same-level ghost exchange: one thread per cell of the region  padded(dst) n interior(src)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) sibling_copy(const SiblingPair* __restrict__ pairs, double* __restrict__ arena,
+                                                    int first_array) {
+  const SiblingPair& p = pairs[blockIdx.y];
+  const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (long long)p.n[0] * p.n[1] * p.n[2]) return;
+  const int i = p.lo[0] + (int)(q % p.n[0]), j = p.lo[1] + (int)((q / p.n[0]) % p.n[1]),
+            k = p.lo[2] + (int)(q / ((long long)p.n[0] * p.n[1]));
+  const int arr = first_array + blockIdx.z;
+  arena[p.dst_off + (long long)arr * p.dst.vol + cell_offset(p.dst, i - p.dst.lo[0], j - p.dst.lo[1], k - p.dst.lo[2])] =
+      arena[p.src_off + (long long)arr * p.src.vol + cell_offset(p.src, i - p.src.lo[0], j - p.src.lo[1], k - p.src.lo[2])];
+}
+
+void launch_sibling_copy(const SiblingPair* pairs_dev, int npairs, long long maxcells, double* arena, int first_array,
+                         int narrays, cudaStream_t st) {
+  if (npairs <= 0 || narrays <= 0 || maxcells <= 0) return;
+  dim3 grd((unsigned)((maxcells + 127) / 128), npairs, narrays);
+  sibling_copy<<<grd, 128, 0, st>>>(pairs_dev, arena, first_array);
+}
+
+// ------------------------------------------------------------------------------------------------
 // a5  restriction, one thread per parent cell, 216-point gather
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) restrict_ref(BoxView ch, BoxView pa, const double* yc, double* yp) {

@@ -297,3 +297,40 @@ def ragged_small() -> Workload:
                     nfields=2, coupling=coupling_matrix(2), coarse_steps=2,
                     xlo=(-1.0, -0.6, -0.7), xhi=(1.0, 0.6, 0.7),
                     init=multi_gaussian_init(3))
+
+
+def global_index_init(w: Workload, level: int, ibox: int, comp: int) -> np.ndarray:
+    """Smooth pulse + a ripple that depends on the LEVEL-GLOBAL cell index only: every decomposition of a level
+    into boxes gets the same numbers (test data of the same-level ghost exchange)."""
+    b = w.box(level, ibox)
+    x, y, z = w.centres(level, ibox)
+    i, j, k = (np.arange(b.lo[a], b.lo[a] + b.n[a], dtype=np.float64) for a in range(3))
+    r2 = z[:, None, None] ** 2 + y[None, :, None] ** 2 + (x[None, None, :] - 0.1) ** 2
+    rip = np.sin(12.9898 * i[None, None, :] + 78.233 * j[None, :, None] + 37.719 * k[:, None, None] + comp + level)
+    amp = 1.0 if comp < w.nfields else 0.3
+    return amp * np.exp(-r2 / 0.1) + 1e-3 * rip
+
+
+def sibling_cut(cuts_x=(), cuts_y=(), cuts_z=(), nfields: int = 1, ko_sigma: float = 0.0,
+                near: bool = False) -> Workload:
+    """Test-only: 3 levels; level 1 = the region [12, 36)^3 of a 24^3 level 0, cut into abutting boxes at the given
+    level-global indices (no cuts = one box); level 2 = one 8x12x16 box that nests in a piece of every cut with
+    x in {24}, y in {20, 22}, z in {20}. `near` adds a level-1 box two cells away from the cut region (only part
+    of its ghost shell lies inside a sibling)."""
+    lo, n = 12, 24
+
+    def segs(cuts):
+        e = [lo] + list(cuts) + [lo + n]
+        return list(zip(e[:-1], e[1:]))
+    boxes = [Box(0, (0, 0, 0), (32, 24, 24))]
+    for z0, z1 in segs(cuts_z):
+        for y0, y1 in segs(cuts_y):
+            for x0, x1 in segs(cuts_x):
+                boxes.append(Box(1, (x0, y0, z0), (x1 - x0, y1 - y0, z1 - z0)))
+    if near:
+        boxes.append(Box(1, (38, 14, 16), (14, 18, 12)))
+    boxes.append(Box(2, (56, 52, 48), (8, 12, 16)))
+    return Workload("siblings: level 1 cut into %d boxes" % (len(boxes) - 2), boxes, (32, 24, 24), nfields=nfields,
+                    coupling=coupling_matrix(nfields) if nfields > 1 else None, coarse_steps=2,
+                    xlo=(-4.0 / 3.0, -1.0, -1.0), xhi=(4.0 / 3.0, 1.0, 1.0),
+                    init=global_index_init, ko_sigma=ko_sigma)

@@ -322,3 +322,71 @@ def test_ko_needs_three_ghost_layers():
     w.ko_sigma = 0.1
     with pytest.raises(sc.SubcycleError):
         sc.Hierarchy.from_workload(w)
+
+
+# ---- NEXT-2: same-level ghost exchange between sibling boxes (kernels.h a7) -------------------------------------
+SIB_CUTS = {"x halves": ((24,), (), ()), "z 8+16": ((), (), (20,)), "quarters + near box": ((24,), (22,), ()),
+            "eight boxes": ((24,), (20,), (20,))}
+
+
+@pytest.mark.parametrize("sigma", [0.0, 0.2])
+@pytest.mark.parametrize("sub", [True, False])
+def test_sibling_exchange_parity(sub, sigma):
+    """Abutting, edge-touching and near (2 cells apart) level-1 boxes, 2 coupled fields: CUDA path vs oracle,
+    ghosts included (a ghost cell inside a sibling holds the sibling's value)."""
+    for name, (cx, cy, cz) in SIB_CUTS.items():
+        w = wl.sibling_cut(cx, cy, cz, nfields=2, ko_sigma=sigma, near="near" in name)
+        G, O = _pair(w)
+        for _ in range(w.coarse_steps):
+            G.sc_step(w.dt_coarse, sub)
+            O.step(w.dt_coarse, sub)
+        _compare_state(G, O, w, what=f"siblings {name} sub={sub} sigma={sigma}")
+        G.close()
+
+
+@pytest.mark.parametrize("sigma", [0.0, 0.2])
+@pytest.mark.parametrize("sub", [True, False])
+def test_cut_level_reproduces_the_uncut_level_on_the_gpu(sub, sigma):
+    """Decomposition invariance without the oracle: a cell update reads the same numbers whether its neighbour
+    lives in the same box or arrives through the exchange, so the cut level must match the uncut one to rounding
+    (not bit for bit: the z-march accumulates the stencil's z terms in march order, which depends on where a
+    cell sits in its box's z-chunks)."""
+    def run(cuts):
+        w = wl.sibling_cut(*cuts, ko_sigma=sigma)
+        G = sc.Hierarchy.from_workload(w)
+        for _ in range(3):
+            G.sc_step(w.dt_coarse, sub)
+        l1 = np.full((24, 24, 24), np.nan)
+        for ib, b in enumerate(w.level_boxes(1)):
+            o = [b.lo[a] - 12 for a in range(3)]
+            l1[o[2]:o[2] + b.n[2], o[1]:o[1] + b.n[1], o[0]:o[0] + b.n[0]] = G.sc_read_level(1, ib, 0)
+        out = (G.sc_read_level(0, 0, 0), l1, G.sc_read_level(2, 0, 0))
+        G.close()
+        return out
+    ref = run(((), (), ()))
+    for name, cuts in SIB_CUTS.items():
+        got = run(cuts)
+        for l in range(3):
+            assert np.max(np.abs(got[l] - ref[l])) <= 1e-13 * np.max(np.abs(ref[l])), (name, l)
+
+
+@pytest.mark.parametrize("sigma", [0.0, 0.2])
+@pytest.mark.parametrize("sub", [True, False])
+def test_exact_quadratic_solution_through_siblings_without_the_oracle(sub, sigma):
+    """Closed form, no oracle: u = x^2+y^2+z^2+3t^2, rho = 6t through level-1 boxes that abut on a face, touch
+    along an edge, or sit two cells apart; every box, ghosts included, must hold it to rounding."""
+    n, o = 64, 16
+    l1 = [wl.Box(1, (24 + o, 24 + o, 24 + o), (16, 24, 24)), wl.Box(1, (40 + o, 24 + o, 24 + o), (16, 24, 24)),
+          wl.Box(1, (56 + o, 48 + o, 24 + o), (12, 16, 24)), wl.Box(1, (24 + o, 50 + o, 24 + o), (30, 14, 24))]
+    boxes = [wl.Box(0, (0, 0, 0), (n, n, n))] + l1 + [wl.Box(2, (88 + 2 * o, 60 + 2 * o, 60 + 2 * o), (16, 16, 16))]
+    w = wl.Workload("quadratic siblings", boxes, (n, n, n), init=wl.quadratic_init, ko_sigma=sigma)
+    G = sc.Hierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, sub)
+    t = w.dt_coarse
+    for l in (1, 2):
+        for ib in range(len(w.level_boxes(l))):
+            for c in (0, 1):
+                got = G.sc_debug_read_padded(l, ib, c)
+                want = wl.quadratic_exact(w, l, ib, c, t, pad=w.ghost)
+                assert np.max(np.abs(got - want)) < 3e-12, (sub, l, ib, c, float(np.max(np.abs(got - want))))
+    G.close()

@@ -85,8 +85,10 @@ def test_nesting_validator_rejects_bad_hierarchies(built):
     assert rc(base + [B(1, (16, 16, 16), (15, 16, 16))])[0] == SC_ERR_NESTING      # odd n
     assert rc(base + [B(1, (6, 16, 16), (16, 16, 16))])[0] == SC_ERR_NESTING       # margin 3 < 4
     assert rc(base + [B(1, (8, 16, 16), (16, 16, 16))])[0] != SC_ERR_NESTING       # margin 4 ok
-    assert rc(base + [B(1, (8, 8, 8), (16, 16, 16)), B(1, (30, 8, 8), (16, 16, 16))])[0] == SC_ERR_NESTING  # gap 6 < 8
-    assert rc(base + [B(1, (8, 8, 8), (16, 16, 16)), B(1, (32, 8, 8), (16, 16, 16))])[0] != SC_ERR_NESTING  # gap 8 ok
+    # siblings: any distance is fine (they exchange ghosts, NEXT-2), interiors must not overlap
+    assert rc(base + [B(1, (8, 8, 8), (16, 16, 16)), B(1, (30, 8, 8), (16, 16, 16))])[0] != SC_ERR_NESTING  # gap 6
+    assert rc(base + [B(1, (8, 8, 8), (16, 16, 16)), B(1, (24, 8, 8), (16, 16, 16))])[0] != SC_ERR_NESTING  # abutting
+    assert rc(base + [B(1, (8, 8, 8), (16, 16, 16)), B(1, (22, 8, 8), (16, 16, 16))])[0] == SC_ERR_NESTING  # overlap
     assert rc([B(0, (0, 0, 0), (32, 32, 16))])[0] == SC_ERR_NESTING                # level 0 must cover the domain
     assert rc(base + [B(2, (40, 40, 40), (16, 16, 16))], nlevels=3)[0] == SC_ERR_NESTING  # empty level 1
     assert rc(base, ref_ratio=4)[0] == SC_ERR_UNSUPPORTED
