@@ -33,8 +33,10 @@ METRIC = "grid-point updates/s (all levels, fp64 RK4)"
 UNIT = "updates/s"
 
 
-def pick_workload(idx: int, sigma: float = 0.0):
+def pick_workload(idx: int, sigma: float = 0.0, cut: int = 1):
     w = {1: wl.cfg1, 2: lambda: wl.cfg2(128), 3: wl.cfg3, 4: wl.cfg4, 5: wl.cfg5}[idx]()
+    if cut > 1:
+        w = wl.cut_finest(w, cut)
     if sigma:
         w.ko_sigma = sigma
         w.name += f" + Kreiss-Oliger sigma={sigma}"
@@ -86,7 +88,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    w = pick_workload(args.config, args.sigma)
+    w = pick_workload(args.config, args.sigma, args.cut_finest)
     sub = args.mode == "sub"
     r = time_oracle(w, max(1, args.steps), min(args.warmup, 1), sub, max_levels=args.oracle_levels)
     ms = 1e3 * r.pop("_seconds") / r.pop("_steps")
@@ -181,7 +183,7 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    w = pick_workload(args.config, args.sigma)
+    w = pick_workload(args.config, args.sigma, args.cut_finest)
     sub = args.mode == "sub"
     dt = w.dt_coarse
     H = sc.Hierarchy(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling, device=f"cuda:{local}",
@@ -238,7 +240,7 @@ def run_gpu(args):
     dom = max(kinds, key=lambda k: kinds[k]["ms_total"])
     ksum = sum(k["ms_total"] for k in kinds.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["algorithmic_GBps"], "peak": peak,
-                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom) if args.config == 5 and not args.sigma else None,
+                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom) if args.config == 5 and not args.sigma and args.cut_finest == 1 else None,
                 "peak_source": peak_src, "share_of_step": kinds[dom]["ms_total"] / ksum,
                 "bytes_per_launch": kinds[dom]["bytes_per_launch"], "avg_launch_us": kinds[dom]["avg_us"]}
 
@@ -307,6 +309,8 @@ def main():
     ap.add_argument("--mode", default="sub", choices=["sub", "uniform"])
     ap.add_argument("--sigma", type=float, default=0.0,
                     help="Kreiss-Oliger dissipation strength (PAPER.md eqs 35-36); 0 = the configs as BASELINE states them")
+    ap.add_argument("--cut-finest", type=int, default=1,
+                    help="cut the finest level into this many abutting slabs that exchange ghosts (NEXT-2 variant)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--oracle-levels", type=int, default=2,
                     help="levels of the workload the CPU oracle is timed on (bounded sample)")

@@ -334,3 +334,21 @@ def sibling_cut(cuts_x=(), cuts_y=(), cuts_z=(), nfields: int = 1, ko_sigma: flo
                     coupling=coupling_matrix(nfields) if nfields > 1 else None, coarse_steps=2,
                     xlo=(-4.0 / 3.0, -1.0, -1.0), xhi=(4.0 / 3.0, 1.0, 1.0),
                     init=global_index_init, ko_sigma=ko_sigma)
+
+
+def cut_finest(w: Workload, pieces: int, axis: int = 2) -> Workload:
+    """The same hierarchy with every box of the finest level cut into `pieces` abutting slabs along `axis`
+    (same cells, same work; the slabs exchange ghosts — NEXT-2). Measurement variant of a BASELINE configuration."""
+    top = w.nlevels - 1
+    boxes = [b for b in w.boxes if b.level != top]
+    for b in w.level_boxes(top):
+        step = (b.n[axis] // pieces) & ~1
+        assert step >= 8
+        for p in range(pieces):
+            lo, n = list(b.lo), list(b.n)
+            lo[axis] = b.lo[axis] + p * step
+            n[axis] = step if p < pieces - 1 else b.n[axis] - p * step
+            boxes.append(Box(top, tuple(lo), tuple(n)))
+    out = dataclasses.replace(w, boxes=boxes)
+    out.name = w.name + f", finest level cut into {pieces} abutting slabs"
+    return out
