@@ -352,3 +352,32 @@ def cut_finest(w: Workload, pieces: int, axis: int = 2) -> Workload:
     out = dataclasses.replace(w, boxes=boxes)
     out.name = w.name + f", finest level cut into {pieces} abutting slabs"
     return out
+
+
+# ----------------------------------------------------------------------------------------------
+# the paper's own scalar-wave test (eqs 41-42, Fig. 1)
+# ----------------------------------------------------------------------------------------------
+SPH_A, SPH_SIGMA = 1.0, 0.25 / math.sqrt(2.0)
+
+
+def spherical_wave_exact(w: Workload, level: int, ibox: int, comp: int, t: float) -> np.ndarray:
+    """u = [f(t-r) - f(t+r)] / r,  Pi = -[f(t-r)(t-r) - f(t+r)(t+r)] / (sigma^2 r),  f(v) = A exp(-v^2 / (2 sigma^2)),
+    A = 1, sigma = 0.25/sqrt(2) (eqs 41-42). Cell-centred grids never put a centre at r = 0 (S1)."""
+    x, y, z = w.centres(level, ibox)
+    r = np.sqrt(z[:, None, None] ** 2 + y[None, :, None] ** 2 + x[None, None, :] ** 2)
+    f = lambda v: SPH_A * np.exp(-v * v / (2.0 * SPH_SIGMA ** 2))  # noqa: E731
+    if comp < w.nfields:
+        return (f(t - r) - f(t + r)) / r
+    return -(f(t - r) * (t - r) - f(t + r) * (t + r)) / (SPH_SIGMA ** 2 * r)
+
+
+def paper_wave(n0: int = 64) -> Workload:
+    """The paper's Fig. 1 set-up: three levels with refinement boundaries at r = 4, 1, 0.5 (read as
+    the half-widths of cubic boxes), dx_0 = 8 / n0: n0 = 64, 96, 128 are its h_1 = 1/8, h_1/1.5, h_1/2. The outer
+    boundary is periodic here (S9): valid until the pulse reaches r = 4."""
+    assert n0 % 16 == 0
+    q = n0 // 4
+    boxes = [Box(0, (0, 0, 0), (n0, n0, n0)), Box(1, (n0 - q,) * 3, (2 * q,) * 3), Box(2, (2 * n0 - q,) * 3, (2 * q,) * 3)]
+    return Workload(f"paper Fig. 1: Gaussian spherical wave, 3 levels (r = 4, 1, 0.5), dx_0 = 8/{n0}", boxes,
+                    (n0, n0, n0), xlo=(-4.0, -4.0, -4.0), xhi=(4.0, 4.0, 4.0),
+                    init=lambda w, l, ib, c: spherical_wave_exact(w, l, ib, c, 0.0))

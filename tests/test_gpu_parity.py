@@ -390,3 +390,35 @@ def test_exact_quadratic_solution_through_siblings_without_the_oracle(sub, sigma
                 want = wl.quadratic_exact(w, l, ib, c, t, pad=w.ghost)
                 assert np.max(np.abs(got - want)) < 3e-12, (sub, l, ib, c, float(np.max(np.abs(got - want))))
     G.close()
+
+
+# ---- the paper's own validation run (Fig. 1) --------------------------------------------------
+def test_paper_fig1_ladder_on_the_gpu():
+    """Gaussian spherical wave (eqs 41-42), three levels (r = 4, 1, 0.5), h_1 = 1/8, h_1/1.5, h_1/2, to t = 1.5
+    (the pulse has crossed both refinement boundaries): fourth-order convergence of the error on the second
+    refinement level against the exact solution, subcycled and uniform — no oracle involved; then parity with the
+    oracle on the low resolution."""
+    T = 1.5
+    err = {}
+    for sub in (True, False):
+        for n0 in (64, 96, 128):
+            w = wl.paper_wave(n0)
+            G = sc.Hierarchy.from_workload(w)
+            ns = int(round(T / w.dt_coarse))
+            for _ in range(ns):
+                G.sc_step(w.dt_coarse, sub)
+            err[(sub, n0)] = max(np.max(np.abs(G.sc_read_level(2, 0, c) - wl.spherical_wave_exact(w, 2, 0, c, T)))
+                                 for c in (0, 1))
+            G.close()
+        o1 = np.log(err[(sub, 64)] / err[(sub, 96)]) / np.log(1.5)
+        o2 = np.log(err[(sub, 64)] / err[(sub, 128)]) / np.log(2.0)
+        print(f"Fig. 1 on the GPU, sub={sub}: errors {err[(sub, 64)]:.3e} {err[(sub, 96)]:.3e} {err[(sub, 128)]:.3e}, orders {o1:.2f} {o2:.2f}")
+        assert 3.7 < o1 < 4.3 and 3.7 < o2 < 4.3
+    for n0 in (64, 96, 128):
+        assert abs(err[(True, n0)] / err[(False, n0)] - 1.0) < 0.05
+    w = wl.paper_wave(64)
+    G, O = _pair(w)
+    for _ in range(8):
+        G.sc_step(w.dt_coarse, True)
+        O.step(w.dt_coarse, True)
+    _compare_state(G, O, w, what="paper Fig. 1, 8 subcycled steps")

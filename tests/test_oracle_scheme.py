@@ -417,3 +417,29 @@ def test_dissipation_damps_grid_noise_and_keeps_smooth_data(oracle_mod):
             H.step(0.25 * 2.0 / n, True)
         out[sigma] = np.max(np.abs(H.read_level(0, 0, 1)))
     assert out[0.5] < 0.2 * out[0.0]
+
+
+@pytest.mark.slow
+def test_paper_fig1_spherical_wave_fourth_order(oracle_mod):
+    """The paper's own validation (eqs 41-42, Fig. 1): Gaussian spherical wave, three levels with
+    refinement boundaries at r = 4, 1, 0.5, resolutions h_1 = 1/8, h_1/1.5, h_1/2; errors on the second refinement
+    level against the exact solution after the pulse has crossed the level-2 boundary (t = 0.75), 'assuming
+    fourth-order convergence' for subcycling and for uniform stepping alike."""
+    T = 0.75
+    err = {}
+    for sub, n0 in ((True, 64), (True, 96), (True, 128), (False, 64), (False, 96)):
+        w = wl.paper_wave(n0)
+        H = oracle_mod.OracleHierarchy.from_workload(w)
+        ns = int(round(T / w.dt_coarse))
+        assert abs(ns * w.dt_coarse - T) < 1e-12
+        for _ in range(ns):
+            H.step(w.dt_coarse, sub)
+        err[(sub, n0)] = [max(np.max(np.abs(H.read(l, 0, c) - wl.spherical_wave_exact(w, l, 0, c, T))) for c in (0, 1))
+                          for l in range(3)]
+    o_med = math.log(err[(True, 64)][2] / err[(True, 96)][2]) / math.log(1.5)
+    o_high = math.log(err[(True, 64)][2] / err[(True, 128)][2]) / math.log(2.0)
+    o_uni = math.log(err[(False, 64)][2] / err[(False, 96)][2]) / math.log(1.5)
+    print("Fig. 1 orders (level 2): sub %.2f %.2f, uniform %.2f; errors %s" % (o_med, o_high, o_uni, err))
+    assert 3.7 < o_med < 4.3 and 3.7 < o_high < 4.3 and 3.7 < o_uni < 4.3
+    for n0 in (64, 96):  # subcycling and uniform stepping give the same error curve (Fig. 1)
+        assert abs(err[(True, n0)][2] / err[(False, n0)][2] - 1.0) < 0.05
