@@ -473,7 +473,7 @@ void level_step_ko(Seq& q, int level, double dt, double theta) {
     } else if (s < 4) {  // the stage vector just produced: ghosts inside a sibling take the sibling's Y_{s+1}
       sibling_level(q, level, L.a_U(s + 1), L.F);
       sibling_level(q, level, L.a_R(s + 1), L.F);
-    } else {
+    } else if (theta != 0.0) {
       sibling_level(q, level, L.a_state(1 - yn), L.V);
     }
   }
@@ -534,8 +534,10 @@ void level_step(Seq& q, int level, double dt, double theta) {
   if (level == 0) {
     periodic_level0(q, L.a_state(1 - yn), L.V);
     q.l0_valid = true;
-  } else {
-    sibling_level(q, level, L.a_state(1 - yn), L.V);  // y_{n+1}: read by the restriction and sc_debug_read_padded
+  } else if (theta != 0.0) {
+    // y_{n+1} of the step that ends at the parent's t_{n+1}: read by the restriction and sc_debug_read_padded. After
+    // a first sub-step (theta = 0) nothing reads these ghosts before the next launch refills and re-exchanges them.
+    sibling_level(q, level, L.a_state(1 - yn), L.V);
   }
   q.cur[level] = 1 - yn;
 }
