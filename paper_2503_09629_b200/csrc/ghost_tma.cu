@@ -38,6 +38,7 @@
 #include <cstdlib>
 
 #include "kernels.h"
+#include "pdl.h"
 
 namespace sc {
 
@@ -303,6 +304,7 @@ __device__ __forceinline__ void phase2x(const GhostArgs& a, const GhostProblem& 
 __global__ void __launch_bounds__(NTHR, 2)
     ghost_fill_tma(const __grid_constant__ CUtensorMap mapx, const __grid_constant__ CUtensorMap mapy,
                    const __grid_constant__ CUtensorMap mapz, const __grid_constant__ GhostArgs a) {
+  pdl_enter();
   extern __shared__ unsigned char gsm_raw[];
   __shared__ double sWt[4][PT];  // thin-axis weights (ghost widths other than 3): thin cell k <- footprint cell c
   __shared__ __align__(8) unsigned long long sbar;
@@ -509,7 +511,7 @@ void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st) {
   const long long rounds = (nitems + want - 1) / want;
   const unsigned grid = (unsigned)(nitems <= want ? nitems : (nitems + rounds - 1) / rounds);
   const CUtensorMap* m = static_cast<const CUtensorMap*>(a.tmaps);
-  ghost_fill_tma<<<grid, NTHR, smem, st>>>(m[0], m[1], m[2], a);
+  launch_pdl(ghost_fill_tma, dim3(grid), dim3(NTHR), smem, st, m[0], m[1], m[2], a);
 }
 
 }  // namespace sc

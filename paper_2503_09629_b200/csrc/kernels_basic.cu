@@ -7,6 +7,7 @@
 // containing fine cell I is I >> 1 (arithmetic shift = floor), its parity I & 1 (1: fine centre at
 // +dx_parent/4). Cell-centred grids (reading S1).
 #include "kernels.h"
+#include "pdl.h"
 
 namespace sc {
 
@@ -201,6 +202,7 @@ void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st) {
 __device__ inline int wrap(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
 
 __global__ void __launch_bounds__(128) periodic_fill_ref(BoxView b, double* y, long long nshell) {
+  pdl_enter();
   const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= nshell) return;
   int i, j, k;
@@ -212,7 +214,7 @@ __global__ void __launch_bounds__(128) periodic_fill_ref(BoxView b, double* y, l
 void launch_periodic_fill(const BoxView& b, int V, double* y, cudaStream_t st) {
   const long long ns = ghost_cell_count(b);
   dim3 grd((unsigned)((ns + 127) / 128), V, 1);
-  periodic_fill_ref<<<grd, 128, 0, st>>>(b, y, ns);
+  launch_pdl(periodic_fill_ref, grd, dim3(128), 0, st, b, y, ns);
 }
 
 // ------------------------------------------------------------------------------------------------

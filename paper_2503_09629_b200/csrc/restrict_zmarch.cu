@@ -17,6 +17,7 @@
 #include <cstdlib>
 
 #include "kernels.h"
+#include "pdl.h"
 
 namespace sc {
 
@@ -59,6 +60,7 @@ struct RestrictParams {
 
 __global__ void __launch_bounds__(RNT, 3)
     restrict_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ RestrictParams p) {
+  pdl_enter();
   extern __shared__ unsigned char rsm[];
   const uint32_t s0 = (smem_u32r(rsm) + 127u) & ~127u;
   const double* const tiles = reinterpret_cast<const double*>(rsm + (s0 - smem_u32r(rsm)));  // [NSTR][2][RFY][RPITCH]
@@ -172,7 +174,7 @@ void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st) {
   p.nzc = (npz + p.pz_per_cta - 1) / p.pz_per_cta;
   p.yp = a.yparent;
   dim3 grd(gx, gy, p.nzc * a.V);
-  restrict_zmarch<<<grd, RNT, restrict_smem(), st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
+  launch_pdl(restrict_zmarch, grd, dim3(RNT), restrict_smem(), st, *static_cast<const CUtensorMap*>(a.tmap), p);
 }
 
 }  // namespace sc

@@ -20,6 +20,7 @@
 #include <type_traits>
 
 #include "kernels.h"
+#include "pdl.h"
 
 namespace sc {
 
@@ -130,6 +131,7 @@ template <int MODE, bool COUPLED>
 __global__ void __launch_bounds__(NTHR, 2)
     stage_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ TmaStageParams p) {
   constexpr int NH = MODE == STAGE_12 ? 2 : 3;  // halo-read arrays per plane
+  pdl_enter();
   extern __shared__ unsigned char smraw[];
   // [NST][NH] tiles, 128-byte aligned for TMA, then NST mbarriers
   const uint32_t s0 = (smem_u32(smraw) + 127u) & ~127u;
@@ -346,7 +348,7 @@ void launch_zmarch(const StageArgs& a, cudaStream_t st) {
   for (int d = 0; d < 3; ++d) p.w[d] = a.inv12dx2[d];
   p.S = a.S;
   dim3 grd((a.b.n[0] + TX - 1) / TX, (a.b.n[1] + TY - 1) / TY, p.nchunks * a.F);
-  stage_zmarch<MODE, COUPLED><<<grd, NTHR, stage_smem<MODE>(), st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
+  launch_pdl(stage_zmarch<MODE, COUPLED>, grd, dim3(NTHR), stage_smem<MODE>(), st, *static_cast<const CUtensorMap*>(a.tmap), p);
 }
 
 }  // namespace
