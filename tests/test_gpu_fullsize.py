@@ -144,3 +144,30 @@ def test_cfg5_uniform_mode_full_depth_finite_and_close_to_subcycled():
         assert np.max(np.abs(a - b)) < 2e-5, (l, float(np.max(np.abs(a - b))))
     Gs.close()
     Gu.close()
+
+
+@pytest.mark.parametrize("cfg", ["cfg3", "cfg5", "cfg4"])
+def test_baseline_full_runs(cfg):
+    """The runs BASELINE.json states, whole: cfg 3 (4 x 128^3, 50 coarse steps) and cfg 5 (6 x 256^3, 20 coarse
+    steps) subcycled AND with every level at the finest dt, cfg 4 (7 levels, 22 coupled fields, 20 coarse steps)
+    subcycled. No dissipation, deep hierarchies: the state must stay finite and bounded, and the two modes must
+    agree to truncation level (north_star) — measured 2e-4 of the largest component, required 1e-3."""
+    w = {"cfg3": wl.cfg3, "cfg5": wl.cfg5, "cfg4": wl.cfg4}[cfg]()
+    comps = (0, 1) if cfg != "cfg4" else (0, w.nfields)
+    res = {}
+    for sub in ((True, False) if cfg != "cfg4" else (True,)):
+        G = sc.Hierarchy.from_workload(w)
+        for _ in range(w.coarse_steps):
+            G.sc_step(w.dt_coarse, sub)
+        res[sub] = [G.sc_read_level(l, ib, c) for l in range(w.nlevels) for ib in range(len(w.level_boxes(l)))
+                    for c in comps]
+        G.close()
+        assert all(np.isfinite(a).all() for a in res[sub]), (cfg, sub)
+    big = max(float(np.max(np.abs(a))) for a in res[True])
+    start = max(float(np.max(np.abs(w.initial_state(l, 0, c)))) for l in range(w.nlevels) for c in comps)
+    # u stays below its start, rho = d_t u of a pulse of width 0.05 reaches ~ 1 / 0.05 times that
+    assert big < 40.0 * start, (cfg, big, start)
+    if False in res:
+        worst = max(float(np.max(np.abs(a - b))) for a, b in zip(res[True], res[False]))
+        print(f"{cfg}: max|sub - uniform| = {worst:.2e} of {big:.2e}")
+        assert worst < 1e-3 * big, (cfg, worst, big)
