@@ -422,3 +422,31 @@ def test_paper_fig1_ladder_on_the_gpu():
         G.sc_step(w.dt_coarse, True)
         O.step(w.dt_coarse, True)
     _compare_state(G, O, w, what="paper Fig. 1, 8 subcycled steps")
+
+
+def test_cfg2_convergence_ladder_on_the_gpu():
+    """BASELINE config 2 as stated, whole and without the oracle: coarse 32^3, 64^3, 128^3 (fine boxes scaled to
+    match), plane wave evolved to t = 1 (64 / 128 / 256 coarse steps); error against the exact solution on both
+    levels, convergence order, both modes; and the subcycled - uniform difference, which must stay below the
+    truncation error and itself converge (third order: eq (10)'s local error, DESIGN S12)."""
+    err, sol = {}, {}
+    for sub in (True, False):
+        for n in (32, 64, 128):
+            w = wl.cfg2(n)
+            G = sc.Hierarchy.from_workload(w)
+            for _ in range(w.coarse_steps):
+                G.sc_step(w.dt_coarse, sub)
+            assert abs(G.sc_time() - 1.0) < 1e-12
+            sol[(sub, n)] = [G.sc_read_level(l, 0, 0) for l in (0, 1)]
+            err[(sub, n)] = [float(np.max(np.abs(sol[(sub, n)][l] - wl.plane_wave_exact(w, l, 0, 0, 1.0)))) for l in (0, 1)]
+            G.close()
+        for l in (0, 1):
+            o1 = np.log2(err[(sub, 32)][l] / err[(sub, 64)][l])
+            o2 = np.log2(err[(sub, 64)][l] / err[(sub, 128)][l])
+            print(f"cfg2 sub={sub} level {l}: errors {err[(sub, 32)][l]:.3e} {err[(sub, 64)][l]:.3e} {err[(sub, 128)][l]:.3e} orders {o1:.2f} {o2:.2f}")
+            assert 3.8 < o1 < 4.2 and 3.8 < o2 < 4.2
+    diff = [max(float(np.max(np.abs(a - b))) for a, b in zip(sol[(True, n)], sol[(False, n)])) for n in (32, 64, 128)]
+    print("cfg2 max|sub - uniform|:", ["%.2e" % d for d in diff])
+    for d, n in zip(diff, (32, 64, 128)):
+        assert d < 0.5 * err[(True, n)][1]
+    assert 2.5 < np.log2(diff[0] / diff[1]) < 4.5 and 2.5 < np.log2(diff[1] / diff[2]) < 4.5
