@@ -313,10 +313,10 @@ def test_convergence_ladder_and_sub_vs_uniform(oracle_mod):
         for l in (0, 1):
             order = math.log2(e32[l] / e64[l])
             assert 3.8 < order < 4.2, (l, e32, e64, order)
-    assert np.allclose(e32s, [6.201e-5, 6.208e-5], rtol=0.03)
-    assert np.allclose(e64s, [3.972e-6, 3.984e-6], rtol=0.03)
-    assert np.allclose(e32u, [6.001e-5, 6.009e-5], rtol=0.03)
-    assert np.allclose(e64u, [3.829e-6, 3.838e-6], rtol=0.03)
+    assert np.allclose(e32s, [6.201e-5, 6.208e-5], rtol=2e-3)
+    assert np.allclose(e64s, [3.972e-6, 3.984e-6], rtol=2e-3)
+    assert np.allclose(e32u, [6.001e-5, 6.009e-5], rtol=2e-3)
+    assert np.allclose(e64u, [3.829e-6, 3.838e-6], rtol=2e-3)
     d32 = max(np.max(np.abs(a - b)) for a, b in zip(u32s, u32u))
     d64 = max(np.max(np.abs(a - b)) for a, b in zip(u64s, u64u))
     assert d32 < 0.2 * max(e32s) and d64 < 0.3 * max(e64s)
