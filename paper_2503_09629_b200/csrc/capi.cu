@@ -45,6 +45,10 @@ struct sc_hierarchy {
   bool own_arena = false;
   cudaStream_t stream = nullptr;
   bool own_stream = false;
+  // second stream of the level scheduler: a level's theta = 1/2 ghost fill runs beside its children's sub-steps
+  cudaStream_t side = nullptr;
+  std::vector<cudaEvent_t> ev_fork, ev_join;  // per level
+  int overlap_mode = -1;                      // SC_OVERLAP: 0 / 1 force the side stream off / on, default by level size
   double* staging = nullptr;      // device, largest padded dense box
   size_t staging_bytes = 0;
   std::vector<double> coupling_host;  // F*F, host copy of the coupling matrix
@@ -131,6 +135,8 @@ struct Seq {
   bool l0_valid;         // working copy of l0_ghosts_valid
   uint64_t n = 0;
   bool sub = true;       // subcycled mode (parents keep k_4 for their children)
+  bool capturing = false;       // the launches are being captured into a CUDA graph (fork / join allowed)
+  std::vector<char> prefilled;  // per level: the next level-step's refinement ghosts are already written
 };
 
 enum { KIND_STAGE = 0, KIND_GHOST = 1, KIND_PERIODIC = 2, KIND_RESTRICT = 3, NKIND = 4 };
@@ -456,12 +462,53 @@ void fill_level_dense_ko(Seq& q, int level, double theta, double dt) {
   }
 }
 
+// Fork / join of the level scheduler. The refinement ghosts of a level's SECOND sub-step (theta = 1/2) depend only on
+// the parent's stored step, which is complete once the parent has stepped: they can be written as soon as the
+// first sub-step's kernels have read the shells they replace — while the children of this level take their two
+// sub-steps and restrict (those read and write this level's INTERIOR only: footprints lie 4 cells inside, S13).
+// In a captured step the fill is recorded on a second stream (a parallel branch of the graph) and joined before
+// the second sub-step's first stage kernel; eager / profiled steps issue it in place on the one stream.
+void prefill_second_substep(Seq& q, int level, double dt) {
+  sc_hierarchy* h = q.h;
+  const Layout& L = h->L;
+  cudaStream_t main = h->stream;
+  if (q.capturing) {
+    cudaEventRecord(h->ev_fork[level], main);
+    cudaStreamWaitEvent(h->side, h->ev_fork[level], 0);
+    h->stream = h->side;
+  }
+  if (L.ko_sigma > 0.0) fill_level_dense_ko(q, level, 0.5, dt);
+  else fill_level_dense(q, level, 0.5, dt);
+  sibling_level(q, level, L.a_state(q.cur[level]), L.V);
+  if (q.capturing) {
+    cudaEventRecord(h->ev_join[level], h->side);
+    h->stream = main;
+  }
+  q.prefilled[level] = 1;
+}
+// Measured (profiles/r01_v4.md): beside the children's kernels the fill costs nothing on 128^3 levels (cfg 3 0.806 ->
+// 0.798 ms per coarse step, cfg 4 184.4 -> 183.6 ms) but its CTAs disturb the bandwidth-bound stage kernels of 256^3
+// levels (cfg 5 21.68 -> 21.9 ms): the branch is taken for levels of at most 6 M cells. SC_OVERLAP=0 / 1 forces it.
+bool overlap_wanted(const sc_hierarchy* h, int level) {
+  if (h->overlap_mode >= 0) return h->overlap_mode != 0;
+  double n = 0.0;
+  for (int ib : h->L.level_boxes[level]) n += cells(h->L.boxes[ib].v);
+  return n <= 6.0e6;
+}
+// true if the ghosts of the level-step about to start were prefilled (and, in a captured step, joins the branch)
+bool join_prefill(Seq& q, int level) {
+  if (!q.prefilled[level]) return false;
+  q.prefilled[level] = 0;
+  if (q.capturing) cudaStreamWaitEvent(q.h->stream, q.h->ev_join[level], 0);
+  return true;
+}
+
 void level_step_ko(Seq& q, int level, double dt, double theta) {
   const Layout& L = q.h->L;
   const int yn = q.cur[level];
   if (level == 0) {
     if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
-  } else {
+  } else if (!join_prefill(q, level)) {
     fill_level_dense_ko(q, level, theta, dt);
     sibling_level(q, level, L.a_state(yn), L.V);
   }
@@ -523,7 +570,7 @@ void level_step(Seq& q, int level, double dt, double theta) {
   const int yn = q.cur[level];
   if (level == 0) {
     if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
-  } else {
+  } else if (!join_prefill(q, level)) {
     fill_level_dense(q, level, theta, dt);
     sibling_level(q, level, L.a_state(yn), L.V);  // u_n, rho_n: on a sibling's interior u_n + a_1 dt rho_n IS Y_{2,u}
   }
@@ -546,6 +593,7 @@ void level_step(Seq& q, int level, double dt, double theta) {
 void advance(Seq& q, int level, double dt, double theta) {
   level_step(q, level, dt, theta);
   if (level + 1 < q.h->L.nlevels) {
+    if (level >= 1 && theta == 0.0 && overlap_wanted(q.h, level)) prefill_second_substep(q, level, dt);
     advance(q, level + 1, 0.5 * dt, 0.0);
     advance(q, level + 1, 0.5 * dt, 0.5);
     restrict_level(q, level + 1);
@@ -770,6 +818,17 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   h->l0_ghosts_valid = false;
   const char* env = getenv("SC_KERNELS");
   select_kernels(env && !strcmp(env, "ref") ? 0 : 1);
+  {
+    const char* eo = getenv("SC_OVERLAP");
+    h->overlap_mode = eo ? (strcmp(eo, "0") ? 1 : 0) : -1;
+    if ((ce = cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking)) != cudaSuccess) return bail("cudaStreamCreate(side)", ce);
+    h->ev_fork.assign(h->L.nlevels, nullptr);
+    h->ev_join.assign(h->L.nlevels, nullptr);
+    for (int l = 0; l < h->L.nlevels; ++l) {
+      cudaEventCreateWithFlags(&h->ev_fork[l], cudaEventDisableTiming);
+      cudaEventCreateWithFlags(&h->ev_join[l], cudaEventDisableTiming);
+    }
+  }
   const char* eg = getenv("SC_GRAPH");
   h->use_graph = !(eg && !strcmp(eg, "0"));
   const char* ed = getenv("SC_DEBUG_SYNC");
@@ -807,6 +866,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
   if (!std::isfinite(dt_coarse) || dt_coarse <= 0.0) { set_error("dt_coarse must be finite and > 0"); return SC_ERR_INVALID_ARG; }
   subcycling = subcycling ? 1 : 0;
   Seq q{h, h->cur, h->l0_ghosts_valid, 0};
+  q.prefilled.assign(h->L.nlevels, 0);
   if (!h->use_graph || h->profiling) {
     record_step(q, dt_coarse, subcycling);
     SC_CUDA(cudaGetLastError());
@@ -820,6 +880,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
     if (it == h->graphs.end()) {
       cudaGraph_t g = nullptr;
       SC_CUDA(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+      q.capturing = true;
       record_step(q, dt_coarse, subcycling);
       cudaError_t le = cudaGetLastError();
       cudaError_t ee = cudaStreamEndCapture(h->stream, &g);
@@ -939,6 +1000,9 @@ int32_t sc_destroy(sc_hierarchy* h) {
   for (auto& bt : h->tiles) if (bt.dev) cudaFree(bt.dev);
   for (auto& s : h->sib) if (s.dev) cudaFree(s.dev);
   if (h->own_arena && h->arena) cudaFree(h->arena);
+  for (auto e : h->ev_fork) if (e) cudaEventDestroy(e);
+  for (auto e : h->ev_join) if (e) cudaEventDestroy(e);
+  if (h->side) cudaStreamDestroy(h->side);
   if (h->own_stream) cudaStreamDestroy(h->stream);
   delete h;
   return SC_OK;
