@@ -241,7 +241,7 @@ def run_gpu(args):
     ksum = sum(k["ms_total"] for k in kinds.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["algorithmic_GBps"], "peak": peak,
                 "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom) if args.config == 5 and not args.sigma and args.cut_finest == 1 else None,
-                "peak_source": peak_src, "share_of_step": kinds[dom]["ms_total"] / ksum,
+                "peak_source": peak_src, "frac_of_nominal_8TBps": kinds[dom]["algorithmic_GBps"] / 8000.0, "share_of_step": kinds[dom]["ms_total"] / ksum,
                 "bytes_per_launch": kinds[dom]["bytes_per_launch"], "avg_launch_us": kinds[dom]["avg_us"]}
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the whole state, step, D2H ---------

@@ -147,6 +147,11 @@ int32_t sc_debug_read_padded(sc_hierarchy* h, int32_t level, int32_t box, int32_
 int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t slot, int32_t comp,
                            double* dst);
 
+/* Debug: max |value| over the INTERIOR of one component of the current state of a box, reduced on the device
+ * (one 8-byte read-back). *out (HOST) is NaN as soon as one value is NaN, +inf if one is infinite: the check
+ * for a run that blew up, without copying the state. Synchronises the stream. */
+int32_t sc_debug_max_abs(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, double* out);
+
 /* Per-kernel timing for the roofline report. sc_profile(h, 1): from now on sc_step launches its kernels
  * one by one (no graph replay) with a CUDA-event pair around each on the hierarchy's stream;
  * sc_profile(h, 0) stops and discards the records. sc_profile_read sums, over the records since

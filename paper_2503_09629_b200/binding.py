@@ -19,7 +19,7 @@ SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NESTING, SC_ERR_UNSUPPORTED, SC_ERR_OOM, SC_ER
 
 EXPORTS = ["sc_arena_bytes", "sc_create_hierarchy", "sc_set_state", "sc_step", "sc_read_level", "sc_time",
            "sc_launch_count", "sc_debug_ghost_map", "sc_debug_read_padded", "sc_debug_read_slot", "sc_destroy",
-           "sc_last_error", "sc_profile", "sc_profile_read"]
+           "sc_last_error", "sc_profile", "sc_profile_read", "sc_debug_max_abs"]
 
 
 class sc_box(C.Structure):
@@ -73,6 +73,8 @@ def lib():
         L.sc_debug_read_padded.argtypes = [H, C.c_int32, C.c_int32, C.c_int32, dp]
         L.sc_debug_read_slot.restype = C.c_int32
         L.sc_debug_read_slot.argtypes = [H, C.c_int32, C.c_int32, C.c_int32, C.c_int32, dp]
+        L.sc_debug_max_abs.restype = C.c_int32
+        L.sc_debug_max_abs.argtypes = [H, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
         L.sc_destroy.restype = C.c_int32
         L.sc_destroy.argtypes = [H]
         L.sc_profile.restype = C.c_int32
@@ -220,6 +222,11 @@ class Hierarchy:
         out = np.empty((b.n[2] + 2 * g, b.n[1] + 2 * g, b.n[0] + 2 * g), dtype=np.float64)
         _check(lib().sc_debug_read_padded(self._h, level, ibox, comp, out.ctypes.data))
         return out
+
+    def sc_debug_max_abs(self, level: int, ibox: int, comp: int) -> float:
+        out = C.c_double(0.0)
+        _check(lib().sc_debug_max_abs(self._h, level, ibox, comp, C.byref(out)))
+        return out.value
 
     def sc_debug_read_slot(self, level: int, ibox: int, slot: int, comp: int) -> np.ndarray:
         b = self._box(level, ibox)

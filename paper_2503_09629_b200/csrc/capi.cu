@@ -947,6 +947,23 @@ int32_t sc_debug_read_padded(sc_hierarchy* h, int32_t level, int32_t box, int32_
   return read_array(h, gb, h->arr(gb, h->L.a_state(h->cur[level]) + comp), dst, 1, 0);
 }
 
+int32_t sc_debug_max_abs(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, double* out) {
+  int gb;
+  int rc = check_box(h, level, box, comp, &gb);
+  if (rc != SC_OK) return rc;
+  if (!out) { set_error("null out"); return SC_ERR_INVALID_ARG; }
+  unsigned long long* bits = reinterpret_cast<unsigned long long*>(h->staging);
+  SC_CUDA(cudaMemsetAsync(bits, 0, sizeof(unsigned long long), h->stream));
+  launch_max_abs(h->L.boxes[gb].v, h->arr(gb, h->L.a_state(h->cur[level]) + comp), bits, h->stream);
+  ++h->launches;
+  SC_CUDA(cudaGetLastError());
+  unsigned long long r = 0;
+  SC_CUDA(cudaMemcpyAsync(&r, bits, sizeof r, cudaMemcpyDeviceToHost, h->stream));
+  SC_CUDA(cudaStreamSynchronize(h->stream));
+  memcpy(out, &r, sizeof r);
+  return SC_OK;
+}
+
 int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t slot, int32_t comp, double* dst) {
   int gb;
   int rc = check_box(h, level, box, comp, &gb);

@@ -159,6 +159,10 @@ void launch_sibling_copy(const SiblingPair* pairs_dev, int npairs, long long max
 void launch_pack(const BoxView& b, const double* padded, double* dense, int with_ghosts, cudaStream_t st);
 void launch_unpack(const BoxView& b, const double* dense, double* padded, cudaStream_t st);
 
+// debug: max |x| over the interior (NaN if any value is NaN); *out_bits (device) must be zeroed by the caller and
+// receives the bit pattern of the result (non-negative doubles order like their bit patterns)
+void launch_max_abs(const BoxView& b, const double* padded, unsigned long long* out_bits, cudaStream_t st);
+
 // debug: ghost index map with the same device index arithmetic as the ghost kernels
 void launch_ghost_map(const BoxView& child, const BoxView& parent, int* out, cudaStream_t st);
 long long ghost_cell_count(const BoxView& b);

@@ -240,6 +240,29 @@ void launch_sibling_copy(const SiblingPair* pairs_dev, int npairs, long long max
 }
 
 // ------------------------------------------------------------------------------------------------
+// debug: max |x| over the interior. |x| of a NaN has a larger bit pattern than +inf, so the integer maximum of
+// the bit patterns returns NaN if there is one, else +inf if there is one, else the largest magnitude.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) max_abs_kernel(BoxView b, const double* __restrict__ a,
+                                                      unsigned long long* __restrict__ out) {
+  const int j = blockIdx.x, k = blockIdx.y;
+  unsigned long long m = 0ull;
+  for (int i = threadIdx.x; i < b.n[0]; i += blockDim.x) {
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(fabs(a[cell_offset(b, i, j, k)]));
+    m = bits > m ? bits : m;
+  }
+  for (int s = 16; s > 0; s >>= 1) {
+    const unsigned long long o = __shfl_xor_sync(0xffffffffu, m, s);
+    m = o > m ? o : m;
+  }
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+void launch_max_abs(const BoxView& b, const double* padded, unsigned long long* out_bits, cudaStream_t st) {
+  dim3 grd(b.n[1], b.n[2], 1);
+  max_abs_kernel<<<grd, 128, 0, st>>>(b, padded, out_bits);
+}
+
+// ------------------------------------------------------------------------------------------------
 // a5  restriction, one thread per parent cell, 216-point gather
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) restrict_ref(BoxView ch, BoxView pa, const double* yc, double* yp) {

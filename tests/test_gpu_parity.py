@@ -450,3 +450,22 @@ def test_cfg2_convergence_ladder_on_the_gpu():
     for d, n in zip(diff, (32, 64, 128)):
         assert d < 0.5 * err[(True, n)][1]
     assert 2.5 < np.log2(diff[0] / diff[1]) < 4.5 and 2.5 < np.log2(diff[1] / diff[2]) < 4.5
+
+
+def test_debug_max_abs():
+    """sc_debug_max_abs: device-side max |x| over the interior; NaN as soon as one value is NaN, inf if one is
+    infinite — the check for a run that blew up, without copying the state."""
+    w = wl.ragged_small()
+    G = sc.Hierarchy.from_workload(w)
+    for l in range(w.nlevels):
+        for ib in range(len(w.level_boxes(l))):
+            for c in range(w.ncomp):
+                assert G.sc_debug_max_abs(l, ib, c) == float(np.max(np.abs(w.initial_state(l, ib, c))))
+    a = w.initial_state(1, 0, 0).copy()
+    a[3, 5, 7] = np.inf
+    G.sc_set_state(1, 0, 0, a)
+    assert G.sc_debug_max_abs(1, 0, 0) == np.inf
+    a[2, 1, 0] = np.nan
+    G.sc_set_state(1, 0, 0, a)
+    assert np.isnan(G.sc_debug_max_abs(1, 0, 0))
+    G.close()
