@@ -47,6 +47,7 @@ def lib():
         L.oc_create.argtypes = [C.c_int, C.c_int, ip, ip, ip, C.c_int, C.c_int, ip, dp, dp, dp]
         L.oc_destroy.argtypes = [C.c_void_p]
         L.oc_set_dissipation.argtypes = [C.c_void_p, C.c_double]
+        L.oc_set_fd_order.argtypes = [C.c_void_p, C.c_int]
         L.oc_set_state.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, dp]
         L.oc_read.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, dp]
         L.oc_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
@@ -103,7 +104,7 @@ class OracleHierarchy:
 
     def __init__(self, boxes, domain_cells, nfields: int = 1, ghost: int = 3,
                  xlo=(-1.0, -1.0, -1.0), xhi=(1.0, 1.0, 1.0), coupling: Optional[np.ndarray] = None,
-                 ko_sigma: float = 0.0):
+                 ko_sigma: float = 0.0, fd_order: int = 4):
         L = lib()
         self.boxes = list(boxes)
         self.nfields, self.ghost = nfields, ghost
@@ -125,11 +126,13 @@ class OracleHierarchy:
         self.nlevels = nlev
         if ko_sigma and L.oc_set_dissipation(self._h, float(ko_sigma)) != 0:
             raise ValueError("oracle: " + L.oc_last_error().decode())
+        if fd_order != 4 and L.oc_set_fd_order(self._h, int(fd_order)) != 0:
+            raise ValueError("oracle: " + L.oc_last_error().decode())
 
     @classmethod
     def from_workload(cls, w) -> "OracleHierarchy":
         h = cls(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling,
-                ko_sigma=getattr(w, "ko_sigma", 0.0))
+                ko_sigma=getattr(w, "ko_sigma", 0.0), fd_order=getattr(w, "fd_order", 4))
         for l in range(w.nlevels):
             for ib in range(len(w.level_boxes(l))):
                 for c in range(w.ncomp):

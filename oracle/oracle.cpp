@@ -15,6 +15,7 @@
 //   wave system, eqs (39)-(40) ............. PAPER.md:222-226   -> rhs()
 //   Kreiss-Oliger dissipation, eqs (35)-(36) PAPER.md:194-204   -> add_dissipation()
 //   same-level ghost exchange .............. PAPER.md:20, 347   -> sibling_exchange()
+//   8th-order finite differences ........... PAPER.md:125       -> rhs() with fd_order = 8 (NEXT-3)
 //
 // Where the paper is silent the readings S1..S24 of DESIGN.md apply (cell-centred grids S1, 4th-order
 // centred Laplacian S2, quartic Lagrange prolongation S3, quintic Lagrange restriction S4, parent-step
@@ -161,6 +162,7 @@ struct Hier {
   double xlo[3], xhi[3];
   std::vector<double> A;  // F*F coupling or empty
   double sigma = 0.0;     // Kreiss-Oliger dissipation strength (eqs 35-36); 0 = none
+  int fd_order = 4;       // order of the centred finite differences of the RHS: 4 (S2) or 8 (NEXT-3)
   std::vector<BoxData> boxes;
   std::vector<std::vector<int>> level_boxes;
   double time = 0.0;
@@ -226,6 +228,22 @@ void rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vect
                               16.0 * u.at(i, j + 1, k) - u.at(i, j + 2, k)) * inv12dx2[1];
           const double dzz = (-u.at(i, j, k - 2) + 16.0 * u.at(i, j, k - 1) - 30.0 * u.at(i, j, k) +
                               16.0 * u.at(i, j, k + 1) - u.at(i, j, k + 2)) * inv12dx2[2];
+          if (H.fd_order == 8) {  // the paper's BBH discretisation: 8th-order centred, 9 points per axis
+            static const double c8[9] = {-1.0 / 560.0, 8.0 / 315.0, -1.0 / 5.0, 8.0 / 5.0, -205.0 / 72.0,
+                                         8.0 / 5.0,    -1.0 / 5.0,  8.0 / 315.0, -1.0 / 560.0};
+            double sx = 0.0, sy = 0.0, sz = 0.0;
+            for (int m = -4; m <= 4; ++m) {
+              sx += c8[m + 4] * u.at(i + m, j, k);
+              sy += c8[m + 4] * u.at(i, j + m, k);
+              sz += c8[m + 4] * u.at(i, j, k + m);
+            }
+            double src8 = 0.0;
+            if (!H.A.empty())
+              for (int q = 0; q < F; ++q) src8 += H.A[size_t(f) * F + q] * Y[q].at(i, j, k);
+            ku.at(i, j, k) = rho.at(i, j, k);
+            kr.at(i, j, k) = sx * 12.0 * inv12dx2[0] + sy * 12.0 * inv12dx2[1] + sz * 12.0 * inv12dx2[2] + src8;
+            continue;
+          }
           double src = 0.0;
           if (!H.A.empty())
             for (int q = 0; q < F; ++q) src += H.A[size_t(f) * F + q] * Y[q].at(i, j, k);
@@ -604,11 +622,23 @@ void oc_destroy(void* h) { delete static_cast<Hier*>(h); }
 // Kreiss-Oliger strength sigma of eq (36); needs ghost width >= 3. Returns 0, or -1 with oc_last_error set.
 int oc_set_dissipation(void* h, double sigma) {
   Hier* H = static_cast<Hier*>(h);
-  if (!H || !(sigma >= 0.0) || (sigma != 0.0 && H->g < 3)) {
+  if (!H || !(sigma >= 0.0) || (sigma != 0.0 && (H->g < 3 || H->fd_order != 4))) {
     snprintf(g_err, sizeof g_err, "dissipation needs sigma >= 0 and ghost width >= 3");
     return -1;
   }
   H->sigma = sigma;
+  return 0;
+}
+
+// Order of the centred finite differences of the RHS: 4 (default, S2) or 8 (reads 4 ghost layers;
+// without dissipation: eq (36) with r = 8 would read 5). Returns 0, or -1 with oc_last_error set.
+int oc_set_fd_order(void* h, int order) {
+  Hier* H = static_cast<Hier*>(h);
+  if (!H || (order != 4 && order != 8) || (order == 8 && (H->g < 4 || H->sigma != 0.0))) {
+    snprintf(g_err, sizeof g_err, "fd order must be 4, or 8 with ghost width >= 4 and no dissipation");
+    return -1;
+  }
+  H->fd_order = order;
   return 0;
 }
 

@@ -84,6 +84,7 @@ class Workload:
     init: Optional[Callable[["Workload", int, int, int], np.ndarray]] = None
     note: str = ""
     ko_sigma: float = 0.0                      # Kreiss-Oliger strength (eqs 35-36); 0 = none
+    fd_order: int = 4                          # centred finite differences of the RHS: 4 (S2) or 8 (ghost >= 4)
 
     @property
     def nlevels(self) -> int:
