@@ -66,6 +66,10 @@ typedef struct {
  *   d_t y -> RHS + Q y,  Q y = sigma/64 sum_i delta_i^6 y / h_i  (eqs 35-36 with r = 4);
  *   needs ghost >= 3. With sigma > 0 the step runs the general stage-by-stage kernels (the stage vectors' u parts
  *   are stored: 5 more arrays per field), with sigma = 0 the two-launch formulation of DESIGN.md section 6.
+ * fd_order: 8 selects the paper's BBH discretisation, the 9-point second difference
+ *   (-1/560, 8/315, -1/5, 8/5, -205/72, ...)/h^2 per axis; needs ghost >= 4 and ko_sigma = 0 (eq 36 with r = 8 would
+ *   read 5 layers) -> SC_ERR_UNSUPPORTED otherwise. The prolongation and restriction operators are unchanged (S3, S4).
+ *   Runs on the plain one-thread-per-cell stage kernel (the TMA z-march is written for radius 2).
  * arena: optional DEVICE memory of at least sc_arena_bytes() bytes, 256-byte aligned, owned by the
  *   caller, who keeps it alive and does not touch it until sc_destroy; NULL -> the library allocates.
  * cuda_stream: a cudaStream_t (as void*) on which all work of this hierarchy is enqueued (must not be
@@ -85,6 +89,7 @@ typedef struct {
   uint64_t arena_bytes;
   void* cuda_stream;
   double ko_sigma;         /* Kreiss-Oliger strength sigma >= 0; 0 = none */
+  int32_t fd_order;        /* centred differences of the RHS: 0 or 4 -> 4th order (S2); 8 -> 8th order           */
 } sc_hierarchy_desc;
 
 typedef struct sc_hierarchy sc_hierarchy; /* opaque; created by sc_create_hierarchy, freed by sc_destroy */

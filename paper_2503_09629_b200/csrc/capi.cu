@@ -197,6 +197,7 @@ void stage_level(Seq& q, int level, int mode, double dt) {
     a.b = L.boxes[ib].v;
     a.F = L.F;
     a.mode = mode;
+    a.fd_order = L.fd_order;
     // the slope k_4 (= Y4r) is kept only where a child level reads it for its dense-output ghosts
     a.write_Y4r = (q.sub && level + 1 < L.nlevels) ? 1 : 0;
     a.a_yn = L.a_state(yn);

@@ -29,7 +29,7 @@ void select_kernels(int mode) { g_mode = mode; }
 int selected_kernels() { return g_mode; }
 
 int launch_stage(const StageArgs& a, cudaStream_t st) {
-  if (g_mode == 0) { launch_stage_direct(a, st); return 1; }
+  if (g_mode == 0 || a.fd_order == 8) { launch_stage_direct(a, st); return 1; }  // the z-march is radius 2 only
   return launch_stage_tma(a, st);
 }
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {

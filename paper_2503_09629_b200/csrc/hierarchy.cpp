@@ -49,7 +49,13 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
   if (d->ko_sigma > 0.0 && d->ghost < 3)
     return fail(err, SC_ERR_UNSUPPORTED, "Kreiss-Oliger dissipation reads 3 ghost layers (ghost = %d)", d->ghost);
 
+  if (d->fd_order != 0 && d->fd_order != 4 && d->fd_order != 8)
+    return fail(err, SC_ERR_UNSUPPORTED, "fd_order must be 4 or 8 (got %d)", d->fd_order);
+  if (d->fd_order == 8 && (d->ghost < 4 || d->ko_sigma > 0.0))
+    return fail(err, SC_ERR_UNSUPPORTED, "8th-order differences read 4 ghost layers (ghost = %d) and run without dissipation", d->ghost);
+
   L->nlevels = d->nlevels;
+  L->fd_order = d->fd_order == 8 ? 8 : 4;
   L->ko_sigma = d->ko_sigma;
   L->g = d->ghost;
   L->F = d->nfields;

@@ -29,6 +29,7 @@ struct StageArgs {
   BoxView b;
   int F;
   int mode;
+  int fd_order;        // 4: 13-point Laplacian (S2); 8: 25-point, direct-load kernel only
   int write_Y4r;
   const double* yn;    // (h) state slot of y_n: u_f at f*vol (h), rho_f at (F+f)*vol ((h) in STAGE_12)
   double* Y2r;         // F arrays: written by STAGE_12, read (h) by STAGE_34

@@ -78,13 +78,22 @@ __device__ inline bool shell_cell(const BoxView& b, long long q, int& i, int& j,
 // does not take.
 // ------------------------------------------------------------------------------------------------
 namespace {
-// 13-point 4th-order Laplacian of W = u + c r at one cell (S2); c == 0 -> r is not read
-template <bool WITH_R>
+// Laplacian of W = u + c r at one cell; c == 0 -> r is not read. ORDER 4: 13 points (S2), weights w = 1/(12 dx^2);
+// ORDER 8: 25 points, (-1/560, 8/315, -1/5, 8/5, -205/72, ...)/dx^2 per axis.
+template <bool WITH_R, int ORDER>
 __device__ __forceinline__ double lap_w(const double* u, const double* r, double c, long long sy, long long sz,
                                         const double w[3], double* centre) {
   auto W = [&](long long d) { return WITH_R ? fma(c, r[d], u[d]) : u[d]; };
   const double wc = W(0);
   *centre = wc;
+  if (ORDER == 8) {
+    constexpr double c1 = 8.0 / 5.0, c2 = -1.0 / 5.0, c3 = 8.0 / 315.0, c4 = -1.0 / 560.0, c0 = -205.0 / 72.0;
+    auto d2 = [&](long long s) {
+      return c4 * (W(-4 * s) + W(4 * s)) + c3 * (W(-3 * s) + W(3 * s)) + c2 * (W(-2 * s) + W(2 * s)) +
+             c1 * (W(-s) + W(s)) + c0 * wc;
+    };
+    return 12.0 * (w[0] * d2(1) + w[1] * d2(sy) + w[2] * d2(sz));
+  }
   const double dxx = (-W(-2) + 16.0 * W(-1) - 30.0 * wc + 16.0 * W(1) - W(2)) * w[0];
   const double dyy = (-W(-2 * sy) + 16.0 * W(-sy) - 30.0 * wc + 16.0 * W(sy) - W(2 * sy)) * w[1];
   const double dzz = (-W(-2 * sz) + 16.0 * W(-sz) - 30.0 * wc + 16.0 * W(sz) - W(2 * sz)) * w[2];
@@ -92,6 +101,7 @@ __device__ __forceinline__ double lap_w(const double* u, const double* r, double
 }
 }  // namespace
 
+template <int ORDER>
 __global__ void __launch_bounds__(256) stage_direct(StageArgs a) {
   const BoxView& b = a.b;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -120,13 +130,13 @@ __global__ void __launch_bounds__(256) stage_direct(StageArgs a) {
   double wc;
   if (a.mode == STAGE_12) {
     const double* rhoarr = a.yn + (long long)F * b.vol;
-    const double Lu = lap_w<false>(u, u, 0.0, sy, sz, a.inv12dx2, &wc) + couple(0.0, nullptr);
-    const double L2 = lap_w<true>(u, rhoarr + fo, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt, rhoarr);
+    const double Lu = lap_w<false, ORDER>(u, u, 0.0, sy, sz, a.inv12dx2, &wc) + couple(0.0, nullptr);
+    const double L2 = lap_w<true, ORDER>(u, rhoarr + fo, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt, rhoarr);
     a.Y2r[fo] = fma(0.5 * dt, Lu, rho);
     a.Y3r[fo] = fma(0.5 * dt, L2, rho);
   } else {
-    const double L3 = lap_w<true>(u, a.Y2r + fo, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt, a.Y2r);
-    const double k4r = lap_w<true>(u, a.Y3r + fo, dt, sy, sz, a.inv12dx2, &wc) + couple(dt, a.Y3r);
+    const double L3 = lap_w<true, ORDER>(u, a.Y2r + fo, 0.5 * dt, sy, sz, a.inv12dx2, &wc) + couple(0.5 * dt, a.Y2r);
+    const double k4r = lap_w<true, ORDER>(u, a.Y3r + fo, dt, sy, sz, a.inv12dx2, &wc) + couple(dt, a.Y3r);
     const double y2 = a.Y2r[fo], y3 = a.Y3r[fo], y4 = fma(dt, L3, rho);
     const double third = 1.0 / 3.0;
     a.ynew[fo] = fma(dt / 6.0, (rho + y4) + 2.0 * (y2 + y3), u[0]);
@@ -139,7 +149,8 @@ __global__ void __launch_bounds__(256) stage_direct(StageArgs a) {
 void launch_stage_direct(const StageArgs& a, cudaStream_t st) {
   dim3 blk(64, 4, 1);
   dim3 grd((a.b.n[0] + 63) / 64, (a.b.n[1] + 3) / 4, a.b.n[2] * a.F);
-  stage_direct<<<grd, blk, 0, st>>>(a);
+  if (a.fd_order == 8) stage_direct<8><<<grd, blk, 0, st>>>(a);
+  else stage_direct<4><<<grd, blk, 0, st>>>(a);
 }
 
 // ------------------------------------------------------------------------------------------------

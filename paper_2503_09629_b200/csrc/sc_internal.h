@@ -76,6 +76,7 @@ struct Layout {
   unsigned long long arena_bytes = 0;
   bool has_coupling = false;
   double ko_sigma = 0.0;                    // > 0: Kreiss-Oliger dissipation, general stage-by-stage path
+  int fd_order = 4;                         // 4 (S2) or 8: centred differences of the RHS
   double dx(int level, int a) const { return (xhi[a] - xlo[a]) / ((double)domain[a] * (double)(1u << level)); }
   // first array index of each role
   int a_state(int slot) const { return slot * V; }

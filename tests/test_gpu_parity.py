@@ -469,3 +469,54 @@ def test_debug_max_abs():
     G.sc_set_state(1, 0, 0, a)
     assert np.isnan(G.sc_debug_max_abs(1, 0, 0))
     G.close()
+
+
+# ---- NEXT-3: 8th-order centred differences on the plain stage kernel ----------------------------
+def _fd8(w):
+    w.ghost, w.fd_order = 4, 8
+    w.name += " + 8th-order FD"
+    return w
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_fd8_parity(sub):
+    """cfg 1 (8 steps) and the ragged coupled multi-box hierarchy with 8th-order differences (ghost width 4)."""
+    for w in (_fd8(wl.cfg1()), _fd8(wl.ragged_small())):
+        G, O = _pair(w)
+        for _ in range(w.coarse_steps):
+            G.sc_step(w.dt_coarse, sub)
+            O.step(w.dt_coarse, sub)
+        _compare_state(G, O, w, what=f"{w.name} sub={sub}")
+        G.close()
+
+
+def test_fd8_closed_forms_without_the_oracle():
+    """The CUDA path against closed forms: the exact quadratic solution through 3 levels, and the one-level plane
+    wave whose error is RK4's omega T (omega dt)^4 / 120 once the differences are 8th order."""
+    n = 64
+    w = wl.Workload("quadratic fd8", wl.nested_cubes(3, n), (n, n, n), init=wl.quadratic_init, ghost=4, fd_order=8)
+    G = sc.Hierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, True)
+    for l in (1, 2):
+        for c in (0, 1):
+            got = G.sc_debug_read_padded(l, 0, c)
+            assert np.max(np.abs(got - wl.quadratic_exact(w, l, 0, c, w.dt_coarse, pad=4))) < 5e-12, (l, c)
+    G.close()
+    base = wl.cfg2(32)
+    one = wl.Workload("one level fd8", base.boxes[:1], base.domain_cells, init=wl.plane_wave_init, ghost=4, fd_order=8)
+    G = sc.Hierarchy.from_workload(one)
+    for _ in range(base.coarse_steps):
+        G.sc_step(one.dt_coarse, True)
+    om = np.sqrt(3.0) * np.pi
+    model = om * (om * one.dt_coarse) ** 4 / 120.0
+    e = np.max(np.abs(G.sc_read_level(0, 0, 0) - wl.plane_wave_exact(one, 0, 0, 0, 1.0)))
+    assert 0.7 * model < e < 1.3 * model, (e, model)
+    G.close()
+
+
+def test_fd8_needs_four_ghost_layers_and_no_dissipation():
+    w = wl.cfg1()
+    with pytest.raises(sc.SubcycleError):
+        sc.Hierarchy(w.boxes, w.domain_cells, ghost=3, fd_order=8)
+    with pytest.raises(sc.SubcycleError):
+        sc.Hierarchy(w.boxes, w.domain_cells, ghost=4, fd_order=8, ko_sigma=0.1)

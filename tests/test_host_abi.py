@@ -94,6 +94,10 @@ def test_nesting_validator_rejects_bad_hierarchies(built):
     assert rc(base, ref_ratio=4)[0] == SC_ERR_UNSUPPORTED
     assert rc(base, ghost=1)[0] == SC_ERR_UNSUPPORTED
     assert rc(base, ghost=5)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, fd_order=8)[0] == SC_ERR_UNSUPPORTED            # 8th-order differences read 4 ghost layers
+    assert rc(base, fd_order=6)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, ghost=4, fd_order=8, ko_sigma=0.1)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, ghost=4, fd_order=8)[0] != SC_ERR_UNSUPPORTED
     assert rc(base, nfields=0)[0] == SC_ERR_UNSUPPORTED
     assert rc(base, xlo=(1.0, -1.0, -1.0), xhi=(1.0, 1.0, 1.0))[0] == SC_ERR_INVALID_ARG
     r, msg = rc(base + [B(1, (6, 16, 16), (16, 16, 16))])
