@@ -757,7 +757,10 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
     if (h->L.boxes[ib].level == 0) continue;
     std::vector<GhostTile> tl;
-    build_ghost_tiles(h->L.boxes[ib].v, h->L.boxes[h->L.boxes[ib].parent].v, tl);
+    std::vector<BoxView> sibs;
+    for (int jb : h->L.level_boxes[h->L.boxes[ib].level])
+      if (jb != (int)ib) sibs.push_back(h->L.boxes[jb].v);
+    build_ghost_tiles(h->L.boxes[ib].v, h->L.boxes[h->L.boxes[ib].parent].v, tl, &sibs);
     sc_hierarchy::BoxTiles& bt = h->tiles[ib];
     bt.n = (int)tl.size();
     if (tl.empty()) continue;

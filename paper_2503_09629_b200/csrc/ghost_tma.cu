@@ -437,12 +437,20 @@ GhostTile make_tile(const BoxView& ch, const BoxView& pa, int axT, const int lo[
 // LEVEL-GLOBAL index: the parent footprint of an x-extended tile then starts at an even parent x index,
 // i.e. on a 16-byte boundary (XOFF and lo are even) — a TMA tiled load whose innermost fp64 coordinate is
 // odd faults on sm_100a ("illegal instruction", measured).
-void build_ghost_tiles(const BoxView& ch, const BoxView& pa, std::vector<GhostTile>& tiles) {
+void build_ghost_tiles(const BoxView& ch, const BoxView& pa, std::vector<GhostTile>& tiles,
+                       const std::vector<BoxView>* siblings) {
   tiles.clear();
   const int g = ch.g;
   std::vector<Piece> as, bs;
   auto push = [&](int ax, int l0, int l1, int l2, int n0, int n1, int n2, int o0, int o1, int o2) {
     const int lo[3] = {l0, l1, l2}, n[3] = {n0, n1, n2}, org[3] = {o0, o1, o2};
+    if (siblings)
+      for (const BoxView& s : *siblings) {
+        bool inside = true;
+        for (int a = 0; a < 3; ++a)
+          if (ch.lo[a] + lo[a] < s.lo[a] || ch.lo[a] + lo[a] + n[a] > s.lo[a] + s.n[a]) inside = false;
+        if (inside) return;  // the exchange supplies every cell of this tile
+      }
     tiles.push_back(make_tile(ch, pa, ax, lo, n, org));
   };
   // z-slabs: A = x over the padded extent, B = y over the padded extent

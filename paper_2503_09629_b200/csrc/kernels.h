@@ -126,7 +126,10 @@ struct GhostArgs {
   const void* tmaps;          // host pointer to the parent's three footprint CUtensorMaps (thin axis x, y, z;
                               // 128 bytes each, contiguous), or null -> direct-load kernel
 };
-void build_ghost_tiles(const BoxView& child, const BoxView& parent, std::vector<GhostTile>& tiles);
+// `siblings`: the other boxes of the child's level; a tile whose cells ALL lie in the interior of one sibling is
+// left out (the same-level exchange a7 overwrites every one of them right after the fill).
+void build_ghost_tiles(const BoxView& child, const BoxView& parent, std::vector<GhostTile>& tiles,
+                       const std::vector<BoxView>* siblings = nullptr);
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st);
 
 // a4: periodic ghost fill of `narrays` consecutive arrays of the level-0 box (reading S9).
