@@ -8,6 +8,7 @@
 namespace sc {
 
 void launch_stage_direct(const StageArgs& a, cudaStream_t st);
+void launch_stage_fd8(const StageArgs& a, cudaStream_t st);
 int launch_stage_tma(const StageArgs& a, cudaStream_t st);
 bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned box[4], int l2_promotion,
                              bool swizzle64, void* out_map128);
@@ -29,7 +30,8 @@ void select_kernels(int mode) { g_mode = mode; }
 int selected_kernels() { return g_mode; }
 
 int launch_stage(const StageArgs& a, cudaStream_t st) {
-  if (g_mode == 0 || a.fd_order == 8) { launch_stage_direct(a, st); return 1; }  // the z-march is radius 2 only
+  if (g_mode == 0) { launch_stage_direct(a, st); return 1; }
+  if (a.fd_order == 8) { launch_stage_fd8(a, st); return 1; }  // the TMA z-march is radius 2 only
   return launch_stage_tma(a, st);
 }
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {
