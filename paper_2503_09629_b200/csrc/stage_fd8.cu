@@ -1,17 +1,19 @@
 // stage_fd8.cu — the two RK4 stage kernels (kernels.h: STAGE_12, STAGE_34) with 8th-order centred differences
 // (the paper's BBH discretisation), sm_100a. First tiled version: it replaces the
-// one-thread-per-cell kernel (stage_direct<8>, 2 x 25 global loads per cell: 660 us per 256^3 launch) at 343 us
-// (0.31 of the HBM peak); it is not yet the radius-4 counterpart of the TMA z-march of stage_tma.cu (136 us for
+// one-thread-per-cell kernel (stage_direct<8>, 2 x 25 global loads per cell: 660 us per 256^3 launch) at 331 us
+// (0.33 of the HBM peak); it is not yet the radius-4 counterpart of the TMA z-march of stage_tma.cu (136 us for
 // the 4th-order stencil). What the profile of its first version showed: half of all stall samples sat on the FMA
 // that formed an operand right after its global load — the loads of the next plane must stay RAW in registers
 // until they are stored to shared memory one iteration later (625 -> 516 us), and the 80-register cap of a third
-// CTA per SM spilled the nine-slot accumulators (516 -> 343 us with two CTAs and 128 registers).
+// CTA per SM spilled the nine-slot accumulators (516 -> 343 us with two CTAs and 128 registers); interleaving the
+// two operands in shared memory halves the shared loads (343 -> 331 us).
 //
 // A CTA owns a 32 x 8 (x, y) tile of one field and marches along a z-chunk. Per arriving plane k
 //   * all threads build the two stage operands W1, W2 of the launch (kernels.h) on the tile plus a 4-cell halo
 //     in shared memory (40 x 16 cells, double-buffered by plane parity: one barrier per plane); the global loads
 //     of plane k+1 are issued before plane k is worked on and wait in registers;
-//   * each thread forms the in-plane part of the 25-point Laplacian of its cell (2 x 16 shared loads) and
+//   * each thread forms the in-plane part of the 25-point Laplacian of its cell (17 16-byte shared loads: the two
+//     operands are interleaved) and
 //     SCATTERS the z part: plane k contributes c_|d| W(k) to the nine pending outputs k-4 .. k+4, held in
 //     registers and shifted by one per plane, so the output of plane k-4 completes as plane k arrives;
 //   * the completed plane is combined with the centre-only operands exactly as in stage_direct.
@@ -32,7 +34,7 @@ __device__ __forceinline__ double c8(int d) {
 
 template <int MODE>
 __global__ void __launch_bounds__(NT8, 2) stage_fd8(StageArgs a, int chunk, int nchunks) {
-  __shared__ double sW[2][2][HY8][HX8];  // [plane parity][operand][y][x]: 20 KB
+  __shared__ double2 sW[2][HY8][HX8];  // [plane parity][y][x] -> (W1, W2): 20 KB, one 16-byte load serves both operands
   const BoxView& b = a.b;
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * BX + tx;
   const int X0 = blockIdx.x * BX, Y0 = blockIdx.y * BY;
@@ -96,10 +98,8 @@ __global__ void __launch_bounds__(NT8, 2) stage_fd8(StageArgs a, int chunk, int 
 #pragma unroll
     for (int t = 0; t < NF; ++t) {
       const int q = tid + t * NT8;
-      if (q < HX8 * HY8) {
-        (&sW[p][0][0][0])[q] = MODE == STAGE_12 ? pu[t] : fma(s1, pa[t], pu[t]);
-        (&sW[p][1][0][0])[q] = fma(s2, pb[t], pu[t]);
-      }
+      if (q < HX8 * HY8)
+        (&sW[p][0][0])[q] = make_double2(MODE == STAGE_12 ? pu[t] : fma(s1, pa[t], pu[t]), fma(s2, pb[t], pu[t]));
     }
     __syncthreads();
     if (k + 1 < z1 + R8) fetch(k + 1);
@@ -108,23 +108,27 @@ __global__ void __launch_bounds__(NT8, 2) stage_fd8(StageArgs a, int chunk, int 
       cx[0] = a.yn[(long long)(F + f) * b.vol + o];
       if (MODE == STAGE_34) { cx[1] = r1[o]; cx[2] = r2[o]; cx[3] = u[o]; }
     }
-#pragma unroll
-    for (int op = 0; op < 2; ++op) {
-      const double* __restrict__ s = &sW[p][op][ty + R8][tx + R8];
-      double(&acc)[9] = op ? acc2 : acc1;
-      const double wc = s[0];
-      double dx = 0.0, dy = 0.0;
+    {
+      const double2* __restrict__ s = &sW[p][ty + R8][tx + R8];
+      const double2 wc = s[0];
+      double2 dx = make_double2(0.0, 0.0), dy = dx;
 #pragma unroll
       for (int d = 1; d <= R8; ++d) {
-        dx = fma(c8(d), s[-d] + s[d], dx);
-        dy = fma(c8(d), s[-d * HX8] + s[d * HX8], dy);
+        const double2 xm = s[-d], xp = s[d], ym = s[-d * HX8], yp = s[d * HX8];
+        dx.x = fma(c8(d), xm.x + xp.x, dx.x);
+        dx.y = fma(c8(d), xm.y + xp.y, dx.y);
+        dy.x = fma(c8(d), ym.x + yp.x, dy.x);
+        dy.y = fma(c8(d), ym.y + yp.y, dy.y);
       }
-      acc[4] += fma(wx, dx, fma(wy, dy, ccen * wc));
+      acc1[4] += fma(wx, dx.x, fma(wy, dy.x, ccen * wc.x));
+      acc2[4] += fma(wx, dx.y, fma(wy, dy.y, ccen * wc.y));
 #pragma unroll
       for (int d = 1; d <= R8; ++d) {
-        const double t = wzc[d] * wc;
-        acc[4 - d] += t;
-        acc[4 + d] += t;
+        const double t1 = wzc[d] * wc.x, t2 = wzc[d] * wc.y;
+        acc1[4 - d] += t1;
+        acc1[4 + d] += t1;
+        acc2[4 - d] += t2;
+        acc2[4 + d] += t2;
       }
     }
     const int kz = k - R8;  // the plane whose Laplacians are now complete
