@@ -60,19 +60,36 @@ def measured_peaks():
 # reference arm / cpu_baseline: the oracle as it stands on the host cores, bounded sample
 # ------------------------------------------------------------------------------------------------
 def oracle_sample(w, max_levels: int):
-    """The first `max_levels` levels of the workload (same boxes, same inputs)."""
+    """The first `max_levels` levels of the workload (same boxes, same inputs, same discretisation)."""
     if w.nlevels <= max_levels:
         return w, f"all {w.nlevels} levels"
     boxes = [b for b in w.boxes if b.level < max_levels]
     s = wl.Workload(w.name + f" [levels 0..{max_levels - 1}]", boxes, w.domain_cells, w.nfields, w.ghost,
-                    w.xlo, w.xhi, w.coupling, w.coarse_steps, w.init, ko_sigma=w.ko_sigma)
-    return s, f"levels 0..{max_levels - 1} of {w.nlevels} ({'+'.join(str(b.n[0]) + '^3' for b in boxes)})"
+                    w.xlo, w.xhi, w.coupling, w.coarse_steps, w.init, ko_sigma=w.ko_sigma, fd_order=w.fd_order)
+    for k in ("integrator", "boundary", "ko_order", "interp_order"):  # options added after round 1, if present
+        if hasattr(w, k):
+            setattr(s, k, getattr(w, k))
+    return s, f"SAMPLE: levels 0..{max_levels - 1} of {w.nlevels} ({'+'.join(str(b.n[0]) + '^3' for b in boxes)})"
 
 
-def time_oracle(w, steps: int, warmup: int, sub: bool, max_levels: int):
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def time_oracle(w, steps: int, warmup: int, sub: bool, max_levels: int, threads: int = 0):
+    """The oracle as it stands on `threads` host threads (0 = all), on a bounded sample of the workload."""
     import oracle
 
     oracle.build()
+    allthreads = oracle.max_threads()
+    if threads > 0:
+        oracle.set_threads(threads)
     s, what = oracle_sample(w, max_levels)
     H = oracle.OracleHierarchy.from_workload(s)
     for _ in range(warmup):
@@ -81,10 +98,24 @@ def time_oracle(w, steps: int, warmup: int, sub: bool, max_levels: int):
     for _ in range(steps):
         H.step(s.dt_coarse, sub)
     dt = time.perf_counter() - t0
+    used = oracle.max_threads()
+    H.close()
+    if threads > 0:
+        oracle.set_threads(allthreads)
     upd = s.updates_per_coarse_step(sub) * steps
-    return {"value": upd / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+    return {"value": upd / dt, "unit": UNIT, "cores": used, "kind": "oracle", "cpu": cpu_model(),
+            "flags": "g++ -O2 -fopenmp, no fast-math",
             "sample": f"{what}, {steps} coarse step(s), {'subcycled' if sub else 'uniform'}, {dt:.1f} s",
             "_seconds": dt, "_steps": steps}
+
+
+def config_dict(w, sub: bool, world: int):
+    """The `config` object of the JSON line; the same for the GPU arm and the reference arm."""
+    return {"workload": w.name, "mode": "subcycled" if sub else "uniform", "ghost": w.ghost, "nfields": w.nfields,
+            "ko_sigma": w.ko_sigma, "fd_order": w.fd_order, "dt_coarse": w.dt_coarse,
+            "updates_per_step": w.updates_per_coarse_step(sub), "zone_cycles_per_step": w.zone_cycles_per_coarse_step(),
+            "l2": "inputs larger than L2 (state and stage buffers of every level stream through once per launch)",
+            "parallelism": "replicas only" if world > 1 else "1 GPU"}
 
 
 def run_reference(args):
@@ -98,7 +129,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "mode": args.mode, "note": "CPU oracle on a bounded sample"},
+            "config": config_dict(w, sub, 1),
+            "note": "CPU oracle (as it stands, all host threads) on a bounded SAMPLE of the workload: " + r["sample"],
             "cpu_baseline": r,
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -242,10 +274,43 @@ def run_gpu(args):
     H.sc_profile(False)
     dom = max(kinds, key=lambda k: kinds[k]["ms_total"])
     ksum = sum(k["ms_total"] for k in kinds.values())
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["algorithmic_GBps"], "peak": peak,
-                "unit": "GB/s", "frac": kinds[dom]["frac"], "traffic": TRAFFIC.get(dom) if args.config == 5 and not args.sigma and args.cut_finest == 1 and args.fd_order == 4 else None,
-                "peak_source": peak_src, "frac_of_nominal_8TBps": kinds[dom]["algorithmic_GBps"] / 8000.0, "share_of_step": kinds[dom]["ms_total"] / ksum,
-                "bytes_per_launch": kinds[dom]["bytes_per_launch"], "avg_launch_us": kinds[dom]["avg_us"]}
+    wkey = f"cfg{args.config}/{args.mode}/sigma{args.sigma:g}/cut{args.cut_finest}/fd{args.fd_order}"
+
+    def roof(kind):
+        k = kinds[kind]
+        tr = ncu_traffic(kind, wkey)
+        return {"bound": "hbm", "kernel": kind, "achieved": k["algorithmic_GBps"], "peak": peak, "unit": "GB/s",
+                "frac": k["frac"], "traffic": tr["bytes_per_launch"] if tr else None,
+                "traffic_source": tr["source"] if tr else "no ncu --set full capture of this kernel source under profiles/",
+                "peak_source": peak_src, "frac_of_nominal_8TBps": k["algorithmic_GBps"] / 8000.0,
+                "share_of_step": k["ms_total"] / ksum, "bytes_per_launch": k["bytes_per_launch"],
+                "avg_launch_us": k["avg_us"]}
+    roofline = roof(dom)
+    # north_star sets a bar on the ghost-fill kernel as well: its roofline entry next to the dominant kernel's
+    roofline_ghost = roof("ghost_dense_prolong") if "ghost_dense_prolong" in kinds else None
+
+    # ---- the OTHER mode in the same run: north_star's bar "subcycling beats the non-subcycled hierarchy step by at
+    # least the level-work ratio minus 15 %" (read as 0.85 x ratio, and as ratio - 0.15) ------------------
+    other = None
+    if args.other_mode_steps > 0:
+        osub = not sub
+        for _ in range(3):
+            H.sc_step(dt, osub)
+        barrier()
+        o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        o0.record(st)
+        for _ in range(args.other_mode_steps):
+            H.sc_step(dt, osub)
+        o1.record(st)
+        barrier()
+        oms = max_over_ranks(o0.elapsed_time(o1), dist, f"cuda:{local}") / args.other_mode_steps
+        ms_sub = ms_total / args.steps if sub else oms
+        ms_uni = oms if sub else ms_total / args.steps
+        ratio = w.updates_per_coarse_step(False) / w.updates_per_coarse_step(True)
+        other = {"ms_per_step_subcycled": ms_sub, "ms_per_step_uniform": ms_uni, "uniform_steps_timed": args.other_mode_steps if sub else args.steps,
+                 "speedup_vs_uniform": ms_uni / ms_sub, "level_work_ratio": ratio,
+                 "bar_0.85_x_ratio": 0.85 * ratio, "bar_ratio_minus_0.15": ratio - 0.15,
+                 "meets_bar": bool(ms_uni / ms_sub >= max(0.85 * ratio, ratio - 0.15))}
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the whole state, step, D2H ---------
     for k, t in host_in.items():
@@ -276,18 +341,18 @@ def run_gpu(args):
     if world == 1 and not args.no_cpu_baseline:
         cpu = time_oracle(w, 1, 0, sub, max_levels=args.oracle_levels)
         cpu.pop("_seconds"), cpu.pop("_steps")
+        if not args.no_cpu_1thread:  # one thread and all threads
+            one = time_oracle(w, 1, 0, sub, max_levels=args.oracle_levels, threads=1)
+            cpu["value_1thread"] = one["value"]
+            cpu["sample_1thread"] = one["sample"]
 
     # model bytes of the whole step for the whole-step roofline fraction
     step_bytes = sum(k["bytes_per_launch"] * k["launches"] for k in kinds.values()) / max(1, min(args.steps, 2))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "mode": "subcycled" if sub else "uniform", "ghost": w.ghost,
-                       "nfields": w.nfields, "ko_sigma": w.ko_sigma, "dt_coarse": dt, "updates_per_step": upd_step,
-                       "zone_cycles_per_step": w.zone_cycles_per_coarse_step(),
-                       "l2": "inputs larger than L2 (state + stage buffers %.1f GB)" % (H.arena_bytes / 1e9),
-                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "config": config_dict(w, sub, world), "arena_GB": H.arena_bytes / 1e9,
+            "roofline": roofline, "roofline_ghost": roofline_ghost, "sub_vs_uniform": other, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
             "kernels": kinds, "zone_cycles_per_s": world * w.zone_cycles_per_coarse_step() * args.steps / (ms_total * 1e-3),
             "step_algorithmic_GB": step_bytes / 1e9,
             "step_roofline_frac": step_bytes / (ms_total / args.steps * 1e-3) / 1e9 / peak,
@@ -298,9 +363,28 @@ def run_gpu(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of the
-# dominant kernel (profiles/): filled in per round; None until a capture exists.
-TRAFFIC = {"rk_stage": 678.0e6}  # profiles/r01_v3.md: (298+228 + 589+240)/2 MB per 256^3 launch (cfg 5)
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of a kernel kind, from the committed
+# `ncu --set full` capture listed in profiles/traffic.csv. A row counts only while the kernel's SOURCE FILE still has
+# the hash the capture was taken with (first 16 hex digits of its sha256) and the workload key matches; otherwise the
+# line says null — a later kernel change can never carry an old figure along.
+KIND_SOURCES = {"rk_stage": "stage_tma.cu", "ghost_dense_prolong": "ghost_tma.cu", "restrict": "restrict_zmarch.cu",
+                "periodic_fill": "kernels_basic.cu"}
+
+
+def ncu_traffic(kind: str, wkey: str):
+    import csv
+    import hashlib
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    src = os.path.join(ROOT, "paper_2503_09629_b200", "csrc", KIND_SOURCES.get(kind, ""))
+    if not (os.path.exists(path) and os.path.isfile(src)):
+        return None
+    sha = hashlib.sha256(open(src, "rb").read()).hexdigest()[:16]
+    with open(path, newline="") as f:
+        for row in csv.DictReader(f):
+            if row["kind"] == kind and row["workload"] == wkey and row["source_sha256_16"] == sha:
+                return {"bytes_per_launch": float(row["dram_bytes_per_launch"]),
+                        "source": f"profiles/{row['capture']} ({row['source_file']} sha256 {sha})"}
+    return None
 
 
 def main():
@@ -315,11 +399,14 @@ def main():
     ap.add_argument("--cut-finest", type=int, default=1,
                     help="cut the finest level into this many abutting slabs that exchange ghosts (NEXT-2 variant)")
     ap.add_argument("--fd-order", type=int, default=4, choices=[4, 8],
-                    help="8: the paper's BBH discretisation (PAPER.md:125) on the plain stage kernel, ghost width 4")
+                    help="8: the paper's BBH discretisation (PAPER.md:125): 8th-order centred differences, ghost width 4")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--oracle-levels", type=int, default=2,
                     help="levels of the workload the CPU oracle is timed on (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cpu-1thread", action="store_true", help="skip the one-thread leg of cpu_baseline")
+    ap.add_argument("--other-mode-steps", type=int, default=3,
+                    help="coarse steps of the OTHER mode timed in the same run for speedup_vs_uniform (0 = skip)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3

@@ -69,7 +69,6 @@ typedef struct {
  * fd_order: 8 selects the paper's BBH discretisation, the 9-point second difference
  *   (-1/560, 8/315, -1/5, 8/5, -205/72, ...)/h^2 per axis; needs ghost >= 4 and ko_sigma = 0 (eq 36 with r = 8 would
  *   read 5 layers) -> SC_ERR_UNSUPPORTED otherwise. The prolongation and restriction operators are unchanged (S3, S4).
- *   Runs on the plain one-thread-per-cell stage kernel (the TMA z-march is written for radius 2).
  * arena: optional DEVICE memory of at least sc_arena_bytes() bytes, 256-byte aligned, owned by the
  *   caller, who keeps it alive and does not touch it until sc_destroy; NULL -> the library allocates.
  * cuda_stream: a cudaStream_t (as void*) on which all work of this hierarchy is enqueued (must not be
@@ -108,7 +107,10 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out);
  * src_on_device == 0, DEVICE otherwise. box is the box's index within its level (0-based, in the
  * order given at creation). Ghost cells are never supplied: the first stage of every level-step
  * refills them (reading S8). Enqueued on the hierarchy's stream; a host source is consumed before the
- * call returns. */
+ * call returns. A DEVICE source is read by a kernel enqueued on the hierarchy's stream and the call returns
+ * without waiting for it: the caller must (i) have made that stream wait for whatever produces src (an event
+ * or stream wait; the library knows nothing about the caller's streams) and (ii) keep src alive and unchanged
+ * until the hierarchy's stream has passed this point. The Python binding does both for torch tensors. */
 int32_t sc_set_state(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, const double* src,
                      int32_t src_on_device);
 
@@ -132,8 +134,10 @@ double sc_time(const sc_hierarchy* h);
 /* Number of kernels the library has launched (or replayed inside CUDA graphs) for this hierarchy. */
 uint64_t sc_launch_count(const sc_hierarchy* h);
 
-/* Debug: the refinement-boundary ghost index map of a level >= 1 box, computed by the same device code
- * the ghost kernel uses. For every ghost cell of the padded box, in canonical order (k, then j, then
+/* Debug: the refinement-boundary ghost index map of a level >= 1 box, computed on the device with the index
+ * arithmetic of the direct-load ghost kernel (parent = I >> 1, parity = I & 1 on level-global indices). The tuned
+ * ghost kernel works from tile descriptors built on the host with the same arithmetic; it is held to this map
+ * through the element-wise parity of every ghost value. For every ghost cell of the padded box, in canonical order (k, then j, then
  * i over [-g, n+g), skipping the interior), 7 int32: (i, j, k) box-local fine index, (pi, pj, pk)
  * parent-box-local index of the containing parent cell, and parity bits (px | py<<1 | pz<<2) where
  * p = 1 means the fine centre sits at +dx_parent/4 from the parent centre. out: HOST, cap = capacity in

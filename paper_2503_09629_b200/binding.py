@@ -194,7 +194,15 @@ class Hierarchy:
         if nel != b.n[0] * b.n[1] * b.n[2]:
             raise ValueError("sc_set_state: src must hold n[0]*n[1]*n[2] doubles")
         p, dev = self._ptr(src)
+        if dev:
+            # device source: the copy kernel runs on the hierarchy's stream. Order it after the work that produced
+            # `src` on the caller's current stream, and keep `src`'s memory from being recycled until it has run
+            # (include/subcycle.h, sc_set_state: ordering contract for device pointers).
+            import torch
+            self._stream.wait_stream(torch.cuda.current_stream(self._dev))
         _check(lib().sc_set_state(self._h, level, ibox, comp, p, dev))
+        if dev:
+            src.record_stream(self._stream)
 
     def sc_step(self, dt_coarse: float, subcycling: bool = True) -> None:
         _check(lib().sc_step(self._h, float(dt_coarse), int(bool(subcycling))))
@@ -204,6 +212,9 @@ class Hierarchy:
         if out is None:
             out = np.empty((b.n[2], b.n[1], b.n[0]), dtype=np.float64)
         p, dev = self._ptr(out)
+        if dev:  # `out` may still be in use on the caller's stream (sc_read_level itself synchronises ours)
+            import torch
+            self._stream.wait_stream(torch.cuda.current_stream(self._dev))
         _check(lib().sc_read_level(self._h, level, ibox, comp, p, dev))
         return out
 

@@ -1,10 +1,9 @@
 """GPU parity at BASELINE.json's full box sizes, in the launch configuration bench.py times.
 
-The kernels' grids, tiles, z-chunks and tensor maps depend on the BOX shape (and F), not on how many levels
-are stacked, so every kernel launch configuration of cfg 3 / 4 / 5 is exercised by a hierarchy of the same
-boxes truncated to the depth the CPU oracle finishes in seconds; those are compared element by element.
-The full-depth cfg-5 hierarchy (what bench.py times) is then checked through properties that hold at any
-size: exact homogeneity under scaling by 2 (bit-exact), reflection symmetry of symmetric data (to
+cfg 5 (6 x 256^3) and cfg 4 (7 levels x 96^3, 22 fields) are compared with the oracle element by element at
+their stated depth for one coarse step (test_cfg5_full_depth_vs_oracle, test_cfg4_full_depth_vs_oracle); the
+truncated hierarchies of the same boxes cover more steps and both modes cheaply. The full-depth cfg-5
+hierarchy (what bench.py times) is also checked through properties that hold at any size: exact homogeneity under scaling by 2 (bit-exact), reflection symmetry of symmetric data (to
 rounding), graph replay = eager launches (bit-exact), and agreement of its level-0 and level-1 data far
 from the refined region with the truncated run the oracle verified (finite propagation speed: the 13-point
 stencil moves information at most 8 cells per level-step)."""
@@ -16,22 +15,11 @@ import paper_2503_09629_b200 as sc
 from paper_2503_09629_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
-RTOL = 1e-11
+from oracle.parity import RTOL, compare_state
 
 
 def _compare_all(G, O, w, what):
-    scale = max(np.max(np.abs(O.read_level(l, ib, c))) for l in range(w.nlevels)
-                for ib in range(len(w.level_boxes(l))) for c in range(w.ncomp))
-    worst = 0.0
-    for l in range(w.nlevels):
-        for ib in range(len(w.level_boxes(l))):
-            for c in range(w.ncomp):
-                a = G.sc_debug_read_padded(l, ib, c)
-                b = O.read(l, ib, c, padded=True)
-                d = float(np.max(np.abs(a - b)))
-                worst = max(worst, d)
-                assert d <= RTOL * scale, f"{what}: level {l} box {ib} comp {c}: max|d|={d:.3e} scale={scale:.3e}"
-    return worst / scale
+    return compare_state(G, O, w, padded=True, what=what)
 
 
 @pytest.mark.parametrize("sub", [True, False])
@@ -69,6 +57,34 @@ def test_cfg4_boxes_full_fields():
     O.step(w.dt_coarse, True)
     rel = _compare_all(G, O, w, "cfg4/96 x3 F=22")
     print(f"cfg4 96^3 x 3 levels, 22 fields: max rel diff {rel:.2e}")
+    G.close()
+    O.close()
+
+
+@pytest.mark.parametrize("sub", [True, False])
+def test_cfg5_full_depth_vs_oracle(sub):
+    """BASELINE config 5 exactly as bench.py times it (6 levels x 256^3), one coarse step, against the oracle:
+    every element of every level, ghosts included (SURVEY 7.6 / BASELINE.md section 4). About 30 s (subcycled) /
+    90 s (uniform) of oracle on 16 cores and 12 GB of host memory."""
+    w = wl.cfg5()
+    G, O = sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, sub)
+    O.step(w.dt_coarse, sub)
+    rel = _compare_all(G, O, w, f"cfg5 full depth sub={sub}")
+    print(f"cfg5 6 x 256^3 sub={sub}: max|d|/max|u| = {rel:.2e}")
+    G.close()
+    O.close()
+
+
+def test_cfg4_full_depth_vs_oracle():
+    """BASELINE config 4 exactly as stated (7 levels x 96^3, the finest = two 80x96x96 boxes, 22 coupled fields),
+    one subcycled coarse step against the oracle, every element of all 44 components, ghosts included."""
+    w = wl.cfg4()
+    G, O = sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+    G.sc_step(w.dt_coarse, True)
+    O.step(w.dt_coarse, True)
+    rel = _compare_all(G, O, w, "cfg4 full depth")
+    print(f"cfg4 7 levels x 96^3, 22 fields: max|d|/max|u| = {rel:.2e}")
     G.close()
     O.close()
 
