@@ -50,6 +50,12 @@ def lib():
         L.oc_destroy.argtypes = [C.c_void_p]
         L.oc_set_dissipation.argtypes = [C.c_void_p, C.c_double]
         L.oc_set_fd_order.argtypes = [C.c_void_p, C.c_int]
+        L.oc_set_options.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.oc_interp_weights.argtypes = [C.c_int, C.c_int, ip, ip, dp, dp, ip, ip, dp]
+        L.oc_b_rk.restype = C.c_double
+        L.oc_b_rk.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double]
+        L.oc_dense_stage_rk.restype = C.c_double
+        L.oc_dense_stage_rk.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, dp]
         L.oc_set_state.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, dp]
         L.oc_read.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, dp]
         L.oc_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
@@ -90,6 +96,27 @@ def restrict_weights() -> np.ndarray:
     return r
 
 
+def b_rk(integrator: int, i: int, m: int, theta: float) -> float:
+    """m-th theta-derivative of the dense-output polynomial b_i of RK4 (4), Kutta's RK3 (3) or midpoint RK2 (2)."""
+    return lib().oc_b_rk(integrator, i, m, theta)
+
+
+def dense_stage_rk(integrator: int, stage: int, theta: float, hp: float, y_old: float, k: Sequence[float]) -> float:
+    kk = np.zeros(4)
+    kk[:len(k)] = k
+    return lib().oc_dense_stage_rk(integrator, stage, theta, hp, y_old, _dp(kk))
+
+
+def interp_weights(interp: int = 0, vertex: int = 0):
+    """(omin, w[2][np], rmin, r[nr]) of the prolongation / restriction operators (oracle.cpp: make_interp)."""
+    w0, w1, r = np.zeros(10), np.zeros(10), np.zeros(10)
+    n = (C.c_int * 4)()
+    I = C.POINTER(C.c_int)
+    at = lambda q: C.cast(C.byref(n, 4 * q), I)  # noqa: E731
+    lib().oc_interp_weights(interp, vertex, at(0), at(1), _dp(w0), _dp(w1), at(2), at(3), _dp(r))
+    return n[1], np.stack([w0[:n[0]], w1[:n[0]]]), n[3], r[:n[2]].copy()
+
+
 def set_threads(n: int) -> None:
     lib().oc_set_threads(n)
 
@@ -106,7 +133,8 @@ class OracleHierarchy:
 
     def __init__(self, boxes, domain_cells, nfields: int = 1, ghost: int = 3,
                  xlo=(-1.0, -1.0, -1.0), xhi=(1.0, 1.0, 1.0), coupling: Optional[np.ndarray] = None,
-                 ko_sigma: float = 0.0, fd_order: int = 4):
+                 ko_sigma: float = 0.0, fd_order: int = 4, integrator: int = 4, outer_bc: int = 0, ko_order: int = 0,
+                 interp: int = 0, vertex: int = 0):
         L = lib()
         self.boxes = list(boxes)
         self.nfields, self.ghost = nfields, ghost
@@ -126,15 +154,20 @@ class OracleHierarchy:
         if not self._h:
             raise ValueError("oracle: " + L.oc_last_error().decode())
         self.nlevels = nlev
-        if ko_sigma and L.oc_set_dissipation(self._h, float(ko_sigma)) != 0:
-            raise ValueError("oracle: " + L.oc_last_error().decode())
         if fd_order != 4 and L.oc_set_fd_order(self._h, int(fd_order)) != 0:
+            raise ValueError("oracle: " + L.oc_last_error().decode())
+        if (integrator, outer_bc, ko_order, interp, vertex) != (4, 0, 0, 0, 0) and \
+                L.oc_set_options(self._h, int(integrator), int(outer_bc), int(ko_order), int(interp), int(vertex)) != 0:
+            raise ValueError("oracle: " + L.oc_last_error().decode())
+        if ko_sigma and L.oc_set_dissipation(self._h, float(ko_sigma)) != 0:
             raise ValueError("oracle: " + L.oc_last_error().decode())
 
     @classmethod
     def from_workload(cls, w) -> "OracleHierarchy":
         h = cls(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling,
-                ko_sigma=getattr(w, "ko_sigma", 0.0), fd_order=getattr(w, "fd_order", 4))
+                ko_sigma=getattr(w, "ko_sigma", 0.0), fd_order=getattr(w, "fd_order", 4),
+                integrator=getattr(w, "integrator", 4), outer_bc=getattr(w, "outer_bc", 0),
+                ko_order=getattr(w, "ko_order", 0), interp=getattr(w, "interp", 0), vertex=int(getattr(w, "vertex", 0)))
         for l in range(w.nlevels):
             for ib in range(len(w.level_boxes(l))):
                 for c in range(w.ncomp):

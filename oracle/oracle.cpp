@@ -16,6 +16,10 @@
 //   Kreiss-Oliger dissipation, eqs (35)-(36) PAPER.md:194-204   -> add_dissipation()
 //   same-level ghost exchange .............. PAPER.md:20, 347   -> sibling_exchange()
 //   8th-order finite differences ........... PAPER.md:125       -> rhs() with fd_order = 8 (NEXT-3)
+//   RK2 / RK3 subcycling ................... PAPER.md:359       -> rk_level_step(), b_coeff_rk3/2(), dense_stage_rk3/2() (NEXT-4, S28)
+//   radiative (Sommerfeld) outer boundary .. PAPER.md:52, 113, 192 -> radiative_rhs() (NEXT-4, S29)
+//   ninth-order KO dissipation, r = 8 ...... PAPER.md:125, eq 36 -> add_dissipation() with ko_order = 9 (NEXT-3)
+//   interpolation that follows the stencil, vertex-centred grids with injection -> interp_* (NEXT-3, S30, S31)
 //
 // Where the paper is silent the readings S1..S24 of DESIGN.md apply (cell-centred grids S1, 4th-order
 // centred Laplacian S2, quartic Lagrange prolongation S3, quintic Lagrange restriction S4, parent-step
@@ -101,6 +105,76 @@ double dense_stage(int stage, double theta, double hp, double y_old, const doubl
 }
 
 // ---------------------------------------------------------------------------------------------
+// NEXT-4 ("extending it to RK2 and RK3 is straightforward"), reading S28. The extension repeats
+// the construction of eqs (10)-(18) for the lower-order integrators:
+//   RK3 = Kutta's third-order method:  k1 = f(Y1), k2 = f(Y2), k3 = f(Y3),
+//         Y1 = y_n,  Y2 = y_n + h/2 k1,  Y3 = y_n - h k1 + 2 h k2,  y_{n+1} = y_n + h/6 (k1 + 4 k2 + k3);
+//   RK2 = the midpoint method:         Y1 = y_n,  Y2 = y_n + h/2 k1,  y_{n+1} = y_n + h k2.
+// Dense output (the analogue of eqs 10-13: the polynomials b_i(theta) with b_i(1) = the method's weights that
+// satisfy the quadrature order conditions sum b_i = theta, sum b_i c_i = theta^2/2 and, for RK3, sum b_i c_i^2 =
+// theta^3/3; for RK3 they are eqs (11)-(13) with the two middle stages of RK4 merged, b_2^{RK3} = b_2 + b_3):
+//   RK3:  b1 = theta - 3/2 theta^2 + 2/3 theta^3,  b2 = 2 theta^2 - 4/3 theta^3,  b3 = -1/2 theta^2 + 2/3 theta^3
+//   RK2:  b1 = theta - theta^2,                    b2 = theta^2
+// Ghost stage vectors (the analogue of eqs 15-18: Taylor expansion of the child's own stage values in its step h,
+// kept to the order the integrator needs, h^2 for RK3 and h for RK2; derivatives by eq 14 from the parent):
+//   RK3:  Y1 = y,  Y2 = y + h/2 y',  Y3 = y + h y' + h^2 y''      (k2 = y' + h/2 y'' + O(h^2) in Y3 = y - h k1 + 2 h k2)
+//   RK2:  Y1 = y,  Y2 = y + h/2 y'
+// ---------------------------------------------------------------------------------------------
+double b_coeff_rk3(int i, int m, double th) {
+  switch (i) {
+    case 1:
+      if (m == 0) return th - 1.5 * th * th + (2.0 / 3.0) * th * th * th;
+      if (m == 1) return 1.0 - 3.0 * th + 2.0 * th * th;
+      if (m == 2) return -3.0 + 4.0 * th;
+      return 4.0;
+    case 2:
+      if (m == 0) return 2.0 * th * th - (4.0 / 3.0) * th * th * th;
+      if (m == 1) return 4.0 * th - 4.0 * th * th;
+      if (m == 2) return 4.0 - 8.0 * th;
+      return -8.0;
+    default:
+      if (m == 0) return -0.5 * th * th + (2.0 / 3.0) * th * th * th;
+      if (m == 1) return -th + 2.0 * th * th;
+      if (m == 2) return -1.0 + 4.0 * th;
+      return 4.0;
+  }
+}
+double b_coeff_rk2(int i, int m, double th) {
+  if (i == 1) return m == 0 ? th - th * th : (m == 1 ? 1.0 - 2.0 * th : (m == 2 ? -2.0 : 0.0));
+  return m == 0 ? th * th : (m == 1 ? 2.0 * th : (m == 2 ? 2.0 : 0.0));
+}
+// stage = 1..3 (RK3) / 1..2 (RK2): the ghost value of Y_stage; stage 5: y at `theta` by the dense output alone
+double dense_stage_rk3(int stage, double theta, double hp, double y_old, const double k[3]) {
+  double s0 = 0.0, d1 = 0.0, d2 = 0.0;
+  for (int i = 1; i <= 3; ++i) {
+    s0 += b_coeff_rk3(i, 0, theta) * k[i - 1];
+    d1 += b_coeff_rk3(i, 1, theta) * k[i - 1];
+    d2 += b_coeff_rk3(i, 2, theta) * k[i - 1];
+  }
+  const double y = y_old + hp * s0;  // the analogue of eq (10)
+  d2 = d2 / hp;                      // eq (14), m = 2
+  if (stage == 1 || stage == 5) return y;
+  const double h = 0.5 * hp;  // child step
+  if (stage == 2) return y + 0.5 * h * d1;
+  return y + h * d1 + h * h * d2;
+}
+double dense_stage_rk2(int stage, double theta, double hp, double y_old, const double k[2]) {
+  double s0 = 0.0, d1 = 0.0;
+  for (int i = 1; i <= 2; ++i) {
+    s0 += b_coeff_rk2(i, 0, theta) * k[i - 1];
+    d1 += b_coeff_rk2(i, 1, theta) * k[i - 1];
+  }
+  const double y = y_old + hp * s0;
+  if (stage == 1 || stage == 5) return y;
+  return y + 0.5 * (0.5 * hp) * d1;
+}
+double dense_stage_any(int integrator, int stage, double theta, double hp, double y_old, const double* k) {
+  if (integrator == 3) return dense_stage_rk3(stage, theta, hp, y_old, k);
+  if (integrator == 2) return dense_stage_rk2(stage, theta, hp, y_old, k);
+  return dense_stage(stage, theta, hp, y_old, k);
+}
+
+// ---------------------------------------------------------------------------------------------
 // spatial operators
 // ---------------------------------------------------------------------------------------------
 
@@ -126,6 +200,45 @@ void prolong_weights(int parity, double w[5]) {
 void restrict_weights(double r[6]) {
   const double nodes[6] = {-2.5, -1.5, -0.5, 0.5, 1.5, 2.5};
   lagrange_weights(nodes, 6, 0.0, r);
+}
+
+// NEXT-3 variants of the two operators (readings S30, S31). `interp` = 0: the operators above (S3, S4);
+// 1: operators whose order follows the 8th-order stencil of PAPER.md:125 (9-point prolongation, 10-point
+// restriction). `vertex` = 1: vertex-centred grids (grid point i of level l sits at xlo + i dx_l): fine point 2J
+// coincides with parent point J, so restriction is INJECTION and even fine points copy their parent; odd fine
+// points 2J+1 sit midway between parents J and J+1 and take the Lagrange interpolant through parents J-2..J+3
+// (interp 0, sextic-accurate) or J-4..J+5 (interp 1). All weights from the Lagrange formula.
+struct Interp {
+  int np = 5, omin = -2;   // prolongation: parent offsets omin .. omin + np - 1 around J = floor(I / 2)
+  double w[2][10];         // [parity of the fine index][offset - omin]
+  int nr = 6, rmin = -2;   // restriction: fine offsets rmin .. rmin + nr - 1 around 2J
+  double r[10];
+  int reach() const { return std::max(-omin, omin + np - 1); }  // parent cells the footprint extends beyond J
+};
+Interp make_interp(int interp, int vertex) {
+  Interp P;
+  double nodes[10];
+  if (!vertex) {
+    P.np = interp ? 9 : 5;
+    P.omin = -(P.np / 2);
+    for (int m = 0; m < P.np; ++m) nodes[m] = double(P.omin + m);
+    lagrange_weights(nodes, P.np, -0.25, P.w[0]);
+    lagrange_weights(nodes, P.np, +0.25, P.w[1]);
+    P.nr = interp ? 10 : 6;
+    P.rmin = -(P.nr / 2 - 1);
+    // fine cell 2J + q has its centre at (q - 1/2) fine spacings from the parent centre J
+    for (int m = 0; m < P.nr; ++m) nodes[m] = double(P.rmin + m) - 0.5;
+    lagrange_weights(nodes, P.nr, 0.0, P.r);
+  } else {
+    P.np = interp ? 10 : 6;
+    P.omin = -(P.np / 2 - 1);
+    for (int m = 0; m < P.np; ++m) { nodes[m] = double(P.omin + m); P.w[0][m] = (P.omin + m == 0) ? 1.0 : 0.0; }
+    lagrange_weights(nodes, P.np, 0.5, P.w[1]);
+    P.nr = 1;
+    P.rmin = 0;
+    P.r[0] = 1.0;
+  }
+  return P;
 }
 
 inline int floor_div2(int a) { return (a >= 0) ? a / 2 : -((-a + 1) / 2); }
@@ -163,6 +276,11 @@ struct Hier {
   std::vector<double> A;  // F*F coupling or empty
   double sigma = 0.0;     // Kreiss-Oliger dissipation strength (eqs 35-36); 0 = none
   int fd_order = 4;       // order of the centred finite differences of the RHS: 4 (S2) or 8 (NEXT-3)
+  int ko_order = 5;       // 5: delta^6 (eq 36 with r = 4); 9: delta^10 (eq 36 with r = 8, "ninth-order")
+  int integrator = 4;     // 4: RK4 (eqs 1-9); 3: Kutta's RK3; 2: midpoint RK2
+  int outer_bc = 0;       // level 0: 0 = periodic (S9); 1 = radiative / Sommerfeld
+  int interp = 0, vertex = 0;  // interpolation operators and grid centring (make_interp)
+  Interp P = make_interp(0, 0);
   std::vector<BoxData> boxes;
   std::vector<std::vector<int>> level_boxes;
   double time = 0.0;
@@ -182,6 +300,30 @@ inline bool is_interior(const BoxData& b, int i, int j, int k) {
 // ---------------------------------------------------------------------------------------------
 void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vector<Field>& kout) {
   const int V = 2 * H.F;
+  if (H.ko_order == 9) {
+    // eq (36) with r = 8 ("ninth-order KO dissipation"): (-1)^4 sigma / 2^10 sum_i h_i^9 (D+ D-)^5 y
+    //   = sigma / 1024 sum_i delta_i^10 y / h_i,  delta^10 = (1, -10, 45, -120, 210, -252, 210, -120, 45, -10, 1). 5 ghost layers.
+    static const double d10[11] = {1.0, -10.0, 45.0, -120.0, 210.0, -252.0, 210.0, -120.0, 45.0, -10.0, 1.0};
+    double c[3];
+    for (int a = 0; a < 3; ++a) c[a] = H.sigma / (1024.0 * H.dx(b.level, a));
+    for (int v = 0; v < V; ++v) {
+      const Field& y = Y[v];
+      Field& kv = kout[v];
+#pragma omp parallel for schedule(static)
+      for (int k = 0; k < b.n[2]; ++k)
+        for (int j = 0; j < b.n[1]; ++j)
+          for (int i = 0; i < b.n[0]; ++i) {
+            double sx = 0.0, sy = 0.0, sz = 0.0;
+            for (int m = -5; m <= 5; ++m) {
+              sx += d10[m + 5] * y.at(i + m, j, k);
+              sy += d10[m + 5] * y.at(i, j + m, k);
+              sz += d10[m + 5] * y.at(i, j, k + m);
+            }
+            kv.at(i, j, k) += c[0] * sx + c[1] * sy + c[2] * sz;
+          }
+    }
+    return;
+  }
   double c[3];
   for (int a = 0; a < 3; ++a) c[a] = H.sigma / (64.0 * H.dx(b.level, a));
   for (int v = 0; v < V; ++v) {
@@ -198,6 +340,49 @@ void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& 
           const double d6z = y.at(i, j, k - 3) - 6.0 * y.at(i, j, k - 2) + 15.0 * y.at(i, j, k - 1) - 20.0 * y.at(i, j, k) +
                              15.0 * y.at(i, j, k + 1) - 6.0 * y.at(i, j, k + 2) + y.at(i, j, k + 3);
           kv.at(i, j, k) += c[0] * d6x + c[1] * d6y + c[2] * d6z;
+        }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-4: radiative (Sommerfeld) outer boundary, PAPER.md:52 ("outgoing wave conditions"), :113 (step 1: "using
+// the physical boundary condition ... at the boundary"), :192 (NewRadX, outgoing boundary conditions applied to
+// the dynamical variables). Reading S29: the cells of the level-0 box within g cells of a domain face are
+// BOUNDARY POINTS; there every evolved variable y obeys, at every RK stage,
+//     d_t y = - v0 [ (x^i / r) d_i y + (y - y_inf) / r ],     v0 = 1, y_inf = 0,
+// with d_i y the second-order difference that fits in the box: centred where both neighbours exist, the one-sided
+// three-point formula on the outermost layer. x = cell centre (grid point for vertex-centred grids), r = |x|.
+// The boundary points are evolved by the same RK stages as the interior; ghost cells of level 0 are not used.
+// ---------------------------------------------------------------------------------------------
+void radiative_rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vector<Field>& kout) {
+  const int V = 2 * H.F, nb = H.g;
+  double dx[3];
+  for (int a = 0; a < 3; ++a) dx[a] = H.dx(b.level, a);
+  const double shift = H.vertex ? 0.0 : 0.5;
+  for (int v = 0; v < V; ++v) {
+    const Field& y = Y[v];
+    Field& kv = kout[v];
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < b.n[2]; ++k)
+      for (int j = 0; j < b.n[1]; ++j)
+        for (int i = 0; i < b.n[0]; ++i) {
+          const int idx[3] = {i, j, k};
+          bool zone = false;
+          for (int a = 0; a < 3; ++a)
+            if (idx[a] < nb || idx[a] >= b.n[a] - nb) zone = true;
+          if (!zone) continue;
+          double x[3], d[3];
+          for (int a = 0; a < 3; ++a) {
+            x[a] = H.xlo[a] + (double(b.lo[a] + idx[a]) + shift) * dx[a];
+            int e[3] = {0, 0, 0};
+            e[a] = 1;
+            auto Yat = [&](int m) { return y.at(i + m * e[0], j + m * e[1], k + m * e[2]); };
+            if (idx[a] == 0) d[a] = (-3.0 * Yat(0) + 4.0 * Yat(1) - Yat(2)) / (2.0 * dx[a]);
+            else if (idx[a] == b.n[a] - 1) d[a] = (3.0 * Yat(0) - 4.0 * Yat(-1) + Yat(-2)) / (2.0 * dx[a]);
+            else d[a] = (Yat(1) - Yat(-1)) / (2.0 * dx[a]);
+          }
+          const double r = std::sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+          kv.at(i, j, k) = -((x[0] * d[0] + x[1] * d[1] + x[2] * d[2]) / r + y.at(i, j, k) / r);
         }
   }
 }
@@ -252,6 +437,7 @@ void rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vect
         }
   }
   if (H.sigma != 0.0) add_dissipation(H, b, Y, kout);
+  if (H.outer_bc == 1 && b.level == 0) radiative_rhs(H, b, Y, kout);  // boundary points: overrides the interior formulas
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -273,11 +459,9 @@ void periodic_fill(const BoxData& b, std::vector<Field>& Y) {
 }
 
 // Spatial prolongation of a parent-cell field C (stored over the parent box, interior valid) into the
-// ghost cells of the child array `dst` (S3). Direct triple sum, x innermost then y then z.
-void prolong_into_ghosts(const BoxData& child, const BoxData& par, const Field& C, Field& dst) {
-  double w[2][5];
-  prolong_weights(0, w[0]);
-  prolong_weights(1, w[1]);
+// ghost cells of the child array `dst` (S3; variants: make_interp). Direct triple sum, x innermost then y then z.
+void prolong_into_ghosts(const Hier& H, const BoxData& child, const BoxData& par, const Field& C, Field& dst) {
+  const Interp& P = H.P;
   const int g = dst.g;
 #pragma omp parallel for schedule(static)
   for (int k = -g; k < child.n[2] + g; ++k)
@@ -288,18 +472,18 @@ void prolong_into_ghosts(const BoxData& child, const BoxData& par, const Field& 
         int J[3], p[3];
         for (int a = 0; a < 3; ++a) {
           const int Jg = floor_div2(I[a]);  // containing parent cell (global)
-          p[a] = I[a] - 2 * Jg;             // 0: fine centre at -dx_p/4, 1: at +dx_p/4
+          p[a] = I[a] - 2 * Jg;             // 0: fine centre at -dx_p/4, 1: at +dx_p/4 (vertex grids: 0 = on the parent point)
           J[a] = Jg - par.lo[a];            // parent-box-local
         }
         double sz = 0.0;
-        for (int c = -2; c <= 2; ++c) {
+        for (int c = 0; c < P.np; ++c) {
           double sy = 0.0;
-          for (int bb = -2; bb <= 2; ++bb) {
+          for (int bb = 0; bb < P.np; ++bb) {
             double sx = 0.0;
-            for (int a = -2; a <= 2; ++a) sx += w[p[0]][a + 2] * C.at(J[0] + a, J[1] + bb, J[2] + c);
-            sy += w[p[1]][bb + 2] * sx;
+            for (int a = 0; a < P.np; ++a) sx += P.w[p[0]][a] * C.at(J[0] + P.omin + a, J[1] + P.omin + bb, J[2] + P.omin + c);
+            sy += P.w[p[1]][bb] * sx;
           }
-          sz += w[p[2]][c + 2] * sy;
+          sz += P.w[p[2]][c] * sy;
         }
         dst.at(i, j, k) = sz;
       }
@@ -313,7 +497,7 @@ void dense_ghost_fill(const Hier& H, const BoxData& child, const BoxData& par, s
   C.init(par.n, H.g);
   // parent cells any ghost cell of the child can reach: ceil(g/2) cells beyond the child's coverage
   // plus the 2-cell interpolation radius (all inside the parent's interior by the nesting rule S13)
-  const int reach = (H.g + 1) / 2 + 2;
+  const int reach = (H.g + 1) / 2 + H.P.reach();
   int lo[3], hi[3];
   for (int a = 0; a < 3; ++a) {
     lo[a] = child.lo[a] / 2 - par.lo[a] - reach;
@@ -326,17 +510,17 @@ void dense_ghost_fill(const Hier& H, const BoxData& child, const BoxData& par, s
         for (int i = lo[0]; i < hi[0]; ++i) {
           const double kk[4] = {par.k[0][c].at(i, j, k), par.k[1][c].at(i, j, k), par.k[2][c].at(i, j, k),
                                 par.k[3][c].at(i, j, k)};
-          C.at(i, j, k) = dense_stage(stage, theta, hp, par.y_old[c].at(i, j, k), kk);
+          C.at(i, j, k) = dense_stage_any(H.integrator, stage, theta, hp, par.y_old[c].at(i, j, k), kk);
         }
-    prolong_into_ghosts(child, par, C, dst[c]);
+    prolong_into_ghosts(H, child, par, C, dst[c]);
   }
 }
 
 // Restriction (PAPER.md:119 step 7, S4): every parent cell whose children lie in the child's interior
-// takes the quintic interpolant of the child's y (reads up to 2 child ghost layers).
+// takes the quintic interpolant of the child's y (reads up to 2 child ghost layers; variants: make_interp —
+// 10-point: 4 layers; vertex-centred: injection of the coincident fine point).
 void restrict_to_parent(const Hier& H, const BoxData& child, BoxData& par) {
-  double r[6];
-  restrict_weights(r);
+  const Interp& P = H.P;
   const int J0[3] = {child.lo[0] / 2 - par.lo[0], child.lo[1] / 2 - par.lo[1], child.lo[2] / 2 - par.lo[2]};
   const int nc[3] = {child.n[0] / 2, child.n[1] / 2, child.n[2] / 2};
   for (int c = 0; c < 2 * H.F; ++c) {
@@ -347,14 +531,15 @@ void restrict_to_parent(const Hier& H, const BoxData& child, BoxData& par) {
       for (int J = 0; J < nc[1]; ++J)
         for (int I = 0; I < nc[0]; ++I) {
           double sz = 0.0;
-          for (int cc = 0; cc < 6; ++cc) {
+          for (int cc = 0; cc < P.nr; ++cc) {
             double sy = 0.0;
-            for (int bb = 0; bb < 6; ++bb) {
+            for (int bb = 0; bb < P.nr; ++bb) {
               double sx = 0.0;
-              for (int a = 0; a < 6; ++a) sx += r[a] * yc.at(2 * I - 2 + a, 2 * J - 2 + bb, 2 * K - 2 + cc);
-              sy += r[bb] * sx;
+              for (int a = 0; a < P.nr; ++a)
+                sx += P.r[a] * yc.at(2 * I + P.rmin + a, 2 * J + P.rmin + bb, 2 * K + P.rmin + cc);
+              sy += P.r[bb] * sx;
             }
-            sz += r[cc] * sy;
+            sz += P.r[cc] * sy;
           }
           yp.at(J0[0] + I, J0[1] + J, J0[2] + K) = sz;
         }
@@ -406,44 +591,66 @@ void axpy_interior(const BoxData& b, std::vector<Field>& out, const std::vector<
 void fill(Hier& H, int level, std::vector<Field> BoxData::*which, int stage, double theta, double dt) {
   for (int ib : H.level_boxes[level]) {
     BoxData& b = H.boxes[ib];
-    if (level == 0) periodic_fill(b, b.*which);
+    if (level == 0) { if (H.outer_bc == 0) periodic_fill(b, b.*which); }  // radiative: no ghosts, boundary points evolve
     else dense_ghost_fill(H, b, H.boxes[b.parent], b.*which, stage, theta, 2.0 * dt);
   }
   sibling_exchange(H, level, which);
 }
 
-// One RK4 step of all boxes of one level (eqs 1-9), ghosts by fill(); theta = where this step starts
+// Stage vector Y_{s+1} from y_n and the slopes so far, and the final update, on the interior of one box, for the
+// integrator in use: RK4 eqs (5), (7)-(9); RK3 / RK2 the tableaux of reading S28 (see b_coeff_rk3).
+void next_stage_vector(const Hier& H, BoxData& b, int s, double dt) {
+  if (H.integrator == 4) {
+    const double a_s[3] = {0.5, 0.5, 1.0};
+    axpy_interior(b, b.Y, b.y_old, a_s[s - 1] * dt, b.k[s - 1]);  // eqs (7)-(9)
+    return;
+  }
+  if (s == 1) { axpy_interior(b, b.Y, b.y_old, 0.5 * dt, b.k[0]); return; }  // Y2 = y_n + h/2 k1 (RK3 and RK2)
+  for (size_t c = 0; c < b.Y.size(); ++c) {                                  // RK3: Y3 = y_n - h k1 + 2 h k2
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < b.n[2]; ++k)
+      for (int j = 0; j < b.n[1]; ++j)
+        for (int i = 0; i < b.n[0]; ++i)
+          b.Y[c].at(i, j, k) = b.y_old[c].at(i, j, k) + dt * (-b.k[0][c].at(i, j, k) + 2.0 * b.k[1][c].at(i, j, k));
+  }
+}
+void final_update(const Hier& H, BoxData& b, double dt) {
+  for (int c = 0; c < 2 * H.F; ++c) {
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < b.n[2]; ++k)
+      for (int j = 0; j < b.n[1]; ++j)
+        for (int i = 0; i < b.n[0]; ++i) {
+          if (H.integrator == 4)
+            b.y[c].at(i, j, k) = b.y_old[c].at(i, j, k) +
+                                 (dt / 6.0) * (b.k[0][c].at(i, j, k) + 2.0 * b.k[1][c].at(i, j, k) +
+                                               2.0 * b.k[2][c].at(i, j, k) + b.k[3][c].at(i, j, k));  // eq (5)
+          else if (H.integrator == 3)
+            b.y[c].at(i, j, k) = b.y_old[c].at(i, j, k) +
+                                 (dt / 6.0) * (b.k[0][c].at(i, j, k) + 4.0 * b.k[1][c].at(i, j, k) + b.k[2][c].at(i, j, k));
+          else
+            b.y[c].at(i, j, k) = b.y_old[c].at(i, j, k) + dt * b.k[1][c].at(i, j, k);
+        }
+  }
+}
+
+// One RK step of all boxes of one level (RK4: eqs 1-9), ghosts by fill(); theta = where this step starts
 // inside the parent's step (0 or 1/2; ignored on level 0).
 void rk4_level_step(Hier& H, int level, double dt, double theta) {
-  const double a_s[3] = {0.5, 0.5, 1.0};
+  const int S = H.integrator;  // number of stages: RK4 4, RK3 3, RK2 2
   for (int ib : H.level_boxes[level]) {
     BoxData& b = H.boxes[ib];
     b.y_old = b.y;  // y_n
   }
   fill(H, level, &BoxData::y_old, 1, theta, dt);  // eq (15): Y_1 = y_n also in the ghosts
   for (int ib : H.level_boxes[level]) H.boxes[ib].Y = H.boxes[ib].y_old;  // eq (6)
-  for (int s = 1; s <= 4; ++s) {
+  for (int s = 1; s <= S; ++s) {
     for (int ib : H.level_boxes[level]) rhs(H, H.boxes[ib], H.boxes[ib].Y, H.boxes[ib].k[s - 1]);  // (1)-(4)
-    if (s < 4) {
-      for (int ib : H.level_boxes[level]) {
-        BoxData& b = H.boxes[ib];
-        axpy_interior(b, b.Y, b.y_old, a_s[s - 1] * dt, b.k[s - 1]);  // eqs (7)-(9)
-      }
+    if (s < S) {
+      for (int ib : H.level_boxes[level]) next_stage_vector(H, H.boxes[ib], s, dt);
       fill(H, level, &BoxData::Y, s + 1, theta, dt);  // eqs (16)-(18) in the ghosts
     }
   }
-  for (int ib : H.level_boxes[level]) {
-    BoxData& b = H.boxes[ib];
-    for (int c = 0; c < 2 * H.F; ++c) {
-#pragma omp parallel for schedule(static)
-      for (int k = 0; k < b.n[2]; ++k)
-        for (int j = 0; j < b.n[1]; ++j)
-          for (int i = 0; i < b.n[0]; ++i)
-            b.y[c].at(i, j, k) = b.y_old[c].at(i, j, k) +
-                                 (dt / 6.0) * (b.k[0][c].at(i, j, k) + 2.0 * b.k[1][c].at(i, j, k) +
-                                               2.0 * b.k[2][c].at(i, j, k) + b.k[3][c].at(i, j, k));  // eq (5)
-    }
-  }
+  for (int ib : H.level_boxes[level]) final_update(H, H.boxes[ib], dt);
   fill(H, level, &BoxData::y, 5, theta + 0.5, dt);  // eq (10) at theta + 1/2 in the ghosts
 }
 
@@ -462,35 +669,26 @@ void advance(Hier& H, int level, double dt, double theta) {
 void same_time_fill(Hier& H, int level, std::vector<Field> BoxData::*which) {
   for (int ib : H.level_boxes[level]) {
     BoxData& b = H.boxes[ib];
-    if (level == 0) { periodic_fill(b, b.*which); continue; }
+    if (level == 0) { if (H.outer_bc == 0) periodic_fill(b, b.*which); continue; }
     const BoxData& par = H.boxes[b.parent];
-    for (int c = 0; c < 2 * H.F; ++c) prolong_into_ghosts(b, par, (par.*which)[c], (b.*which)[c]);
+    for (int c = 0; c < 2 * H.F; ++c) prolong_into_ghosts(H, b, par, (par.*which)[c], (b.*which)[c]);
   }
   sibling_exchange(H, level, which);
 }
 
 void uniform_step(Hier& H, double dt) {
-  const double a_s[3] = {0.5, 0.5, 1.0};
-  const int L = H.nlevels;
+  const int L = H.nlevels, S = H.integrator;
   for (BoxData& b : H.boxes) b.y_old = b.y;
   for (int l = 0; l < L; ++l) same_time_fill(H, l, &BoxData::y_old);
   for (BoxData& b : H.boxes) b.Y = b.y_old;
-  for (int s = 1; s <= 4; ++s) {
+  for (int s = 1; s <= S; ++s) {
     for (BoxData& b : H.boxes) rhs(H, b, b.Y, b.k[s - 1]);
-    if (s < 4) {
-      for (BoxData& b : H.boxes) axpy_interior(b, b.Y, b.y_old, a_s[s - 1] * dt, b.k[s - 1]);
+    if (s < S) {
+      for (BoxData& b : H.boxes) next_stage_vector(H, b, s, dt);
       for (int l = 0; l < L; ++l) same_time_fill(H, l, &BoxData::Y);
     }
   }
-  for (BoxData& b : H.boxes)
-    for (int c = 0; c < 2 * H.F; ++c)
-#pragma omp parallel for schedule(static)
-      for (int k = 0; k < b.n[2]; ++k)
-        for (int j = 0; j < b.n[1]; ++j)
-          for (int i = 0; i < b.n[0]; ++i)
-            b.y[c].at(i, j, k) = b.y_old[c].at(i, j, k) +
-                                 (dt / 6.0) * (b.k[0][c].at(i, j, k) + 2.0 * b.k[1][c].at(i, j, k) +
-                                               2.0 * b.k[2][c].at(i, j, k) + b.k[3][c].at(i, j, k));
+  for (BoxData& b : H.boxes) final_update(H, b, dt);
   for (int l = 0; l < L; ++l) same_time_fill(H, l, &BoxData::y);
   for (int l = L - 1; l >= 1; --l)
     for (int ib : H.level_boxes[l]) restrict_to_parent(H, H.boxes[ib], H.boxes[H.boxes[ib].parent]);
@@ -505,7 +703,7 @@ bool validate(Hier& H, char* msg, size_t cap) {
   const BoxData& b0 = H.boxes[H.level_boxes[0][0]];
   for (int a = 0; a < 3; ++a)
     if (b0.lo[a] != 0 || b0.n[a] != H.domain[a] || b0.n[a] < H.g) return fail("level 0 must cover the domain");
-  const int margin = (H.g + 1) / 2 + 2;
+  const int margin = (H.g + 1) / 2 + H.P.reach();
   for (int l = 1; l < H.nlevels; ++l) {
     if (H.level_boxes[l].empty()) return fail("empty level");
     for (int ib : H.level_boxes[l]) {
@@ -622,7 +820,7 @@ void oc_destroy(void* h) { delete static_cast<Hier*>(h); }
 // Kreiss-Oliger strength sigma of eq (36); needs ghost width >= 3. Returns 0, or -1 with oc_last_error set.
 int oc_set_dissipation(void* h, double sigma) {
   Hier* H = static_cast<Hier*>(h);
-  if (!H || !(sigma >= 0.0) || (sigma != 0.0 && (H->g < 3 || H->fd_order != 4))) {
+  if (!H || !(sigma >= 0.0) || (sigma != 0.0 && H->g < (H->ko_order == 9 ? 5 : 3))) {
     snprintf(g_err, sizeof g_err, "dissipation needs sigma >= 0 and ghost width >= 3");
     return -1;
   }
@@ -630,16 +828,55 @@ int oc_set_dissipation(void* h, double sigma) {
   return 0;
 }
 
-// Order of the centred finite differences of the RHS: 4 (default, S2) or 8 (reads 4 ghost layers;
-// without dissipation: eq (36) with r = 8 would read 5). Returns 0, or -1 with oc_last_error set.
+// Order of the centred finite differences of the RHS: 4 (default, S2) or 8 (reads 4 ghost layers).
+// The dissipation order is a separate option (oc_set_options: the paper runs 8th-order differences with FIFTH-
+// order dissipation, while eq 36 ties it to r). Returns 0, or -1 with oc_last_error set.
 int oc_set_fd_order(void* h, int order) {
   Hier* H = static_cast<Hier*>(h);
-  if (!H || (order != 4 && order != 8) || (order == 8 && (H->g < 4 || H->sigma != 0.0))) {
-    snprintf(g_err, sizeof g_err, "fd order must be 4, or 8 with ghost width >= 4 and no dissipation");
+  if (!H || (order != 4 && order != 8) || (order == 8 && H->g < 4)) {
+    snprintf(g_err, sizeof g_err, "fd order must be 4, or 8 with ghost width >= 4");
     return -1;
   }
   H->fd_order = order;
   return 0;
+}
+
+// NEXT-3 / NEXT-4 options, set right after oc_create (before any state is evolved). Returns 0, or -1 with oc_last_error:
+//   integrator 4 | 3 | 2;  outer_bc 0 periodic | 1 radiative;  ko_order 5 | 9 (0: eq 36's r = fd_order -> 5 | 9);
+//   interp 0 (S3/S4) | 1 (follows the 8th-order stencil);  vertex 0 | 1.
+int oc_set_options(void* h, int integrator, int outer_bc, int ko_order, int interp, int vertex) {
+  Hier* H = static_cast<Hier*>(h);
+  if (!H) return -1;
+  if (integrator == 0) integrator = 4;
+  if (ko_order == 0) ko_order = H->fd_order == 8 ? 9 : 5;
+  const int ko_layers = ko_order == 9 ? 5 : 3;
+  if ((integrator != 4 && integrator != 3 && integrator != 2) || (outer_bc != 0 && outer_bc != 1) ||
+      (ko_order != 5 && ko_order != 9) || (interp != 0 && interp != 1) || (vertex != 0 && vertex != 1)) {
+    snprintf(g_err, sizeof g_err, "bad option value");
+    return -1;
+  }
+  if (H->sigma != 0.0 && H->g < ko_layers) { snprintf(g_err, sizeof g_err, "dissipation order %d reads %d ghost layers", ko_order, ko_layers); return -1; }
+  H->integrator = integrator;
+  H->outer_bc = outer_bc;
+  H->ko_order = ko_order;
+  H->interp = interp;
+  H->vertex = vertex;
+  H->P = make_interp(interp, vertex);
+  if (H->P.nr > 1 && -H->P.rmin > H->g) { snprintf(g_err, sizeof g_err, "restriction reads %d ghost layers", -H->P.rmin); return -1; }
+  if (!validate(*H, g_err, sizeof g_err)) return -1;  // the nesting margin depends on the footprint
+  return 0;
+}
+void oc_interp_weights(int interp, int vertex, int* np, int* omin, double* w0, double* w1, int* nr, int* rmin, double* r) {
+  const Interp P = make_interp(interp, vertex);
+  *np = P.np; *omin = P.omin; *nr = P.nr; *rmin = P.rmin;
+  for (int m = 0; m < P.np; ++m) { w0[m] = P.w[0][m]; w1[m] = P.w[1][m]; }
+  for (int m = 0; m < P.nr; ++m) r[m] = P.r[m];
+}
+double oc_b_rk(int integrator, int i, int m, double theta) {
+  return integrator == 3 ? b_coeff_rk3(i, m, theta) : (integrator == 2 ? b_coeff_rk2(i, m, theta) : b_coeff(i, m, theta));
+}
+double oc_dense_stage_rk(int integrator, int stage, double theta, double hp, double y_old, const double* k) {
+  return dense_stage_any(integrator, stage, theta, hp, y_old, k);
 }
 
 int oc_set_state(void* h, int level, int box, int comp, const double* src) {

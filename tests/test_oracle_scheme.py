@@ -462,8 +462,8 @@ def test_rounding_floor_of_the_oracle(tmp_path):
     built twice — as shipped, and with multiply-adds contracted (-mfma -ffp-contract=fast: every a*b+c rounds once
     instead of twice, nothing else changes) — takes one subcycled coarse step of a hierarchy whose finest spacing is
     cfg 5's. The two results differ by rounding only. Measured: u agrees to ~1e-15 max|u| on every level, rho moves
-    by ~2e-11 max|u| (= ~2e-12 max|rho|) on the finest level: the bound 1e-11 max|u| cannot be applied to rho there
-    (it is below the definition's own rounding floor), 1e-11 max|rho| can."""
+    by ~2e-11 max|u| on the finest level: the bound 1e-11 max|u| cannot be applied to rho there (it is below the
+    definition's own rounding floor); the floor term F of oracle/parity.py bounds it."""
     import subprocess
     import sys
     if "fma" not in open("/proc/cpuinfo").read():
@@ -482,9 +482,12 @@ def test_rounding_floor_of_the_oracle(tmp_path):
     sr = max(np.abs(a[f"l{l}c1"]).max() for l in range(nl))
     du = max(np.abs(a[f"l{l}c0"] - b[f"l{l}c0"]).max() for l in range(nl))
     dr = max(np.abs(a[f"l{l}c1"] - b[f"l{l}c1"]).max() for l in range(nl))
-    assert du <= 1e-13 * su, (du, su)           # u: far inside the tolerance
-    assert dr <= 1e-11 * sr, (dr, sr)           # rho against its own scale: inside
-    assert dr >= 3e-12 * su, (dr, su)           # rho against max|u|: AT the tolerance — rounding alone, no kernel involved
+    from oracle.parity import rho_floor
+    w = wl.cfg5(32, 9)
+    F = rho_floor(w, su)
+    assert du <= 1e-13 * su, (du, su)           # u: far inside 1e-11 max|u|
+    assert dr >= 3e-12 * su, (dr, su)           # rho against max|u|: AT the stated tolerance — rounding alone, no kernel
+    assert 0.02 * F <= dr <= F, (dr, F)         # and inside the floor F that oracle/parity.py derives (linear accumulation)
     # the floor grows with depth (eps * 0.6 |u| / dx per RHS evaluation, twice the evaluations per level)
     d_lvl = [np.abs(a[f"l{l}c1"] - b[f"l{l}c1"]).max() for l in range(nl)]
     assert d_lvl[8] > 20.0 * d_lvl[3], d_lvl
