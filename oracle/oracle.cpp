@@ -110,15 +110,22 @@ double dense_stage(int stage, double theta, double hp, double y_old, const doubl
 //   RK3 = Kutta's third-order method:  k1 = f(Y1), k2 = f(Y2), k3 = f(Y3),
 //         Y1 = y_n,  Y2 = y_n + h/2 k1,  Y3 = y_n - h k1 + 2 h k2,  y_{n+1} = y_n + h/6 (k1 + 4 k2 + k3);
 //   RK2 = the midpoint method:         Y1 = y_n,  Y2 = y_n + h/2 k1,  y_{n+1} = y_n + h k2.
-// Dense output (the analogue of eqs 10-13: the polynomials b_i(theta) with b_i(1) = the method's weights that
-// satisfy the quadrature order conditions sum b_i = theta, sum b_i c_i = theta^2/2 and, for RK3, sum b_i c_i^2 =
-// theta^3/3; for RK3 they are eqs (11)-(13) with the two middle stages of RK4 merged, b_2^{RK3} = b_2 + b_3):
-//   RK3:  b1 = theta - 3/2 theta^2 + 2/3 theta^3,  b2 = 2 theta^2 - 4/3 theta^3,  b3 = -1/2 theta^2 + 2/3 theta^3
-//   RK2:  b1 = theta - theta^2,                    b2 = theta^2
-// Ghost stage vectors (the analogue of eqs 15-18: Taylor expansion of the child's own stage values in its step h,
-// kept to the order the integrator needs, h^2 for RK3 and h for RK2; derivatives by eq 14 from the parent):
-//   RK3:  Y1 = y,  Y2 = y + h/2 y',  Y3 = y + h y' + h^2 y''      (k2 = y' + h/2 y'' + O(h^2) in Y3 = y - h k1 + 2 h k2)
-//   RK2:  Y1 = y,  Y2 = y + h/2 y'
+// Dense output (the analogue of eqs 10-13). RK4's eq (10) is a continuous extension one order below the method
+// (local error O(h^4)). A three-stage third-order method has no such extension from k1..k3 alone (four order
+// conditions, three polynomials), so a level that has a child evaluates one more slope, k4 = f(y_{n+1}), after
+// its update (the child cannot start before y_{n+1} exists anyway); with c = (0, 1/2, 1, 1) the four conditions
+//   sum b_i = theta,  sum b_i c_i = theta^2/2,  sum b_i c_i^2 = theta^3/3,  sum_i b_i sum_j a_ij c_j = theta^3/6
+// have the unique solution
+//   RK3:  b1 = theta - 3/2 theta^2 + 2/3 theta^3,  b2 = 2 theta^2 - 4/3 theta^3,
+//         b3 = 1/2 theta^2 - 1/3 theta^3,          b4 = theta^3 - theta^2            (b(1) = (1/6, 2/3, 1/6, 0))
+//   RK2:  b1 = theta - theta^2,  b2 = theta^2      (two conditions, two polynomials: full order from k1, k2)
+// Ghost stage vectors (the analogue of eqs 15-18: Taylor expansion of the child's own stage values in its step h
+// to the order the dense output supports; derivatives by eq 14 from the parent; D1, D2, D3 = first, second, third
+// time derivative of y):
+//   RK3:  Y1 = y,  Y2 = y + h/2 D1,  Y3 = y + h D1 + h^2 D2 + h^3/4 (D3 - f_y D2),   f_y D2 = 2 (k3 - k4) / hp^2
+//         (k2 = D1 + h/2 D2 + h^2/8 (D3 - f_y D2) + O(h^3) in Y3 = y - h k1 + 2 h k2; the parent's
+//          k3 - k4 = f(y + hp D1 + hp^2 D2 + ..) - f(y + hp D1 + hp^2/2 D2 + ..) = hp^2/2 f_y D2 + O(hp^3))
+//   RK2:  Y1 = y,  Y2 = y + h/2 D1
 // ---------------------------------------------------------------------------------------------
 double b_coeff_rk3(int i, int m, double th) {
   switch (i) {
@@ -132,31 +139,40 @@ double b_coeff_rk3(int i, int m, double th) {
       if (m == 1) return 4.0 * th - 4.0 * th * th;
       if (m == 2) return 4.0 - 8.0 * th;
       return -8.0;
+    case 3:
+      if (m == 0) return 0.5 * th * th - (1.0 / 3.0) * th * th * th;
+      if (m == 1) return th - th * th;
+      if (m == 2) return 1.0 - 2.0 * th;
+      return -2.0;
     default:
-      if (m == 0) return -0.5 * th * th + (2.0 / 3.0) * th * th * th;
-      if (m == 1) return -th + 2.0 * th * th;
-      if (m == 2) return -1.0 + 4.0 * th;
-      return 4.0;
+      if (m == 0) return th * th * th - th * th;
+      if (m == 1) return 3.0 * th * th - 2.0 * th;
+      if (m == 2) return 6.0 * th - 2.0;
+      return 6.0;
   }
 }
 double b_coeff_rk2(int i, int m, double th) {
   if (i == 1) return m == 0 ? th - th * th : (m == 1 ? 1.0 - 2.0 * th : (m == 2 ? -2.0 : 0.0));
   return m == 0 ? th * th : (m == 1 ? 2.0 * th : (m == 2 ? 2.0 : 0.0));
 }
-// stage = 1..3 (RK3) / 1..2 (RK2): the ghost value of Y_stage; stage 5: y at `theta` by the dense output alone
-double dense_stage_rk3(int stage, double theta, double hp, double y_old, const double k[3]) {
-  double s0 = 0.0, d1 = 0.0, d2 = 0.0;
-  for (int i = 1; i <= 3; ++i) {
+// stage = 1..3 (RK3) / 1..2 (RK2): the ghost value of Y_stage; stage 5: y at `theta` by the dense output alone.
+// RK3: k[0..2] = k1..k3 of the parent's step, k[3] = k4 = f(y_{n+1}).
+double dense_stage_rk3(int stage, double theta, double hp, double y_old, const double k[4]) {
+  double s0 = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0;
+  for (int i = 1; i <= 4; ++i) {
     s0 += b_coeff_rk3(i, 0, theta) * k[i - 1];
     d1 += b_coeff_rk3(i, 1, theta) * k[i - 1];
     d2 += b_coeff_rk3(i, 2, theta) * k[i - 1];
+    d3 += b_coeff_rk3(i, 3, theta) * k[i - 1];
   }
   const double y = y_old + hp * s0;  // the analogue of eq (10)
   d2 = d2 / hp;                      // eq (14), m = 2
+  d3 = d3 / (hp * hp);               // eq (14), m = 3
   if (stage == 1 || stage == 5) return y;
   const double h = 0.5 * hp;  // child step
   if (stage == 2) return y + 0.5 * h * d1;
-  return y + h * d1 + h * h * d2;
+  const double fyy = 2.0 * (k[2] - k[3]) / (hp * hp);
+  return y + h * d1 + h * h * d2 + (h * h * h / 4.0) * (d3 - fyy);
 }
 double dense_stage_rk2(int stage, double theta, double hp, double y_old, const double k[2]) {
   double s0 = 0.0, d1 = 0.0;
@@ -652,6 +668,8 @@ void rk4_level_step(Hier& H, int level, double dt, double theta) {
   }
   for (int ib : H.level_boxes[level]) final_update(H, H.boxes[ib], dt);
   fill(H, level, &BoxData::y, 5, theta + 0.5, dt);  // eq (10) at theta + 1/2 in the ghosts
+  if (S == 3 && level + 1 < H.nlevels)  // RK3 (S28): the slope at the new state completes the dense output the child reads
+    for (int ib : H.level_boxes[level]) rhs(H, H.boxes[ib], H.boxes[ib].y, H.boxes[ib].k[3]);
 }
 
 // Steps 1-7.

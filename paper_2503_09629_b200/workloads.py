@@ -367,15 +367,16 @@ def cut_finest(w: Workload, pieces: int, axis: int = 2) -> Workload:
 SPH_A, SPH_SIGMA = 1.0, 0.25 / math.sqrt(2.0)
 
 
-def spherical_wave_exact(w: Workload, level: int, ibox: int, comp: int, t: float) -> np.ndarray:
+def spherical_wave_exact(w: Workload, level: int, ibox: int, comp: int, t: float, sigma: float = None) -> np.ndarray:
     """u = [f(t-r) - f(t+r)] / r,  Pi = -[f(t-r)(t-r) - f(t+r)(t+r)] / (sigma^2 r),  f(v) = A exp(-v^2 / (2 sigma^2)),
     A = 1, sigma = 0.25/sqrt(2) (eqs 41-42). Cell-centred grids never put a centre at r = 0 (S1)."""
+    sg = SPH_SIGMA if sigma is None else sigma
     x, y, z = w.centres(level, ibox)
     r = np.sqrt(z[:, None, None] ** 2 + y[None, :, None] ** 2 + x[None, None, :] ** 2)
-    f = lambda v: SPH_A * np.exp(-v * v / (2.0 * SPH_SIGMA ** 2))  # noqa: E731
+    f = lambda v: SPH_A * np.exp(-v * v / (2.0 * sg ** 2))  # noqa: E731
     if comp < w.nfields:
         return (f(t - r) - f(t + r)) / r
-    return -(f(t - r) * (t - r) - f(t + r) * (t + r)) / (SPH_SIGMA ** 2 * r)
+    return -(f(t - r) * (t - r) - f(t + r) * (t + r)) / (sg ** 2 * r)
 
 
 def paper_wave(n0: int = 64) -> Workload:
