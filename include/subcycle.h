@@ -28,7 +28,7 @@ enum {
   SC_OK = 0,
   SC_ERR_INVALID_ARG = -1, /* null pointer, index out of range, non-finite dt, capacity too small */
   SC_ERR_NESTING = -2,     /* box list violates the nesting rules below                           */
-  SC_ERR_UNSUPPORTED = -3, /* ref_ratio != 2, ghost outside [2,4], nlevels > SC_MAX_LEVELS, F > 32  */
+  SC_ERR_UNSUPPORTED = -3, /* ref_ratio != 2, ghost outside [2,5], nlevels > SC_MAX_LEVELS, F > 32, bad option */
   SC_ERR_OOM = -4,         /* arena too small / device allocation failed                          */
   SC_ERR_CUDA = -5         /* a CUDA runtime/driver call failed (message has the CUDA error string) */
 };
@@ -64,11 +64,27 @@ typedef struct {
  *   d_t u_f = rho_f,   d_t rho_f = Lap_h u_f + sum_j A[f][j] u_j       (BASELINE cfg 4)
  * ko_sigma: strength of the Kreiss-Oliger dissipation added to the time derivative of EVERY evolved variable,
  *   d_t y -> RHS + Q y,  Q y = sigma/64 sum_i delta_i^6 y / h_i  (eqs 35-36 with r = 4);
- *   needs ghost >= 3. With sigma > 0 the step runs the general stage-by-stage kernels (the stage vectors' u parts
+ *   needs ghost >= 3 (ko_order 9: sigma/1024 sum_i delta_i^10 y / h_i, ghost >= 5). With sigma > 0 the step runs the general stage-by-stage kernels (the stage vectors' u parts
  *   are stored: 5 more arrays per field), with sigma = 0 the two-launch formulation of DESIGN.md section 6.
  * fd_order: 8 selects the paper's BBH discretisation, the 9-point second difference
- *   (-1/560, 8/315, -1/5, 8/5, -205/72, ...)/h^2 per axis; needs ghost >= 4 and ko_sigma = 0 (eq 36 with r = 8 would
- *   read 5 layers) -> SC_ERR_UNSUPPORTED otherwise. The prolongation and restriction operators are unchanged (S3, S4).
+ *   (-1/560, 8/315, -1/5, 8/5, -205/72, ...)/h^2 per axis; needs ghost >= 4 -> SC_ERR_UNSUPPORTED otherwise.
+ * ko_order: order of the dissipation operator: 5 -> delta^6 (eq 36 with r = 4; 3 ghost layers), 9 -> delta^10 (eq 36 with
+ *   r = 8, "ninth-order"; 5 ghost layers), 0 -> eq 36's rule r = fd_order. (The paper's production runs
+ *   pair 8th-order differences with FIFTH-order dissipation: fd_order = 8, ko_order = 5, ghost = 4.)
+ * integrator: 0 or 4 -> classical RK4 (eqs 1-9); 3 -> Kutta's RK3 with the slope at the new state completing a third-
+ *   order dense output; 2 -> midpoint RK2 (reading S28 gives tableaux, b_i(theta) and the ghost
+ *   stage formulas).
+ * outer_bc: 0 -> periodic level 0 (S9); 1 -> radiative (Sommerfeld) boundary (reading S29): the
+ *   cells of level 0 within `ghost` cells of a domain face are boundary points, every evolved variable obeys
+ *   d_t y = -[(x^i/r) d_i y + y/r] there (second-order centred / one-sided differences), at every stage; the ghost
+ *   cells of level 0 are then unused. The domain must contain the origin strictly inside.
+ * interp_order: 0 -> quartic prolongation, quintic restriction (S3, S4); 1 -> 9-point prolongation and 10-point
+ *   restriction, the orders that follow 8th-order differences (reading S30; needs ghost >= 4; nesting margin
+ *   ceil(g/2) + 4 parent cells).
+ * centering: 0 -> cell-centred grids (S1); 1 -> vertex-centred: grid point i of level l sits at xlo + i dx_l, fine
+ *   point 2J coincides with parent point J: restriction is injection, even ghost points copy, odd ghost points take the
+ *   6-point (interp_order 1: 10-point) midpoint interpolant (reading S31; nesting margin ceil(g/2) + 3 (5)).
+ * Any of ko_sigma > 0, integrator != RK4, outer_bc != 0 selects the general stage-by-stage kernels.
  * arena: optional DEVICE memory of at least sc_arena_bytes() bytes, 256-byte aligned, owned by the
  *   caller, who keeps it alive and does not touch it until sc_destroy; NULL -> the library allocates.
  * cuda_stream: a cudaStream_t (as void*) on which all work of this hierarchy is enqueued (must not be
@@ -89,6 +105,11 @@ typedef struct {
   void* cuda_stream;
   double ko_sigma;         /* Kreiss-Oliger strength sigma >= 0; 0 = none */
   int32_t fd_order;        /* centred differences of the RHS: 0 or 4 -> 4th order (S2); 8 -> 8th order           */
+  int32_t ko_order;        /* 0 (follow fd_order), 5 or 9                                                          */
+  int32_t integrator;      /* 0 / 4: RK4; 3: RK3; 2: RK2                                                           */
+  int32_t outer_bc;        /* 0: periodic; 1: radiative                                                            */
+  int32_t interp_order;    /* 0: quartic / quintic; 1: 9-point / 10-point                                          */
+  int32_t centering;       /* 0: cell-centred; 1: vertex-centred with injection                                    */
 } sc_hierarchy_desc;
 
 typedef struct sc_hierarchy sc_hierarchy; /* opaque; created by sc_create_hierarchy, freed by sc_destroy */

@@ -156,8 +156,8 @@ class OracleHierarchy:
         self.nlevels = nlev
         if fd_order != 4 and L.oc_set_fd_order(self._h, int(fd_order)) != 0:
             raise ValueError("oracle: " + L.oc_last_error().decode())
-        if (integrator, outer_bc, ko_order, interp, vertex) != (4, 0, 0, 0, 0) and \
-                L.oc_set_options(self._h, int(integrator), int(outer_bc), int(ko_order), int(interp), int(vertex)) != 0:
+        # always: ko_order = 0 resolves to eq 36's r = fd_order, which depends on the call above
+        if L.oc_set_options(self._h, int(integrator), int(outer_bc), int(ko_order), int(interp), int(vertex)) != 0:
             raise ValueError("oracle: " + L.oc_last_error().decode())
         if ko_sigma and L.oc_set_dissipation(self._h, float(ko_sigma)) != 0:
             raise ValueError("oracle: " + L.oc_last_error().decode())

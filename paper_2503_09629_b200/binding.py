@@ -31,7 +31,9 @@ class sc_hierarchy_desc(C.Structure):
                 ("ref_ratio", C.c_int32), ("ghost", C.c_int32), ("nfields", C.c_int32),
                 ("domain_cells", C.c_int32 * 3), ("xlo", C.c_double * 3), ("xhi", C.c_double * 3),
                 ("coupling", C.POINTER(C.c_double)), ("arena", C.c_void_p), ("arena_bytes", C.c_uint64),
-                ("cuda_stream", C.c_void_p), ("ko_sigma", C.c_double), ("fd_order", C.c_int32)]
+                ("cuda_stream", C.c_void_p), ("ko_sigma", C.c_double), ("fd_order", C.c_int32),
+                ("ko_order", C.c_int32), ("integrator", C.c_int32), ("outer_bc", C.c_int32),
+                ("interp_order", C.c_int32), ("centering", C.c_int32)]
 
 
 class SubcycleError(RuntimeError):
@@ -94,7 +96,8 @@ def _check(rc: int):
 
 def make_desc(boxes, domain_cells, nfields=1, ghost=3, xlo=(-1.0, -1.0, -1.0), xhi=(1.0, 1.0, 1.0),
               coupling: Optional[np.ndarray] = None, ref_ratio: int = 2, nlevels: Optional[int] = None,
-              ko_sigma: float = 0.0, fd_order: int = 4):
+              ko_sigma: float = 0.0, fd_order: int = 4, ko_order: int = 0, integrator: int = 4, outer_bc: int = 0,
+              interp: int = 0, vertex: int = 0):
     """Marshal a box list into an sc_hierarchy_desc. Returns (desc, keepalive)."""
     arr = (sc_box * len(boxes))()
     for i, b in enumerate(boxes):
@@ -111,6 +114,8 @@ def make_desc(boxes, domain_cells, nfields=1, ghost=3, xlo=(-1.0, -1.0, -1.0), x
     d.xhi[:] = list(xhi)
     d.ko_sigma = float(ko_sigma)
     d.fd_order = int(fd_order)
+    d.ko_order, d.integrator, d.outer_bc = int(ko_order), int(integrator), int(outer_bc)
+    d.interp_order, d.centering = int(interp), int(vertex)
     keep = [arr]
     if coupling is not None:
         cm = np.ascontiguousarray(coupling, dtype=np.float64)
@@ -131,13 +136,15 @@ class Hierarchy:
 
     def __init__(self, boxes, domain_cells, nfields=1, ghost=3, xlo=(-1.0, -1.0, -1.0), xhi=(1.0, 1.0, 1.0),
                  coupling: Optional[np.ndarray] = None, device: str = "cuda:0", use_torch_arena: bool = True,
-                 ko_sigma: float = 0.0, fd_order: int = 4):
+                 ko_sigma: float = 0.0, fd_order: int = 4, ko_order: int = 0, integrator: int = 4, outer_bc: int = 0,
+                 interp: int = 0, vertex: int = 0):
         import torch  # device memory + stream only
 
         self._h = C.c_void_p()
         self.boxes = list(boxes)
         self.nfields, self.ghost = nfields, ghost
-        desc, keep = make_desc(boxes, domain_cells, nfields, ghost, xlo, xhi, coupling, ko_sigma=ko_sigma, fd_order=fd_order)
+        desc, keep = make_desc(boxes, domain_cells, nfields, ghost, xlo, xhi, coupling, ko_sigma=ko_sigma, fd_order=fd_order,
+                               ko_order=ko_order, integrator=integrator, outer_bc=outer_bc, interp=interp, vertex=vertex)
         self.nlevels = desc.nlevels
         self.arena_bytes = sc_arena_bytes(desc)
         if not torch.cuda.is_available():
@@ -158,6 +165,8 @@ class Hierarchy:
     def from_workload(cls, w, **kw) -> "Hierarchy":
         kw.setdefault("ko_sigma", getattr(w, "ko_sigma", 0.0))
         kw.setdefault("fd_order", getattr(w, "fd_order", 4))
+        for opt, default in (("ko_order", 0), ("integrator", 4), ("outer_bc", 0), ("interp", 0), ("vertex", 0)):
+            kw.setdefault(opt, int(getattr(w, opt, default)))
         h = cls(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling, **kw)
         for l in range(w.nlevels):
             for ib in range(len(w.level_boxes(l))):

@@ -128,6 +128,33 @@ void dense_coeffs(int stage, double th, double c[4]) {
   }
 }
 
+// The same for the RK3 / RK2 integrators (reading S28); value = y_old^p + h_p * sum_j c_j k_j^p.
+//   RK3 (k_4 = f(y_{n+1}) is the fourth slope): b = (th - 3/2 th^2 + 2/3 th^3, 2 th^2 - 4/3 th^3, 1/2 th^2 - 1/3 th^3, th^3 - th^2)
+//     stage 2: c = b + (r/2) b';   stage 3: c = b + r b' + r^2 b'' + (r^3/4)(b(3) - phi), b(3) = third theta-derivative,  phi = (0, 0, 2, -2)
+//     (Y_3 = y + h y' + h^2 y'' + h^3/4 (y(3) - f_y y''),  f_y y'' = 2 (k_3 - k_4) / h_p^2)
+//   RK2: b = (th - th^2, th^2);  stage 2: c = b + (r/2) b'
+void dense_coeffs_rk(int integrator, int stage, double th, double c[4]) {
+  if (integrator == 4) { dense_coeffs(stage, th, c); return; }
+  const double r = 0.5;
+  if (integrator == 3) {
+    const double b0[4] = {th - 1.5 * th * th + (2.0 / 3.0) * th * th * th, 2.0 * th * th - (4.0 / 3.0) * th * th * th,
+                          0.5 * th * th - (1.0 / 3.0) * th * th * th, th * th * th - th * th};
+    const double b1[4] = {1.0 - 3.0 * th + 2.0 * th * th, 4.0 * th - 4.0 * th * th, th - th * th, 3.0 * th * th - 2.0 * th};
+    const double b2[4] = {-3.0 + 4.0 * th, 4.0 - 8.0 * th, 1.0 - 2.0 * th, 6.0 * th - 2.0};
+    const double b3[4] = {4.0, -8.0, -2.0, 6.0};
+    const double phi[4] = {0.0, 0.0, 2.0, -2.0};
+    for (int j = 0; j < 4; ++j) {
+      if (stage == 2) c[j] = b0[j] + 0.5 * r * b1[j];
+      else if (stage == 3) c[j] = b0[j] + r * b1[j] + r * r * b2[j] + (r * r * r / 4.0) * (b3[j] - phi[j]);
+      else c[j] = b0[j];
+    }
+    return;
+  }
+  const double b0[2] = {th - th * th, th * th}, b1[2] = {1.0 - 2.0 * th, 2.0 * th};
+  c[2] = c[3] = 0.0;
+  for (int j = 0; j < 2; ++j) c[j] = stage == 2 ? b0[j] + 0.5 * r * b1[j] : b0[j];
+}
+
 // ---- launch recording -----------------------------------------------------------------------
 struct Seq {
   sc_hierarchy* h;
@@ -147,15 +174,15 @@ double cells(const BoxView& v) { return (double)v.n[0] * v.n[1] * v.n[2]; }
 double shell_cells(const BoxView& v) {
   return (double)(v.n[0] + 2 * v.g) * (v.n[1] + 2 * v.g) * (v.n[2] + 2 * v.g) - cells(v);
 }
-double footprint_cells(const BoxView& v) {  // parent cells a ghost fill of this box reads
-  // ghost cells sit in parent cells up to gc = ceil(g/2) beyond the child's coverage [0, nc); the 5-point
-  // interpolation adds 2 more on every side and reaches 2 cells into the coverage
+double footprint_cells(const BoxView& v, int reach = 2) {  // parent cells a ghost fill of this box reads
+  // ghost cells sit in parent cells up to gc = ceil(g/2) beyond the child's coverage [0, nc); the interpolation
+  // stencil adds `reach` more on every side (2 for S3) and reaches as far into the coverage
   const int gc = (v.g + 1) / 2;
   double outer = 1.0, inner = 1.0;
   for (int a = 0; a < 3; ++a) {
     const int nc = v.n[a] / 2;
-    outer *= nc + 2 * gc + 4;
-    inner *= nc > 4 ? nc - 4 : 0;
+    outer *= nc + 2 * gc + 2 * reach;
+    inner *= nc > 2 * reach ? nc - 2 * reach : 0;
   }
   return outer - inner;
 }
@@ -258,9 +285,20 @@ void ghost_launch(Seq& q, int ib, GhostArgs& a) {
   a.tiles = h->tiles[ib].dev;
   a.ntiles = h->tiles[ib].n;
   a.tmaps = h->gmap_ok[b.parent] ? h->gmaps[b.parent].m[0].bytes : nullptr;
+  const InterpOps& P = h->L.ops;
+  a.np = P.np;
+  a.pmin = P.pmin;
+  for (int m = 0; m < 10; ++m) { a.w[0][m] = P.w[0][m]; a.w[1][m] = P.w[1][m]; }
   double bytes = 0.0;
-  for (int p = 0; p < a.nprob; ++p)
-    bytes += 8.0 * h->L.F * (a.prob[p].nsrc * footprint_cells(b.v) + a.prob[p].nout * shell_cells(b.v));
+  for (int p = 0; p < a.nprob; ++p) {
+    int nreal = 0;  // sources padded for the tuned kernel's shape (coefficient column all zero) are not algorithmic traffic
+    for (int sidx = 0; sidx < a.prob[p].nsrc; ++sidx) {
+      bool used = false;
+      for (int o = 0; o < a.prob[p].nout; ++o) used = used || a.prob[p].coef[o][sidx] != 0.0;
+      nreal += used ? 1 : 0;
+    }
+    bytes += 8.0 * h->L.F * (nreal * footprint_cells(b.v, P.reach()) + a.prob[p].nout * shell_cells(b.v));
+  }
   prof_begin(h, KIND_GHOST, bytes);
   launch_ghost_fill(a, h->stream);
   prof_end(h);
@@ -355,46 +393,67 @@ void restrict_level(Seq& q, int level) {  // level -> level-1, into the parents'
     a.ychild = h->arr(ib, a.a_child);
     a.yparent = h->arr(b.parent, h->L.a_state(q.cur[level - 1]));
     a.tmap = h->tmap_ok[ib] ? h->rmaps[ib].bytes : nullptr;
+    a.nr = h->L.ops.nr;
+    a.rmin = h->L.ops.rmin;
+    for (int m = 0; m < 10; ++m) a.r[m] = h->L.ops.r[m];
     launch_restrict(a, h->stream);
     prof_end(h);
     ++q.n;
   }
 }
 
-// ---- NEXT-1: the general stage-by-stage path, used with Kreiss-Oliger dissipation (stage_ko.cu) -----------
-// Arrays of stage s: U_s = a_U(s), R_s = a_R(s) for s = 2..4; Y_1 = y_n lives in the state slot.
+// ---- the general stage-by-stage path (stage_gen.cu / stage_ko_tma.cu): Kreiss-Oliger dissipation of either order,
+// the RK3 / RK2 integrators, the radiative outer boundary ------------------------
+// Arrays of stage s: U_s = a_U(s), R_s = a_R(s) for s = 2..4; Y_1 = y_n lives in the state slot. RK3 keeps k_3 in
+// the (otherwise unused) arrays of stage 4 and k_4 = f(y_{n+1}) in K4; RK2 keeps k_2 in K4.
 void stage_ko_level(Seq& q, int level, int s, double dt) {
   sc_hierarchy* h = q.h;
   const Layout& L = h->L;
-  const int yn = q.cur[level], ynew = 1 - yn, F = L.F;
-  const bool keep_k4 = s == 4 && q.sub && level + 1 < L.nlevels;
+  const int S = L.integrator;
+  // s == S + 1 (RK3 only): the slope at the new state; q.cur[level] has already been flipped
+  const bool extra = s > S;
+  const int yn = extra ? 1 - q.cur[level] : q.cur[level], ynew = 1 - yn, F = L.F;
+  const bool keep = q.sub && level + 1 < L.nlevels;
   for (int ib : L.level_boxes[level]) {
     StageKOArgs a{};
     a.b = L.boxes[ib].v;
     a.F = F;
     a.stage = s;
+    a.integrator = S;
+    a.fd_order = L.fd_order;
+    a.ko_order = L.ko_sigma > 0.0 ? L.ko_order : 0;
     a.yn_u = h->arr(ib, L.a_state(yn));
     a.yn_r = h->arr(ib, L.a_state(yn) + F);
-    a.Yu = s == 1 ? a.yn_u : h->arr(ib, L.a_U(s));
-    a.Yr = s == 1 ? a.yn_r : h->arr(ib, L.a_R(s));
-    a.outU = s < 4 ? h->arr(ib, L.a_U(s + 1)) : h->arr(ib, L.a_state(ynew));
-    a.outR = s < 4 ? h->arr(ib, L.a_R(s + 1)) : h->arr(ib, L.a_state(ynew) + F);
+    const int in_u = s == 1 ? L.a_state(yn) : (extra ? L.a_state(ynew) : L.a_U(s));
+    const int in_r = s == 1 ? L.a_state(yn) + F : (extra ? L.a_state(ynew) + F : L.a_R(s));
+    a.Yu = h->arr(ib, in_u);
+    a.Yr = h->arr(ib, in_r);
+    a.outU = s < S ? h->arr(ib, L.a_U(s + 1)) : h->arr(ib, L.a_state(ynew));
+    a.outR = s < S ? h->arr(ib, L.a_R(s + 1)) : h->arr(ib, L.a_state(ynew) + F);
     a.U2 = h->arr(ib, L.a_U(2)); a.U3 = h->arr(ib, L.a_U(3));
     a.R2 = h->arr(ib, L.a_R(2)); a.R3 = h->arr(ib, L.a_R(3));
-    a.K4u = keep_k4 ? h->arr(ib, L.a_K4()) : nullptr;
-    a.K4r = keep_k4 ? h->arr(ib, L.a_K4() + F) : nullptr;
+    const bool write_k = extra || (keep && s == S && S != 3);
+    a.K4u = write_k ? h->arr(ib, L.a_K4()) : nullptr;
+    a.K4r = write_k ? h->arr(ib, L.a_K4() + F) : nullptr;
+    const bool write_k3 = keep && S == 3 && s == 3;
+    a.K3u = write_k3 ? h->arr(ib, L.a_U(4)) : nullptr;
+    a.K3r = write_k3 ? h->arr(ib, L.a_R(4)) : nullptr;
     a.dt = dt;
     for (int d = 0; d < 3; ++d) {
       const double dx = L.dx(level, d);
       a.inv12dx2[d] = 1.0 / (12.0 * dx * dx);
-      a.ko[d] = L.ko_sigma / (64.0 * dx);
+      a.ko[d] = L.ko_sigma / ((L.ko_order == 9 ? 1024.0 : 64.0) * dx);
+      a.dx[d] = dx;
+      a.x0[d] = L.xlo[d] + ((double)a.b.lo[d] + (L.vertex ? 0.0 : 0.5)) * dx;
     }
+    a.rad_nb = (level == 0 && L.outer_bc == 1) ? L.g : 0;
     a.A = h->coupling();
     a.tmap = h->kmap_ok[ib] ? h->kmaps[ib].bytes : nullptr;
-    a.a_Yu = s == 1 ? L.a_state(yn) : L.a_U(s);
-    a.a_Yr = s == 1 ? L.a_state(yn) + F : L.a_R(s);
-    // reads: Y_s (2 arrays); + y_n (2) for s >= 2; + Y_2, Y_3 (4) for s = 4.  writes: 2 (+ 2 for k_4)
-    const double per = s == 1 ? 4.0 : (s < 4 ? 6.0 : (keep_k4 ? 12.0 : 10.0));
+    a.a_Yu = in_u;
+    a.a_Yr = in_r;
+    // reads: Y_s (2 arrays); + y_n (2) for s >= 2; + the earlier stage vectors of the final combine.  writes: 2 (+ 2 per kept slope)
+    double per = extra ? 4.0 : (s == 1 ? 4.0 : 6.0);
+    if (!extra && s == S) per += 2.0 * (S - 2) + (write_k || write_k3 ? 2.0 : 0.0);
     prof_begin(h, KIND_STAGE, 8.0 * per * F * cells(a.b));
     launch_stage_ko(a, h->stream);
     prof_end(h);
@@ -402,50 +461,80 @@ void stage_ko_level(Seq& q, int level, int s, double dt) {
   }
 }
 
-// ghosts of one stage's output arrays on level 0
+// ghosts of one stage's output arrays on level 0 (periodic boundary; the radiative boundary has no ghosts, S29)
 void periodic_stage_ko(Seq& q, int s) {
   const Layout& L = q.h->L;
+  if (L.outer_bc != 0) return;
   periodic_level0(q, L.a_U(s), L.F);
   periodic_level0(q, L.a_R(s), L.F);
 }
+void periodic_state_gen(Seq& q, int slot) {
+  const Layout& L = q.h->L;
+  if (L.outer_bc != 0) return;
+  periodic_level0(q, L.a_state(slot), L.V);
+}
 
 // Dense-output ghosts of ALL stage vectors of one level-step of `level` >= 1, one launch
-// per box. The parent stores (y_n, Y_2, Y_3, Y_4, k_4) per variable; with K_j = (Y_{j+1} - y_n)/(a_j h_p) for
-// j = 1..3 the value of eqs (15)-(18) at stage s,  y_n^p + h_p sum_j c^(s)_j K_j,  is the combination
-//   (1 - sum_{j<=3} c_j/a_j) y_n^p + sum_{j<=3} (c_j/a_j) Y_{j+1}^p + h_p c_4 k_4^p
-// — one (5 -> 4) problem for the u variables and one for the rho variables. At theta = 1/2 a third problem
+// per box. The parent stores, per variable, (y_n, Y_2, .., Y_S) and the slopes that cannot be recovered from them:
+//   RK4: (y_n, Y_2, Y_3, Y_4, k_4),   k_j = (Y_{j+1} - y_n)/(a_j h_p), j = 1..3
+//   RK3: (y_n, Y_2, Y_3, k_3, k_4),   k_1 = 2 (Y_2 - y_n)/h_p,  k_2 = (Y_3 - y_n)/(2 h_p) + (Y_2 - y_n)/h_p
+//   RK2: (y_n, Y_2, k_2),             k_1 = 2 (Y_2 - y_n)/h_p
+// so the value of the stage formulas,  y_n^p + h_p sum_j c^(s)_j k_j  (dense_coeffs_rk), is a fixed combination of
+// the stored arrays — one (5 -> S) problem for the u variables and one for the rho variables (RK2's three sources
+// are padded to five with zero coefficients: the tuned kernel's shape). At theta = 1/2 a third problem
 // prolongs the parent's new state into the shells of y_{n+1} (eq (10) at theta + 1/2 = 1, S8).
 void fill_level_dense_ko(Seq& q, int level, double theta, double dt) {
   sc_hierarchy* h = q.h;
   const Layout& L = h->L;
   const double hp = 2.0 * dt;
-  const int yn = q.cur[level], F = L.F;
+  const int yn = q.cur[level], F = L.F, S = L.integrator;
   const int pnew = q.cur[level - 1], pold = 1 - pnew;
-  const double as[3] = {0.5, 0.5, 1.0};
   for (int ib : L.level_boxes[level]) {
     GhostArgs a{};
     a.nprob = 2;
     for (int v = 0; v < 2; ++v) {  // v = 0: u variables, v = 1: rho variables
       GhostProblem& d = a.prob[v];
       d.nsrc = 5;
-      d.nout = 4;
-      d.src_arr[0] = L.a_state(pold) + v * F;
+      d.nout = S;
+      const int st_p = L.a_state(pold) + v * F;
+      d.src_arr[0] = st_p;
       d.dst_arr[0] = L.a_state(yn) + v * F;
-      for (int s = 2; s <= 4; ++s) {
-        d.src_arr[s - 1] = v ? L.a_R(s) : L.a_U(s);
-        d.dst_arr[s - 1] = v ? L.a_R(s) : L.a_U(s);
+      for (int s = 2; s <= S; ++s) d.dst_arr[s - 1] = v ? L.a_R(s) : L.a_U(s);
+      auto stage_arr = [&](int s) { return v ? L.a_R(s) : L.a_U(s); };
+      if (S == 4) {
+        for (int s = 2; s <= 4; ++s) d.src_arr[s - 1] = stage_arr(s);
+        d.src_arr[4] = L.a_K4() + v * F;
+      } else if (S == 3) {
+        d.src_arr[1] = stage_arr(2);
+        d.src_arr[2] = stage_arr(3);
+        d.src_arr[3] = stage_arr(4);           // k_3
+        d.src_arr[4] = L.a_K4() + v * F;       // k_4 = f(y_{n+1})
+      } else {
+        d.src_arr[1] = stage_arr(2);
+        d.src_arr[2] = L.a_K4() + v * F;       // k_2
+        d.src_arr[3] = d.src_arr[4] = st_p;    // padding, coefficients 0
       }
-      d.src_arr[4] = L.a_K4() + v * F;
-      for (int s = 1; s <= 4; ++s) {
+      for (int s = 1; s <= S; ++s) {
         double c[4];
-        dense_coeffs(s, theta, c);
-        double c0 = 1.0;
-        for (int j = 0; j < 3; ++j) {
-          d.coef[s - 1][1 + j] = c[j] / as[j];
-          c0 -= c[j] / as[j];
+        dense_coeffs_rk(S, s, theta, c);
+        double* co = d.coef[s - 1];
+        if (S == 4) {
+          const double as[3] = {0.5, 0.5, 1.0};
+          double c0 = 1.0;
+          for (int j = 0; j < 3; ++j) { co[1 + j] = c[j] / as[j]; c0 -= c[j] / as[j]; }
+          co[0] = c0;
+          co[4] = hp * c[3];
+        } else if (S == 3) {
+          co[1] = 2.0 * c[0] + c[1];
+          co[2] = 0.5 * c[1];
+          co[0] = 1.0 - co[1] - co[2];
+          co[3] = hp * c[2];
+          co[4] = hp * c[3];
+        } else {
+          co[1] = 2.0 * c[0];
+          co[0] = 1.0 - co[1];
+          co[2] = hp * c[1];
         }
-        d.coef[s - 1][0] = c0;
-        d.coef[s - 1][4] = hp * c[3];
       }
     }
     if (theta != 0.0) {
@@ -469,23 +558,24 @@ void fill_level_dense_ko(Seq& q, int level, double theta, double dt) {
 // sub-steps and restrict (those read and write this level's INTERIOR only: footprints lie 4 cells inside, S13).
 // In a captured step the fill is recorded on a second stream (a parallel branch of the graph) and joined before
 // the second sub-step's first stage kernel; eager / profiled steps issue it in place on the one stream.
-void prefill_second_substep(Seq& q, int level, double dt) {
+void prefill_second_substep(Seq& q, int level, double dt, bool in_line = false) {
   sc_hierarchy* h = q.h;
   const Layout& L = h->L;
   cudaStream_t main = h->stream;
-  if (q.capturing) {
+  const bool fork = q.capturing && !in_line;
+  if (fork) {
     cudaEventRecord(h->ev_fork[level], main);
     cudaStreamWaitEvent(h->side, h->ev_fork[level], 0);
     h->stream = h->side;
   }
-  if (L.ko_sigma > 0.0) fill_level_dense_ko(q, level, 0.5, dt);
+  if (L.general()) fill_level_dense_ko(q, level, 0.5, dt);
   else fill_level_dense(q, level, 0.5, dt);
   sibling_level(q, level, L.a_state(q.cur[level]), L.V);
-  if (q.capturing) {
+  if (fork) {
     cudaEventRecord(h->ev_join[level], h->side);
     h->stream = main;
   }
-  q.prefilled[level] = 1;
+  q.prefilled[level] = fork ? 1 : 2;  // 2: written in line on the main stream, nothing to join
 }
 // Measured (profiles/r01_v4.md): beside the children's kernels the fill costs nothing on 128^3 levels (cfg 3 0.806 ->
 // 0.798 ms per coarse step, cfg 4 184.4 -> 183.6 ms) but its CTAs disturb the bandwidth-bound stage kernels of 256^3
@@ -499,26 +589,26 @@ bool overlap_wanted(const sc_hierarchy* h, int level) {
 // true if the ghosts of the level-step about to start were prefilled (and, in a captured step, joins the branch)
 bool join_prefill(Seq& q, int level) {
   if (!q.prefilled[level]) return false;
+  if (q.prefilled[level] == 1 && q.capturing) cudaStreamWaitEvent(q.h->stream, q.h->ev_join[level], 0);
   q.prefilled[level] = 0;
-  if (q.capturing) cudaStreamWaitEvent(q.h->stream, q.h->ev_join[level], 0);
   return true;
 }
 
 void level_step_ko(Seq& q, int level, double dt, double theta) {
   const Layout& L = q.h->L;
-  const int yn = q.cur[level];
+  const int yn = q.cur[level], S = L.integrator;
   if (level == 0) {
-    if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
+    if (!q.l0_valid) periodic_state_gen(q, yn);
   } else if (!join_prefill(q, level)) {
     fill_level_dense_ko(q, level, theta, dt);
     sibling_level(q, level, L.a_state(yn), L.V);
   }
-  for (int s = 1; s <= 4; ++s) {
+  for (int s = 1; s <= S; ++s) {
     stage_ko_level(q, level, s, dt);
     if (level == 0) {
-      if (s < 4) periodic_stage_ko(q, s + 1);
-      else periodic_level0(q, L.a_state(1 - yn), L.V);
-    } else if (s < 4) {  // the stage vector just produced: ghosts inside a sibling take the sibling's Y_{s+1}
+      if (s < S) periodic_stage_ko(q, s + 1);
+      else periodic_state_gen(q, 1 - yn);
+    } else if (s < S) {  // the stage vector just produced: ghosts inside a sibling take the sibling's Y_{s+1}
       sibling_level(q, level, L.a_U(s + 1), L.F);
       sibling_level(q, level, L.a_R(s + 1), L.F);
     } else if (theta != 0.0) {
@@ -529,20 +619,20 @@ void level_step_ko(Seq& q, int level, double dt, double theta) {
   q.cur[level] = 1 - yn;
 }
 
-// non-subcycled step with dissipation (S11/S15): same-time prolongation of the parent's same stage vector
+// non-subcycled step of the general path (S11/S15): same-time prolongation of the parent's same stage vector
 void uniform_step_ko(Seq& q, double dt) {
   const Layout& L = q.h->L;
-  const int Lv = L.nlevels, F = L.F;
-  if (!q.l0_valid) periodic_level0(q, L.a_state(q.cur[0]), L.V);
+  const int Lv = L.nlevels, F = L.F, S = L.integrator;
+  if (!q.l0_valid) periodic_state_gen(q, q.cur[0]);
   for (int l = 1; l < Lv; ++l) {
     const int ca[2] = {L.a_state(q.cur[l]), L.a_state(q.cur[l]) + F};
     const int pa[2] = {L.a_state(q.cur[l - 1]), L.a_state(q.cur[l - 1]) + F};
     fill_level_same_time(q, l, 2, ca, pa);
     sibling_level(q, l, ca[0], L.V);
   }
-  for (int s = 1; s <= 4; ++s) {
+  for (int s = 1; s <= S; ++s) {
     for (int l = 0; l < Lv; ++l) stage_ko_level(q, l, s, dt);
-    if (s < 4) {
+    if (s < S) {
       periodic_stage_ko(q, s + 1);
       const int ca[2] = {L.a_U(s + 1), L.a_R(s + 1)};
       for (int l = 1; l < Lv; ++l) {
@@ -552,7 +642,7 @@ void uniform_step_ko(Seq& q, double dt) {
       }
     }
   }
-  periodic_level0(q, L.a_state(1 - q.cur[0]), L.V);
+  periodic_state_gen(q, 1 - q.cur[0]);
   q.l0_valid = true;
   for (int l = 1; l < Lv; ++l) {
     const int ca[2] = {L.a_state(1 - q.cur[l]), L.a_state(1 - q.cur[l]) + F};
@@ -567,7 +657,7 @@ void uniform_step_ko(Seq& q, double dt) {
 // One RK4 step of one level (eqs 1-9) with its ghost fills. theta: start of this step inside the parent's.
 void level_step(Seq& q, int level, double dt, double theta) {
   const Layout& L = q.h->L;
-  if (L.ko_sigma > 0.0) { level_step_ko(q, level, dt, theta); return; }
+  if (L.general()) { level_step_ko(q, level, dt, theta); return; }
   const int yn = q.cur[level];
   if (level == 0) {
     if (!q.l0_valid) periodic_level0(q, L.a_state(yn), L.V);
@@ -594,7 +684,11 @@ void level_step(Seq& q, int level, double dt, double theta) {
 void advance(Seq& q, int level, double dt, double theta) {
   level_step(q, level, dt, theta);
   if (level + 1 < q.h->L.nlevels) {
-    if (level >= 1 && theta == 0.0 && overlap_wanted(q.h, level)) prefill_second_substep(q, level, dt);
+    // RK3 (S28): the child's dense output reads k_4 = f(y_{n+1}) of this level, whose ghosts are the NEXT sub-step's
+    // Y_1 ghosts (S8): after a first sub-step they are written now, in line, by that sub-step's fill
+    const bool rk3 = q.h->L.integrator == 3;
+    if (level >= 1 && theta == 0.0 && (rk3 || overlap_wanted(q.h, level))) prefill_second_substep(q, level, dt, rk3);
+    if (rk3) stage_ko_level(q, level, 4, dt);
     advance(q, level + 1, 0.5 * dt, 0.0);
     advance(q, level + 1, 0.5 * dt, 0.5);
     restrict_level(q, level + 1);
@@ -604,7 +698,7 @@ void advance(Seq& q, int level, double dt, double theta) {
 // non-subcycled step of all levels (reading S11/S15)
 void uniform_step(Seq& q, double dt) {
   const Layout& L = q.h->L;
-  if (L.ko_sigma > 0.0) { uniform_step_ko(q, dt); return; }
+  if (L.general()) { uniform_step_ko(q, dt); return; }
   const int Lv = L.nlevels, F = L.F;
   // ghosts of y_n = (u_n, rho_n): from the parent's y_n after the last restriction
   if (!q.l0_valid) periodic_level0(q, L.a_state(q.cur[0]), L.V);
@@ -760,6 +854,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     std::vector<BoxView> sibs;
     for (int jb : h->L.level_boxes[h->L.boxes[ib].level])
       if (jb != (int)ib) sibs.push_back(h->L.boxes[jb].v);
+    if (!h->L.ops.is_default() || !ghost_tma_geometry_ok(h->L.boxes[ib].v)) continue;  // the direct-load kernel fills these
     build_ghost_tiles(h->L.boxes[ib].v, h->L.boxes[h->L.boxes[ib].parent].v, tl, &sibs);
     sc_hierarchy::BoxTiles& bt = h->tiles[ib];
     bt.n = (int)tl.size();
@@ -811,7 +906,8 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     const BoxInfo& b = h->L.boxes[ib];
     h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
-    h->kmap_ok[ib] = h->L.ko_sigma > 0.0 &&
+    if (h->L.vertex) h->tmap_ok[ib] = 0;  // vertex-centred grids run the direct-load kernels (restriction = injection)
+    h->kmap_ok[ib] = h->L.ko_sigma > 0.0 && h->L.integrator == 4 && h->L.fd_order == 4 && h->L.ko_order == 5 && h->L.outer_bc == 0 &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 5, h->kmaps[ib].bytes);
     h->gmap_ok[ib] = 1;
     for (int ax = 0; ax < 3; ++ax)

@@ -18,7 +18,7 @@ void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
 void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st);
 bool ghost_tma_takes(const GhostArgs& a);
 void ghost_box_dims(int axis, unsigned box[4]);
-void launch_restrict_ref(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st);
+void launch_restrict_ref(const RestrictArgs& a, cudaStream_t st);
 void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st);
 void launch_stage_ko_direct(const StageKOArgs& a, cudaStream_t st);
 void launch_stage_ko_tma(const StageKOArgs& a, cudaStream_t st);
@@ -35,15 +35,18 @@ int launch_stage(const StageArgs& a, cudaStream_t st) {
   return launch_stage_tma(a, st);
 }
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {
-  if (g_mode == 0 || !stage_ko_tma_takes(a)) launch_stage_ko_direct(a, st);
+  // the tuned kernel is the RK4 / 4th-order / delta^6 / periodic case; everything else runs on stage_gen
+  const bool tuned_case = a.integrator == 4 && a.fd_order == 4 && a.ko_order == 5 && a.rad_nb == 0;
+  if (g_mode == 0 || !tuned_case || !stage_ko_tma_takes(a)) launch_stage_ko_direct(a, st);
   else launch_stage_ko_tma(a, st);
 }
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st) {
-  if (g_mode == 0 || !ghost_tma_takes(a)) launch_ghost_fill_direct(a, st);
+  const bool s3 = a.np == 5 && a.pmin == -2;  // the tuned kernel has the quartic cell-centred operator built in
+  if (g_mode == 0 || !s3 || !ghost_tma_takes(a)) launch_ghost_fill_direct(a, st);
   else launch_ghost_fill_tma(a, st);
 }
 void launch_restrict(const RestrictArgs& a, cudaStream_t st) {
-  if (g_mode == 0) launch_restrict_ref(a.child, a.parent, a.V, a.ychild, a.yparent, st);
+  if (g_mode == 0 || a.nr != 6 || !a.tmap) launch_restrict_ref(a, st);
   else launch_restrict_opt(a, st);
 }
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128) {

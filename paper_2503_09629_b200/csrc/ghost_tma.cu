@@ -487,6 +487,8 @@ void ghost_box_dims(int axis, unsigned box[4]) {
   box[3] = 1;
 }
 
+bool ghost_tma_geometry_ok(const BoxView& child) { return child.g <= 4; }
+
 // problems the tuned kernel takes: exactly the (5 -> 4) and (<= 2 -> <= 2) shapes the scheduler produces
 bool ghost_tma_takes(const GhostArgs& a) {
   if (!a.tmaps || a.ntiles == 0 || a.child.g > 4) return false;

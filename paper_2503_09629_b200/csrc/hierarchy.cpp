@@ -22,12 +22,49 @@ static int fail(std::string* err, int code, const char* fmt, int a = 0, int b = 
   return code;
 }
 
+// Lagrange weights of the interpolant through `n` nodes evaluated at x (host, long double accumulation).
+static void lagrange(const double* nodes, int n, double x, double* w) {
+  for (int m = 0; m < n; ++m) {
+    long double v = 1.0L;
+    for (int q = 0; q < n; ++q)
+      if (q != m) v *= ((long double)x - nodes[q]) / ((long double)nodes[m] - nodes[q]);
+    w[m] = (double)v;
+  }
+}
+
+InterpOps make_interp_ops(int interp, int vertex) {
+  InterpOps P;
+  double nodes[10];
+  for (int m = 0; m < 10; ++m) P.w[0][m] = P.w[1][m] = P.r[m] = 0.0;
+  if (!vertex) {  // cell-centred (S1): fine centres at -+1/4 of the parent spacing; parent centre midway between fine cells
+    P.np = interp ? 9 : 5;
+    P.pmin = -(P.np / 2);
+    for (int m = 0; m < P.np; ++m) nodes[m] = P.pmin + m;
+    lagrange(nodes, P.np, -0.25, P.w[0]);
+    lagrange(nodes, P.np, 0.25, P.w[1]);
+    P.nr = interp ? 10 : 6;
+    P.rmin = -(P.nr / 2 - 1);
+    for (int m = 0; m < P.nr; ++m) nodes[m] = (P.rmin + m) - 0.5;
+    lagrange(nodes, P.nr, 0.0, P.r);
+  } else {        // vertex-centred (S31): even fine points coincide with parent points, odd ones sit midway
+    P.np = interp ? 10 : 6;
+    P.pmin = -(P.np / 2 - 1);
+    for (int m = 0; m < P.np; ++m) nodes[m] = P.pmin + m;
+    P.w[0][-P.pmin] = 1.0;
+    lagrange(nodes, P.np, 0.5, P.w[1]);
+    P.nr = 1;
+    P.rmin = 0;
+    P.r[0] = 1.0;
+  }
+  return P;
+}
+
 int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
   if (!d || !L) return fail(err, SC_ERR_INVALID_ARG, "null description");
   if (!d->boxes || d->nboxes < 1 || d->nlevels < 1) return fail(err, SC_ERR_INVALID_ARG, "no boxes / levels");
   if (d->ref_ratio != 2) return fail(err, SC_ERR_UNSUPPORTED, "ref_ratio must be 2 (got %d)", d->ref_ratio);
   if (d->ghost < MIN_GHOST || d->ghost > MAX_GHOST)
-    return fail(err, SC_ERR_UNSUPPORTED, "ghost width %d outside [2, 4]", d->ghost);
+    return fail(err, SC_ERR_UNSUPPORTED, "ghost width %d outside [2, 5]", d->ghost);
   if (d->nlevels > SC_MAX_LEVELS) return fail(err, SC_ERR_UNSUPPORTED, "too many levels (%d)", d->nlevels);
   if (d->nfields < 1 || d->nfields > MAX_FIELDS)
     return fail(err, SC_ERR_UNSUPPORTED, "nfields %d outside [1, 32]", d->nfields);
@@ -46,16 +83,36 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
 
   if (!(d->ko_sigma >= 0.0) || !std::isfinite(d->ko_sigma))
     return fail(err, SC_ERR_INVALID_ARG, "ko_sigma must be finite and >= 0");
-  if (d->ko_sigma > 0.0 && d->ghost < 3)
-    return fail(err, SC_ERR_UNSUPPORTED, "Kreiss-Oliger dissipation reads 3 ghost layers (ghost = %d)", d->ghost);
-
   if (d->fd_order != 0 && d->fd_order != 4 && d->fd_order != 8)
     return fail(err, SC_ERR_UNSUPPORTED, "fd_order must be 4 or 8 (got %d)", d->fd_order);
-  if (d->fd_order == 8 && (d->ghost < 4 || d->ko_sigma > 0.0))
-    return fail(err, SC_ERR_UNSUPPORTED, "8th-order differences read 4 ghost layers (ghost = %d) and run without dissipation", d->ghost);
+  const int fd = d->fd_order == 8 ? 8 : 4;
+  if (fd == 8 && d->ghost < 4)
+    return fail(err, SC_ERR_UNSUPPORTED, "8th-order differences read 4 ghost layers (ghost = %d)", d->ghost);
+  if (d->ko_order != 0 && d->ko_order != 5 && d->ko_order != 9)
+    return fail(err, SC_ERR_UNSUPPORTED, "ko_order must be 0, 5 or 9 (got %d)", d->ko_order);
+  const int ko = d->ko_order ? d->ko_order : (fd == 8 ? 9 : 5);
+  if (d->ko_sigma > 0.0 && d->ghost < (ko == 9 ? 5 : 3))
+    return fail(err, SC_ERR_UNSUPPORTED, "Kreiss-Oliger dissipation of order %d reads %d ghost layers", ko, ko == 9 ? 5 : 3);
+  if (d->integrator != 0 && d->integrator != 4 && d->integrator != 3 && d->integrator != 2)
+    return fail(err, SC_ERR_UNSUPPORTED, "integrator must be 4 (RK4), 3 (RK3) or 2 (RK2) (got %d)", d->integrator);
+  if (d->outer_bc != 0 && d->outer_bc != 1) return fail(err, SC_ERR_UNSUPPORTED, "outer_bc must be 0 or 1 (got %d)", d->outer_bc);
+  if ((d->interp_order != 0 && d->interp_order != 1) || (d->centering != 0 && d->centering != 1))
+    return fail(err, SC_ERR_UNSUPPORTED, "interp_order and centering must be 0 or 1");
+  if (d->outer_bc == 1)
+    for (int a = 0; a < 3; ++a)
+      if (!(d->xlo[a] < 0.0 && d->xhi[a] > 0.0))
+        return fail(err, SC_ERR_INVALID_ARG, "radiative boundary: the origin must lie strictly inside the domain (axis %d)", a);
 
   L->nlevels = d->nlevels;
-  L->fd_order = d->fd_order == 8 ? 8 : 4;
+  L->fd_order = fd;
+  L->ko_order = ko;
+  L->integrator = d->integrator ? d->integrator : 4;
+  L->outer_bc = d->outer_bc;
+  L->interp = d->interp_order;
+  L->vertex = d->centering;
+  L->ops = make_interp_ops(L->interp, L->vertex);
+  if (L->ops.nr > 1 && -L->ops.rmin > d->ghost)
+    return fail(err, SC_ERR_UNSUPPORTED, "the restriction reads %d ghost layers (ghost = %d)", -L->ops.rmin, d->ghost);
   L->ko_sigma = d->ko_sigma;
   L->g = d->ghost;
   L->F = d->nfields;
@@ -66,7 +123,7 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
   L->level_boxes.assign(d->nlevels, {});
 
   const int g = d->ghost;
-  const int margin = (g + 1) / 2 + 2;  // parent cells between a child's coverage and its parent's edge
+  const int margin = (g + 1) / 2 + L->ops.reach();  // parent cells between a child's coverage and its parent's edge
   for (int ib = 0; ib < d->nboxes; ++ib) {
     const sc_box& s = d->boxes[ib];
     if (s.level < 0 || s.level >= d->nlevels) return fail(err, SC_ERR_INVALID_ARG, "box %d: level %d out of range", ib, s.level);
@@ -132,7 +189,7 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
   // of 32 doubles, so every array starts on a 256-byte boundary
   unsigned long long off = 0;
   for (BoxInfo& b : L->boxes) {
-    b.narrays = 2 * L->V + 3 * L->F + (L->has_coupling ? 2 * L->F : 0) + (L->ko_sigma > 0.0 ? 3 * L->F + L->V : 0);
+    b.narrays = 2 * L->V + 3 * L->F + (L->has_coupling ? 2 * L->F : 0) + (L->general() ? 3 * L->F + L->V : 0);
     b.arena_offset = off;
     off += (unsigned long long)b.narrays * (unsigned long long)b.v.vol * sizeof(double);
   }

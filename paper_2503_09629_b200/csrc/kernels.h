@@ -53,31 +53,48 @@ int launch_stage(const StageArgs& a, cudaStream_t st);  // returns the number of
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128);
 
 // ------------------------------------------------------------------------------------------------
-// NEXT-1: one RK4 stage of the general formulation with Kreiss-Oliger dissipation (stage_ko.cu).
-// All pointers are field-0 arrays of one box; field f is f arrays further.
+// The GENERAL stage-by-stage formulation: one launch per RK stage, the stage
+// vectors stored whole. Used with Kreiss-Oliger dissipation (any order), with the RK3 / RK2 integrators and with the
+// radiative outer boundary — everything the two-launch formulation above does not cover (stage_gen.cu; the tuned
+// stage_ko_tma.cu takes the RK4 / 4th-order / delta^6 / periodic case). All pointers are field-0 arrays of one box;
+// field f is f arrays further.
+//   k = M Y_s,   M (U, R) = (R + Q U,  Lap_h U + A U + Q R)      (on level-0 boundary points: the radiative operator)
+//   RK4 (eqs 1-9):   s = 1..3: Y_{s+1} = y_n + a_s dt k;   s = 4: y_{n+1} = y_n + dt/6 (k_1 + 2 k_2 + 2 k_3 + k), K <- k
+//   RK3 (S28):       s = 1: Y_2 = y_n + dt/2 k;  s = 2: Y_3 = y_n - dt k_1 + 2 dt k;  s = 3: y_{n+1} = y_n + dt/6 (k_1 + 4 k_2 + k),
+//                    K3 <- k;  s = 4 (levels with a child): K <- k = M y_{n+1}, nothing else is written
+//   RK2 (S28):       s = 1: Y_2 = y_n + dt/2 k;  s = 2: y_{n+1} = y_n + dt k, K <- k
+// Earlier slopes are not stored: they are recovered from the stage vectors at the cell (k_1 = (Y_2 - y_n) / (dt/2), ...).
 // ------------------------------------------------------------------------------------------------
 struct StageKOArgs {
   BoxView b;
   int F;
-  int stage;             // 1..4
-  const double* Yu;      // u- and rho-part of the stage vector Y_s (stage 1: the state y_n), read with 3 ghost layers
+  int stage;             // 1..S (RK3 on a level with a child: also 4)
+  int integrator;        // 4 | 3 | 2
+  int fd_order;          // 4 | 8
+  int ko_order;          // 0: no dissipation (ko_sigma = 0); 5: delta^6; 9: delta^10
+  const double* Yu;      // u- and rho-part of the stage vector Y_s (stage 1: the state y_n), read with ghost layers
   const double* Yr;
   const double* yn_u;    // y_n, centre only
   const double* yn_r;
-  double* outU;          // stage < 4: Y_{s+1};  stage 4: y_{n+1}
+  double* outU;          // stage < S: Y_{s+1};  stage S: y_{n+1}
   double* outR;
-  const double* U2;      // stage 4, centre only: Y_2, Y_3 (Y_4 is Yu, Yr)
+  const double* U2;      // final stage, centre only: Y_2, Y_3 (the last stage vector is Yu, Yr)
   const double* U3;
   const double* R2;
   const double* R3;
-  double* K4u;           // stage 4: k_4, or null where no child reads it
+  double* K4u;           // slope kept for the child's dense output (see above), or null where no child reads it
   double* K4r;
+  double* K3u;           // RK3, stage 3: k_3, or null
+  double* K3r;
   double dt;
   double inv12dx2[3];    // 1 / (12 dx_a^2)
-  double ko[3];          // sigma / (64 dx_a)
+  double ko[3];          // sigma / (64 dx_a)  (ko_order 9: sigma / (1024 dx_a))
   const double* A;       // device F*F coupling, or null
   const void* tmap;      // host pointer to the box's stage_ko CUtensorMap (kind 5), or null -> direct-load kernel
   int a_Yu, a_Yr;        // array indices of Yu, Yr (field 0) in the tensor map
+  // radiative outer boundary (S29), level 0 only: cells within `rad_nb` of a face are boundary points
+  int rad_nb;            // 0: none
+  double x0[3], dx[3];   // position of cell 0 (centre or grid point) and spacing
 };
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st);
 
@@ -118,6 +135,8 @@ struct GhostArgs {
   BoxView child, parent;
   int F;
   int nprob;
+  int np, pmin;               // prolongation stencil: parent offsets pmin .. pmin + np - 1 (default 5, -2: S3)
+  double w[2][10];            // weights by parity of the fine index (direct kernel; the tuned kernel has S3's built in)
   const double* parent_base;  // array 0 of the parent box
   double* child_base;         // array 0 of the child box
   GhostProblem prob[GF_MAX_PROB];
@@ -130,6 +149,7 @@ struct GhostArgs {
 // left out (the same-level exchange a7 overwrites every one of them right after the fill).
 void build_ghost_tiles(const BoxView& child, const BoxView& parent, std::vector<GhostTile>& tiles,
                        const std::vector<BoxView>* siblings = nullptr);
+bool ghost_tma_geometry_ok(const BoxView& child);  // ghost widths the tuned kernel's tiles cover
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st);
 
 // a4: periodic ghost fill of `narrays` consecutive arrays of the level-0 box (reading S9).
@@ -139,6 +159,8 @@ void launch_periodic_fill(const BoxView& b, int narrays, double* y, cudaStream_t
 struct RestrictArgs {
   BoxView child, parent;
   int V;
+  int nr, rmin;          // restriction stencil: fine offsets rmin .. rmin + nr - 1 around 2J (default 6, -2: S4; 1, 0: injection)
+  double r[10];
   const double* ychild;  // child state, component 0 (read with 2 ghost layers)
   double* yparent;       // parent state, component 0
   const void* tmap;      // host pointer to the child's kind-1 CUtensorMap, or null -> direct-load kernel

@@ -12,17 +12,6 @@
 namespace sc {
 
 // ------------------------------------------------------------------------------------------------
-// weights (device constants; written out as exact binary fractions / rationals)
-//   prolongation: quartic Lagrange at +-1/4 through offsets -2..2   (reading S3)
-//   restriction:  quintic Lagrange at 0 through -5/2..5/2          (reading S4)
-// ------------------------------------------------------------------------------------------------
-__device__ __constant__ double c_wp[2][5] = {
-    {-45.0 / 2048.0, 420.0 / 2048.0, 1890.0 / 2048.0, -252.0 / 2048.0, 35.0 / 2048.0},   // parity 0: x = -1/4
-    {35.0 / 2048.0, -252.0 / 2048.0, 1890.0 / 2048.0, 420.0 / 2048.0, -45.0 / 2048.0}};  // parity 1: x = +1/4
-__device__ __constant__ double c_wr[6] = {3.0 / 256.0,   -25.0 / 256.0, 150.0 / 256.0,
-                                          150.0 / 256.0, -25.0 / 256.0, 3.0 / 256.0};
-
-// ------------------------------------------------------------------------------------------------
 // shell enumeration: q in [0, nshell) -> ghost cell (i,j,k); six slabs (z-lo, z-hi, y-lo, y-hi, x-lo, x-hi)
 // ------------------------------------------------------------------------------------------------
 long long ghost_cell_count(const BoxView& b) {
@@ -154,9 +143,9 @@ void launch_stage_direct(const StageArgs& a, cudaStream_t st) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3  ghost fill, direct version: one thread per (ghost cell, field), 125-point gather per source
+// a3  ghost fill, direct version: one thread per (ghost cell, field), np^3-point gather per source (125 for S3)
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) ghost_fill_direct(GhostArgs a, int ip, long long nshell) {
+__global__ void __launch_bounds__(128) ghost_fill_direct(const __grid_constant__ GhostArgs a, int ip, long long nshell) {
   const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int f = blockIdx.y;
   if (q >= nshell) return;
@@ -173,12 +162,15 @@ __global__ void __launch_bounds__(128) ghost_fill_direct(GhostArgs a, int ip, lo
   double acc[GF_MAX_OUT];
 #pragma unroll
   for (int o = 0; o < GF_MAX_OUT; ++o) acc[o] = 0.0;
-  for (int cc = -2; cc <= 2; ++cc)
-    for (int bb = -2; bb <= 2; ++bb) {
-      const long long row = cell_offset(a.parent, J[0], J[1] + bb, J[2] + cc);
-      const double wyz = c_wp[p[1]][bb + 2] * c_wp[p[2]][cc + 2];
-      for (int aa = -2; aa <= 2; ++aa) {
-        const double w = wyz * c_wp[p[0]][aa + 2];
+  // tensor Lagrange stencil of a.np points per axis starting a.pmin parent cells from the containing one (S3; S30, S31)
+  for (int cc = 0; cc < a.np; ++cc)
+    for (int bb = 0; bb < a.np; ++bb) {
+      const double wyz = a.w[p[1]][bb] * a.w[p[2]][cc];
+      if (wyz == 0.0) continue;  // vertex-centred grids: a point ON a parent point has one non-zero weight per axis
+      const long long row = cell_offset(a.parent, J[0] + a.pmin, J[1] + a.pmin + bb, J[2] + a.pmin + cc);
+      for (int aa = 0; aa < a.np; ++aa) {
+        const double w = wyz * a.w[p[0]][aa];
+        if (w == 0.0) continue;
         double v[GF_MAX_SRC];
 #pragma unroll
         for (int s = 0; s < GF_MAX_SRC; ++s)
@@ -274,36 +266,36 @@ void launch_max_abs(const BoxView& b, const double* padded, unsigned long long* 
 }
 
 // ------------------------------------------------------------------------------------------------
-// a5  restriction, one thread per parent cell, 216-point gather
+// a5  restriction, one thread per parent cell, nr^3-point gather (216 for S4; 1 for injection on vertex-centred grids)
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) restrict_ref(BoxView ch, BoxView pa, const double* yc, double* yp) {
+__global__ void __launch_bounds__(128) restrict_ref(const __grid_constant__ RestrictArgs a) {
+  const BoxView& ch = a.child;
+  const BoxView& pa = a.parent;
   const int I = blockIdx.x * blockDim.x + threadIdx.x;
   const int J = blockIdx.y;
   const int nz = ch.n[2] / 2;
   const int K = blockIdx.z % nz;
   const int c = blockIdx.z / nz;
   if (I >= ch.n[0] / 2) return;
-  const double* s = yc + (long long)c * ch.vol;
+  const double* s = a.ychild + (long long)c * ch.vol;
   double sz = 0.0;
-  for (int cc = 0; cc < 6; ++cc) {
+  for (int cc = 0; cc < a.nr; ++cc) {
     double sy = 0.0;
-    for (int bb = 0; bb < 6; ++bb) {
+    for (int bb = 0; bb < a.nr; ++bb) {
       double sx = 0.0;
-      const long long row = cell_offset(ch, 2 * I - 2, 2 * J - 2 + bb, 2 * K - 2 + cc);
-#pragma unroll
-      for (int aa = 0; aa < 6; ++aa) sx += c_wr[aa] * s[row + aa];
-      sy += c_wr[bb] * sx;
+      const long long row = cell_offset(ch, 2 * I + a.rmin, 2 * J + a.rmin + bb, 2 * K + a.rmin + cc);
+      for (int aa = 0; aa < a.nr; ++aa) sx += a.r[aa] * s[row + aa];
+      sy += a.r[bb] * sx;
     }
-    sz += c_wr[cc] * sy;
+    sz += a.r[cc] * sy;
   }
   const int P0 = (ch.lo[0] >> 1) - pa.lo[0], P1 = (ch.lo[1] >> 1) - pa.lo[1], P2 = (ch.lo[2] >> 1) - pa.lo[2];
-  yp[(long long)c * pa.vol + cell_offset(pa, P0 + I, P1 + J, P2 + K)] = sz;
+  a.yparent[(long long)c * pa.vol + cell_offset(pa, P0 + I, P1 + J, P2 + K)] = sz;
 }
 
-void launch_restrict_ref(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp,
-                         cudaStream_t st) {
-  dim3 grd((ch.n[0] / 2 + 127) / 128, ch.n[1] / 2, (ch.n[2] / 2) * V);
-  restrict_ref<<<grd, 128, 0, st>>>(ch, pa, yc, yp);
+void launch_restrict_ref(const RestrictArgs& a, cudaStream_t st) {
+  dim3 grd((a.child.n[0] / 2 + 127) / 128, a.child.n[1] / 2, (a.child.n[2] / 2) * a.V);
+  restrict_ref<<<grd, 128, 0, st>>>(a);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -21,7 +21,7 @@
 
 namespace sc {
 
-void launch_restrict_ref(const BoxView& ch, const BoxView& pa, int V, const double* yc, double* yp, cudaStream_t st);
+void launch_restrict_ref(const RestrictArgs& a, cudaStream_t st);
 
 namespace {
 constexpr int RPX = 32, RPY = 6;              // parent cells per CTA in x, y
@@ -139,7 +139,7 @@ size_t restrict_smem() { return (size_t)(NSTR * RSTAGE + 2 * RFY * SXP) * 8 + NS
 void restrict_box_dims(unsigned box[4]) { box[0] = RPITCH; box[1] = RFY; box[2] = 2; box[3] = 1; }
 
 void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st) {
-  if (!a.tmap) { launch_restrict_ref(a.child, a.parent, a.V, a.ychild, a.yparent, st); return; }
+  if (!a.tmap) { launch_restrict_ref(a, st); return; }
   static const int forced = [] { const char* e = getenv("SC_RCHUNKS"); return e ? atoi(e) : 0; }();
   static const int nsm = [] {
     int dev = 0, n = 148;

@@ -3,7 +3,7 @@
 // Data layout in HBM. A box owns a run of equally sized ARRAYS; an array is one
 // scalar grid function on the box padded by g ghost cells, stored [z][y][x] with x contiguous:
 //     offset(i,j,k) = (XOFF + i) + px * ((j + g) + py * (k + g)),   i in [-g, n0+g) etc.
-// XOFF = 4 doubles puts interior cell i = 0 on a 32-byte sector boundary; px is a multiple of 16 doubles so
+// XOFF = 8 doubles puts interior cell i = 0 on a 64-byte boundary; px is a multiple of 16 doubles so
 // every row starts on a 128-byte line (and every TMA global stride is a multiple of 16 bytes).
 // Arrays of a box, in order (F = number of fields, V = 2F):
 //     [0, V)            state slot 0:  u_0..u_{F-1}, rho_0..rho_{F-1}
@@ -36,8 +36,8 @@
 
 namespace sc {
 
-constexpr int XOFF = 4;        // doubles of left padding in x (>= max ghost width)
-constexpr int MAX_GHOST = 4;
+constexpr int XOFF = 8;        // doubles of left padding in x (>= max ghost width; a multiple of 4: 32-byte sectors)
+constexpr int MAX_GHOST = 5;
 constexpr int MIN_GHOST = 2;   // stencil radius of the 4th-order Laplacian; restriction reads 2 layers
 constexpr int MAX_FIELDS = 32;
 
@@ -56,6 +56,18 @@ struct BoxView {
 SC_HD inline long long cell_offset(const BoxView& b, int i, int j, int k) {
   return (long long)(XOFF + i) + (long long)b.px * ((long long)(j + b.g) + (long long)b.py * (k + b.g));
 }
+
+// Prolongation / restriction stencils (S3, S4 and their NEXT-3 variants S30, S31), built on the host by
+// make_interp_ops() from the Lagrange formula. Prolongation: parent offsets pmin .. pmin + np - 1 around the parent
+// index I >> 1, weights w[parity of I][.]; restriction: fine offsets rmin .. rmin + nr - 1 around 2J.
+struct InterpOps {
+  int np = 5, pmin = -2, nr = 6, rmin = -2;
+  double w[2][10];
+  double r[10];
+  int reach() const { return -pmin > pmin + np - 1 ? -pmin : pmin + np - 1; }
+  bool is_default() const { return np == 5 && nr == 6; }
+};
+InterpOps make_interp_ops(int interp, int vertex);
 
 struct BoxInfo {
   BoxView v;
@@ -77,6 +89,13 @@ struct Layout {
   bool has_coupling = false;
   double ko_sigma = 0.0;                    // > 0: Kreiss-Oliger dissipation, general stage-by-stage path
   int fd_order = 4;                         // 4 (S2) or 8: centred differences of the RHS
+  int ko_order = 5;                         // 5: delta^6, 9: delta^10 (eq 36)
+  int integrator = 4;                       // 4 | 3 | 2 (S28)
+  int outer_bc = 0;                         // 0 periodic | 1 radiative (S29)
+  int interp = 0, vertex = 0;               // S30, S31
+  InterpOps ops;                            // prolongation / restriction stencils and weights in use
+  // the general stage-by-stage path (stage_gen.cu): whole stage vectors stored, one launch per stage
+  bool general() const { return ko_sigma > 0.0 || integrator != 4 || outer_bc != 0; }
   double dx(int level, int a) const { return (xhi[a] - xlo[a]) / ((double)domain[a] * (double)(1u << level)); }
   // first array index of each role
   int a_state(int slot) const { return slot * V; }

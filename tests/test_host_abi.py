@@ -93,11 +93,26 @@ def test_nesting_validator_rejects_bad_hierarchies(built):
     assert rc(base + [B(2, (40, 40, 40), (16, 16, 16))], nlevels=3)[0] == SC_ERR_NESTING  # empty level 1
     assert rc(base, ref_ratio=4)[0] == SC_ERR_UNSUPPORTED
     assert rc(base, ghost=1)[0] == SC_ERR_UNSUPPORTED
-    assert rc(base, ghost=5)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, ghost=6)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, ghost=5)[0] != SC_ERR_UNSUPPORTED
     assert rc(base, fd_order=8)[0] == SC_ERR_UNSUPPORTED            # 8th-order differences read 4 ghost layers
     assert rc(base, fd_order=6)[0] == SC_ERR_UNSUPPORTED
-    assert rc(base, ghost=4, fd_order=8, ko_sigma=0.1)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, ghost=4, fd_order=8, ko_sigma=0.1)[0] == SC_ERR_UNSUPPORTED   # eq 36 with r = 8: delta^10 reads 5 layers
+    assert rc(base, ghost=4, fd_order=8, ko_sigma=0.1, ko_order=5)[0] != SC_ERR_UNSUPPORTED  # the paper's production pair
+    assert rc(base, ghost=5, fd_order=8, ko_sigma=0.1)[0] != SC_ERR_UNSUPPORTED
     assert rc(base, ghost=4, fd_order=8)[0] != SC_ERR_UNSUPPORTED
+    # NEXT-3 / NEXT-4 options
+    assert rc(base, integrator=5)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, integrator=3)[0] != SC_ERR_UNSUPPORTED and rc(base, integrator=2)[0] != SC_ERR_UNSUPPORTED
+    assert rc(base, outer_bc=2)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, outer_bc=1, xlo=(0.5, -1.0, -1.0), xhi=(2.0, 1.0, 1.0))[0] == SC_ERR_INVALID_ARG  # origin outside
+    assert rc(base, ko_order=7)[0] == SC_ERR_UNSUPPORTED
+    assert rc(base, interp=1)[0] == SC_ERR_UNSUPPORTED              # the 10-point restriction reads 4 ghost layers
+    assert rc(base, interp=1, ghost=4)[0] != SC_ERR_UNSUPPORTED
+    assert rc(base + [B(1, (8, 16, 16), (16, 16, 16))], vertex=1)[0] == SC_ERR_NESTING   # vertex: margin 5
+    assert rc(base + [B(1, (10, 16, 16), (12, 16, 16))], vertex=1)[0] != SC_ERR_NESTING
+    assert rc(base + [B(1, (10, 16, 16), (12, 16, 16))], interp=1, ghost=4)[0] == SC_ERR_NESTING  # 9-point: margin 6
+    assert rc(base + [B(1, (12, 16, 16), (8, 16, 16))], interp=1, ghost=4)[0] != SC_ERR_NESTING
     assert rc(base, nfields=0)[0] == SC_ERR_UNSUPPORTED
     assert rc(base, xlo=(1.0, -1.0, -1.0), xhi=(1.0, 1.0, 1.0))[0] == SC_ERR_INVALID_ARG
     r, msg = rc(base + [B(1, (6, 16, 16), (16, 16, 16))])
