@@ -182,6 +182,13 @@ int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t 
  * for a run that blew up, without copying the state. Synchronises the stream. */
 int32_t sc_debug_max_abs(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp, double* out);
 
+/* Debug: the scheduler's CUDA-graph bookkeeping since creation. A coarse step is captured once per (mode, state-slot
+ * phase) and replayed; a step with a different dt_coarse re-records the launch sequence on the host and updates the
+ * parameters of the existing executable graph in place, so `instantiations` and `cached` stay bounded by the number of
+ * phases however many distinct step sizes a run uses. Out pointers: HOST, may be NULL. */
+int32_t sc_debug_graph_stats(const sc_hierarchy* h, uint64_t* captures, uint64_t* instantiations, uint64_t* updates,
+                             uint64_t* cached);
+
 /* Per-kernel timing for the roofline report. sc_profile(h, 1): from now on sc_step launches its kernels
  * one by one (no graph replay) with a CUDA-event pair around each on the hierarchy's stream;
  * sc_profile(h, 0) stops and discards the records. sc_profile_read sums, over the records since

@@ -1,7 +1,8 @@
 // capi.cu — the C ABI of libsubcycle (include/subcycle.h) and the level scheduler:
 // the Berger–Oliger recursion of PAPER.md:111-119 (steps 1-7) unrolled on the host into a fixed sequence
-// of kernel launches on one CUDA stream, captured once per (mode, dt, buffer phase) into a CUDA graph
-// and replayed. No host synchronisation inside a step.
+// of kernel launches on one CUDA stream, captured once per (mode, buffer phase) into a CUDA graph and replayed
+// (another dt_coarse re-records the sequence and updates the executable graph's parameters in place). No host
+// synchronisation inside a step.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -23,21 +24,24 @@ void select_kernels(int mode);
 
 using namespace sc;
 
+// One executable graph per (mode, state-slot phase). The step size is NOT part of the key: a step with another
+// dt_coarse re-records the same launch sequence (host work only) and updates the executable graph's kernel
+// parameters in place (cudaGraphExecUpdate), so an adaptive-dt caller neither instantiates nor leaks a graph per step.
 struct GraphKey {
   int sub;
-  uint64_t dt_bits;
   uint32_t phase;
   bool operator<(const GraphKey& o) const {
     if (sub != o.sub) return sub < o.sub;
-    if (dt_bits != o.dt_bits) return dt_bits < o.dt_bits;
     return phase < o.phase;
   }
 };
 struct GraphEntry {
   cudaGraphExec_t exec = nullptr;
+  uint64_t dt_bits = 0;  // the step size the executable graph's parameters currently hold
   uint64_t launches = 0;
   std::vector<int> cur_after;
 };
+constexpr size_t kMaxGraphs = 64;  // far above the phases a run visits (2 per mode); beyond it the cache is flushed
 
 struct sc_hierarchy {
   Layout L;
@@ -62,6 +66,7 @@ struct sc_hierarchy {
   int debug_kind = 0;
   std::string debug_fail;
   std::map<GraphKey, GraphEntry> graphs;
+  uint64_t n_captures = 0, n_instantiations = 0, n_updates = 0;  // sc_debug_graph_stats
   struct BoxTiles { GhostTile* dev = nullptr; int n = 0; };
   std::vector<BoxTiles> tiles;    // per box (levels >= 1): ghost-shell tile list on the device
   struct alignas(64) TMap { unsigned char bytes[128]; };
@@ -965,37 +970,68 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
   if (!h) { set_error("null hierarchy"); return SC_ERR_INVALID_ARG; }
   if (!std::isfinite(dt_coarse) || dt_coarse <= 0.0) { set_error("dt_coarse must be finite and > 0"); return SC_ERR_INVALID_ARG; }
   subcycling = subcycling ? 1 : 0;
-  Seq q{h, h->cur, h->l0_ghosts_valid, 0};
+  Seq q{};
+  q.h = h;
+  q.cur = h->cur;
+  q.l0_valid = h->l0_ghosts_valid;
   q.prefilled.assign(h->L.nlevels, 0);
   if (!h->use_graph || h->profiling) {
     record_step(q, dt_coarse, subcycling);
     SC_CUDA(cudaGetLastError());
     h->launches += q.n;
   } else {
-    GraphKey key{subcycling, 0, 0};
-    memcpy(&key.dt_bits, &dt_coarse, sizeof(double));
+    GraphKey key{subcycling, 0};
+    uint64_t dt_bits = 0;
+    memcpy(&dt_bits, &dt_coarse, sizeof(double));
     for (int l = 0; l < h->L.nlevels; ++l) key.phase |= (uint32_t)(h->cur[l] ? 1 : 0) << l;
     if (h->l0_ghosts_valid) key.phase |= 1u << 31;
     auto it = h->graphs.find(key);
-    if (it == h->graphs.end()) {
+    if (it == h->graphs.end() || it->second.dt_bits != dt_bits) {
       cudaGraph_t g = nullptr;
       SC_CUDA(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
       q.capturing = true;
       record_step(q, dt_coarse, subcycling);
       cudaError_t le = cudaGetLastError();
       cudaError_t ee = cudaStreamEndCapture(h->stream, &g);
+      ++h->n_captures;
       if (le != cudaSuccess || ee != cudaSuccess) {
         set_error(std::string("graph capture failed: ") + cudaGetErrorString(le != cudaSuccess ? le : ee));
         if (g) cudaGraphDestroy(g);
         return SC_ERR_CUDA;
       }
-      GraphEntry e;
-      cudaError_t ie = cudaGraphInstantiate(&e.exec, g, 0);
+      bool updated = false;
+      if (it != h->graphs.end()) {  // same launch sequence, other step size: new parameters into the existing executable
+        cudaGraphExecUpdateResultInfo info;
+        if (cudaGraphExecUpdate(it->second.exec, g, &info) == cudaSuccess) {
+          updated = true;
+          ++h->n_updates;
+        } else {
+          cudaGetLastError();
+          cudaGraphExecDestroy(it->second.exec);
+          h->graphs.erase(it);
+          it = h->graphs.end();
+        }
+      }
+      if (!updated) {
+        if (h->graphs.size() >= kMaxGraphs) {
+          for (auto& kv : h->graphs)
+            if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+          h->graphs.clear();
+        }
+        GraphEntry e;
+        cudaError_t ie = cudaGraphInstantiate(&e.exec, g, 0);
+        ++h->n_instantiations;
+        if (ie != cudaSuccess) {
+          cudaGraphDestroy(g);
+          set_error(std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ie));
+          return SC_ERR_CUDA;
+        }
+        it = h->graphs.emplace(key, e).first;
+      }
       cudaGraphDestroy(g);
-      if (ie != cudaSuccess) { set_error(std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ie)); return SC_ERR_CUDA; }
-      e.launches = q.n;
-      e.cur_after = q.cur;
-      it = h->graphs.emplace(key, e).first;
+      it->second.dt_bits = dt_bits;
+      it->second.launches = q.n;
+      it->second.cur_after = q.cur;
     }
     SC_CUDA(cudaGraphLaunch(it->second.exec, h->stream));
     h->launches += it->second.launches;
@@ -1014,6 +1050,16 @@ int32_t sc_read_level(sc_hierarchy* h, int32_t level, int32_t box, int32_t comp,
   if (rc != SC_OK) return rc;
   if (!dst) { set_error("null dst"); return SC_ERR_INVALID_ARG; }
   return read_array(h, gb, h->arr(gb, h->L.a_state(h->cur[level]) + comp), dst, 0, dst_on_device);
+}
+
+int32_t sc_debug_graph_stats(const sc_hierarchy* h, uint64_t* captures, uint64_t* instantiations, uint64_t* updates,
+                             uint64_t* cached) {
+  if (!h) { set_error("null hierarchy"); return SC_ERR_INVALID_ARG; }
+  if (captures) *captures = h->n_captures;
+  if (instantiations) *instantiations = h->n_instantiations;
+  if (updates) *updates = h->n_updates;
+  if (cached) *cached = h->graphs.size();
+  return SC_OK;
 }
 
 double sc_time(const sc_hierarchy* h) { return h ? h->time : 0.0; }

@@ -199,6 +199,43 @@ def test_graph_replay_equals_eager(monkeypatch):
     assert G1.sc_launch_count() == G2.sc_launch_count() > 0
 
 
+def test_varying_dt_updates_the_graph_in_place(monkeypatch):
+    """An adaptive-dt caller: 300 coarse steps with 300 distinct step sizes, modes alternating. The executable graphs are
+    keyed by (mode, slot phase) only; a new dt re-records the launches and updates the existing executable in place:
+    a handful of instantiations, a bounded cache, no growth of device memory, and the same bits as eager launches."""
+    import torch
+    w = wl.ragged_small()
+    G1 = sc.Hierarchy.from_workload(w)
+    monkeypatch.setenv("SC_GRAPH", "0")
+    G2 = sc.Hierarchy.from_workload(w)
+    monkeypatch.delenv("SC_GRAPH")
+    free0 = None
+    for i in range(300):
+        dt = w.dt_coarse * (0.5 + 0.001 * i)
+        sub = (i // 3) % 2 == 0
+        G1.sc_step(dt, sub)
+        G2.sc_step(dt, sub)
+        if i == 20:
+            G1.synchronize()
+            free0 = torch.cuda.mem_get_info()[0]
+    G1.synchronize()
+    st = G1.sc_debug_graph_stats()
+    assert st["instantiations"] <= 8 and st["cached"] <= 8, st
+    assert st["updates"] >= 280 and st["captures"] == st["updates"] + st["instantiations"], st
+    assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20), (free0, torch.cuda.mem_get_info()[0])
+    for l in range(w.nlevels):
+        for ib in range(len(w.level_boxes(l))):
+            for c in range(w.ncomp):
+                assert np.array_equal(G1.sc_debug_read_padded(l, ib, c), G2.sc_debug_read_padded(l, ib, c))
+    assert G2.sc_debug_graph_stats()["captures"] == 0
+    # the same dt again: pure replay
+    G1.sc_step(w.dt_coarse, True)
+    G1.sc_step(w.dt_coarse, True)
+    G1.sc_step(w.dt_coarse, True)
+    st2 = G1.sc_debug_graph_stats()
+    assert st2["captures"] <= st["captures"] + 2, (st, st2)
+
+
 def test_error_paths_on_device():
     w = wl.cfg1()
     G = sc.Hierarchy.from_workload(w)
