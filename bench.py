@@ -33,7 +33,7 @@ METRIC = "grid-point updates/s (all levels, fp64 RK4)"
 UNIT = "updates/s"
 
 
-def pick_workload(idx: int, sigma: float = 0.0, cut: int = 1, fd_order: int = 4):
+def pick_workload(idx: int, sigma: float = 0.0, cut: int = 1, fd_order: int = 4, opts=None):
     w = {1: wl.cfg1, 2: lambda: wl.cfg2(128), 3: wl.cfg3, 4: wl.cfg4, 5: wl.cfg5}[idx]()
     if cut > 1:
         w = wl.cut_finest(w, cut)
@@ -43,7 +43,19 @@ def pick_workload(idx: int, sigma: float = 0.0, cut: int = 1, fd_order: int = 4)
     if sigma:
         w.ko_sigma = sigma
         w.name += f" + Kreiss-Oliger sigma={sigma}"
+    for k, v in (opts or {}).items():  # NEXT-3 / NEXT-4 options: ko_order, integrator, outer_bc, interp, vertex, ghost
+        if v is not None and v != getattr(w, k):
+            setattr(w, k, v)
+            w.name += f" + {k}={v}"
+    if w.ko_sigma and (w.ko_order == 9 or (w.ko_order == 0 and w.fd_order == 8)) and w.ghost < 5:
+        w.ghost = 5  # delta^10 reads five ghost layers
+        w.name += " (ghost 5)"
     return w
+
+
+def workload_opts(args):
+    return {"ko_order": args.ko_order, "integrator": args.integrator, "outer_bc": args.outer_bc,
+            "interp": args.interp, "vertex": args.vertex, "ghost": args.ghost}
 
 
 def measured_peaks():
@@ -66,9 +78,8 @@ def oracle_sample(w, max_levels: int):
     boxes = [b for b in w.boxes if b.level < max_levels]
     s = wl.Workload(w.name + f" [levels 0..{max_levels - 1}]", boxes, w.domain_cells, w.nfields, w.ghost,
                     w.xlo, w.xhi, w.coupling, w.coarse_steps, w.init, ko_sigma=w.ko_sigma, fd_order=w.fd_order)
-    for k in ("integrator", "boundary", "ko_order", "interp_order"):  # options added after round 1, if present
-        if hasattr(w, k):
-            setattr(s, k, getattr(w, k))
+    for k in ("integrator", "outer_bc", "ko_order", "interp", "vertex"):  # the NEXT-3 / NEXT-4 options
+        setattr(s, k, getattr(w, k))
     return s, f"SAMPLE: levels 0..{max_levels - 1} of {w.nlevels} ({'+'.join(str(b.n[0]) + '^3' for b in boxes)})"
 
 
@@ -112,7 +123,8 @@ def time_oracle(w, steps: int, warmup: int, sub: bool, max_levels: int, threads:
 def config_dict(w, sub: bool, world: int):
     """The `config` object of the JSON line; the same for the GPU arm and the reference arm."""
     return {"workload": w.name, "mode": "subcycled" if sub else "uniform", "ghost": w.ghost, "nfields": w.nfields,
-            "ko_sigma": w.ko_sigma, "fd_order": w.fd_order, "dt_coarse": w.dt_coarse,
+            "ko_sigma": w.ko_sigma, "fd_order": w.fd_order, "ko_order": w.ko_order, "integrator": w.integrator,
+            "outer_bc": w.outer_bc, "interp": w.interp, "vertex": w.vertex, "dt_coarse": w.dt_coarse,
             "updates_per_step": w.updates_per_coarse_step(sub), "zone_cycles_per_step": w.zone_cycles_per_coarse_step(),
             "l2": "inputs larger than L2 (state and stage buffers of every level stream through once per launch)",
             "parallelism": "replicas only" if world > 1 else "1 GPU"}
@@ -122,7 +134,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    w = pick_workload(args.config, args.sigma, args.cut_finest, args.fd_order)
+    w = pick_workload(args.config, args.sigma, args.cut_finest, args.fd_order, workload_opts(args))
     sub = args.mode == "sub"
     r = time_oracle(w, max(1, args.steps), min(args.warmup, 1), sub, max_levels=args.oracle_levels)
     ms = 1e3 * r.pop("_seconds") / r.pop("_steps")
@@ -218,11 +230,12 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    w = pick_workload(args.config, args.sigma, args.cut_finest, args.fd_order)
+    w = pick_workload(args.config, args.sigma, args.cut_finest, args.fd_order, workload_opts(args))
     sub = args.mode == "sub"
     dt = w.dt_coarse
     H = sc.Hierarchy(w.boxes, w.domain_cells, w.nfields, w.ghost, w.xlo, w.xhi, w.coupling, device=f"cuda:{local}",
-                     ko_sigma=w.ko_sigma, fd_order=w.fd_order)
+                     ko_sigma=w.ko_sigma, fd_order=w.fd_order, ko_order=w.ko_order, integrator=w.integrator,
+                     outer_bc=w.outer_bc, interp=w.interp, vertex=w.vertex)
 
     # inputs: seeded synthetic state, staged in pinned host memory (also the e2e source buffers)
     host_in, host_out = {}, {}
@@ -275,6 +288,14 @@ def run_gpu(args):
     dom = max(kinds, key=lambda k: kinds[k]["ms_total"])
     ksum = sum(k["ms_total"] for k in kinds.values())
     wkey = f"cfg{args.config}/{args.mode}/sigma{args.sigma:g}/cut{args.cut_finest}/fd{args.fd_order}"
+    if (w.ko_order, w.integrator, w.outer_bc, w.interp, w.vertex) != (0, 4, 0, 0, 0):
+        wkey += f"/ko{w.ko_order}/rk{w.integrator}/bc{w.outer_bc}/ip{w.interp}/v{w.vertex}"
+    # the practical ceiling of THIS device for a plain streaming kernel with a stage kernel's read/write mix over one
+    # 256^3-sized array set (sc_debug_stream): context for the roofline fractions, which stay against the copy peak
+    ceiling = None
+    if rank == 0:
+        ceiling = {f"R{r}W{wr}": round(H.sc_debug_stream(r, wr, 16 << 20), 1) for r, wr in ((1, 1), (2, 2), (4, 3))}
+        ceiling["unit"], ceiling["what"] = "GB/s", "plain grid-stride double2 kernel, R arrays read + W written, 128 MiB each, best of 5"
 
     def roof(kind):
         k = kinds[kind]
@@ -356,7 +377,7 @@ def run_gpu(args):
             "kernels": kinds, "zone_cycles_per_s": world * w.zone_cycles_per_coarse_step() * args.steps / (ms_total * 1e-3),
             "step_algorithmic_GB": step_bytes / 1e9,
             "step_roofline_frac": step_bytes / (ms_total / args.steps * 1e-3) / 1e9 / peak,
-            "finite": finite}
+            "stream_ceiling": ceiling, "graph": H.sc_debug_graph_stats(), "finite": finite}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -400,6 +421,12 @@ def main():
                     help="cut the finest level into this many abutting slabs that exchange ghosts (NEXT-2 variant)")
     ap.add_argument("--fd-order", type=int, default=4, choices=[4, 8],
                     help="8: the paper's BBH discretisation (PAPER.md:125): 8th-order centred differences, ghost width 4")
+    ap.add_argument("--ko-order", type=int, default=None, choices=[0, 5, 9], help="dissipation order (0: eq 36, r = fd order)")
+    ap.add_argument("--integrator", type=int, default=None, choices=[4, 3, 2], help="RK4 (default) / RK3 / RK2 (reading S28)")
+    ap.add_argument("--outer-bc", type=int, default=None, choices=[0, 1], help="0 periodic (default), 1 radiative (S29)")
+    ap.add_argument("--interp", type=int, default=None, choices=[0, 1], help="1: 9-/10-point interpolation (S30)")
+    ap.add_argument("--vertex", type=int, default=None, choices=[0, 1], help="1: vertex-centred grids (S31)")
+    ap.add_argument("--ghost", type=int, default=None, choices=[2, 3, 4, 5])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--oracle-levels", type=int, default=2,
                     help="levels of the workload the CPU oracle is timed on (bounded sample)")

@@ -189,6 +189,13 @@ int32_t sc_debug_max_abs(sc_hierarchy* h, int32_t level, int32_t box, int32_t co
 int32_t sc_debug_graph_stats(const sc_hierarchy* h, uint64_t* captures, uint64_t* instantiations, uint64_t* updates,
                              uint64_t* cached);
 
+/* Measurement: the practical HBM ceiling of this device for a PLAIN streaming kernel with a stage kernel's read / write
+ * mix — nread arrays read and nwrite arrays written, `ndoubles` doubles each (grid-stride, 16-byte accesses, no
+ * stencil, no shared memory), allocated and freed inside the call. *gbps (HOST) receives the best of 5 timed launches,
+ * (nread + nwrite) * 8 * ndoubles bytes / time. Context for the roofline fractions (which stay against the copy peak):
+ * what a kernel that only moves the same bytes reaches. Synchronises the stream. 1 <= nread, nwrite <= 8. */
+int32_t sc_debug_stream(sc_hierarchy* h, int32_t nread, int32_t nwrite, uint64_t ndoubles, double* gbps);
+
 /* Per-kernel timing for the roofline report. sc_profile(h, 1): from now on sc_step launches its kernels
  * one by one (no graph replay) with a CUDA-event pair around each on the hierarchy's stream;
  * sc_profile(h, 0) stops and discards the records. sc_profile_read sums, over the records since

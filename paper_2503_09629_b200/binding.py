@@ -19,7 +19,7 @@ SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NESTING, SC_ERR_UNSUPPORTED, SC_ERR_OOM, SC_ER
 
 EXPORTS = ["sc_arena_bytes", "sc_create_hierarchy", "sc_set_state", "sc_step", "sc_read_level", "sc_time",
            "sc_launch_count", "sc_debug_ghost_map", "sc_debug_read_padded", "sc_debug_read_slot", "sc_destroy",
-           "sc_last_error", "sc_profile", "sc_profile_read", "sc_debug_max_abs", "sc_debug_graph_stats"]
+           "sc_last_error", "sc_profile", "sc_profile_read", "sc_debug_max_abs", "sc_debug_graph_stats", "sc_debug_stream"]
 
 
 class sc_box(C.Structure):
@@ -79,6 +79,8 @@ def lib():
         L.sc_debug_max_abs.argtypes = [H, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
         L.sc_debug_graph_stats.restype = C.c_int32
         L.sc_debug_graph_stats.argtypes = [H] + [C.POINTER(C.c_uint64)] * 4
+        L.sc_debug_stream.restype = C.c_int32
+        L.sc_debug_stream.argtypes = [H, C.c_int32, C.c_int32, C.c_uint64, C.POINTER(C.c_double)]
         L.sc_destroy.restype = C.c_int32
         L.sc_destroy.argtypes = [H]
         L.sc_profile.restype = C.c_int32
@@ -262,6 +264,12 @@ class Hierarchy:
         v = [C.c_uint64() for _ in range(4)]
         _check(lib().sc_debug_graph_stats(self._h, *[C.byref(x) for x in v]))
         return dict(zip(("captures", "instantiations", "updates", "cached"), (int(x.value) for x in v)))
+
+    def sc_debug_stream(self, nread: int, nwrite: int, ndoubles: int) -> float:
+        """GB/s of a plain streaming kernel with `nread` arrays read and `nwrite` written (include/subcycle.h)."""
+        out = C.c_double(0.0)
+        _check(lib().sc_debug_stream(self._h, nread, nwrite, ndoubles, C.byref(out)))
+        return out.value
 
     KERNEL_KINDS = ("rk_stage", "ghost_dense_prolong", "periodic_fill", "restrict")
 

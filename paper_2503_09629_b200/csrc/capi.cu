@@ -1125,6 +1125,43 @@ int32_t sc_debug_read_slot(sc_hierarchy* h, int32_t level, int32_t box, int32_t 
   return read_array(h, gb, h->arr(gb, a), dst, 0, 0);
 }
 
+int32_t sc_debug_stream(sc_hierarchy* h, int32_t nread, int32_t nwrite, uint64_t ndoubles, double* gbps) {
+  if (!h || !gbps || nread < 1 || nread > 8 || nwrite < 1 || nwrite > 8 || ndoubles < 2 || (ndoubles & 1)) {
+    set_error("sc_debug_stream: bad argument");
+    return SC_ERR_INVALID_ARG;
+  }
+  double *in = nullptr, *out = nullptr;
+  if (cudaMalloc(&in, sizeof(double) * ndoubles * nread) != cudaSuccess ||
+      cudaMalloc(&out, sizeof(double) * ndoubles * nwrite) != cudaSuccess) {
+    cudaGetLastError();
+    if (in) cudaFree(in);
+    set_error("sc_debug_stream: allocation failed");
+    return SC_ERR_OOM;
+  }
+  cudaMemsetAsync(in, 0, sizeof(double) * ndoubles * nread, h->stream);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 7; ++rep) {  // two warm-up launches, five timed
+    cudaEventRecord(e0, h->stream);
+    launch_stream_mix(in, out, ndoubles, nread, nwrite, h->stream);
+    cudaEventRecord(e1, h->stream);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep >= 2 && ms < best) best = ms;
+  }
+  h->launches += 7;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(in);
+  cudaFree(out);
+  SC_CUDA(cudaGetLastError());
+  *gbps = (double)(nread + nwrite) * 8.0 * (double)ndoubles / ((double)best * 1e-3) / 1e9;
+  return SC_OK;
+}
+
 int32_t sc_profile(sc_hierarchy* h, int32_t enable) {
   if (!h) { set_error("null hierarchy"); return SC_ERR_INVALID_ARG; }
   SC_CUDA(cudaStreamSynchronize(h->stream));

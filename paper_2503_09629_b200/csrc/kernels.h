@@ -185,6 +185,9 @@ void launch_sibling_copy(const SiblingPair* pairs_dev, int npairs, long long max
 void launch_pack(const BoxView& b, const double* padded, double* dense, int with_ghosts, cudaStream_t st);
 void launch_unpack(const BoxView& b, const double* dense, double* padded, cudaStream_t st);
 
+// measurement: plain streaming kernel, nread arrays in (n doubles apart) summed into nwrite arrays out
+void launch_stream_mix(const double* in, double* out, unsigned long long n, int nread, int nwrite, cudaStream_t st);
+
 // debug: max |x| over the interior (NaN if any value is NaN); *out_bits (device) must be zeroed by the caller and
 // receives the bit pattern of the result (non-negative doubles order like their bit patterns)
 void launch_max_abs(const BoxView& b, const double* padded, unsigned long long* out_bits, cudaStream_t st);

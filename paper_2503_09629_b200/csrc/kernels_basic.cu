@@ -266,6 +266,27 @@ void launch_max_abs(const BoxView& b, const double* padded, unsigned long long* 
 }
 
 // ------------------------------------------------------------------------------------------------
+// measurement (sc_debug_stream): what a kernel that ONLY moves a stage kernel's bytes reaches on this device
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) stream_mix(const double2* __restrict__ in, double2* __restrict__ out,
+                                                  unsigned long long n2, int nread, int nwrite) {
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n2;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    double2 s = make_double2(0.0, 0.0);
+    for (int r = 0; r < nread; ++r) {
+      const double2 v = in[r * n2 + i];
+      s.x += v.x;
+      s.y += v.y;
+    }
+    for (int w = 0; w < nwrite; ++w) out[w * n2 + i] = make_double2(s.x + w, s.y - w);
+  }
+}
+void launch_stream_mix(const double* in, double* out, unsigned long long n, int nread, int nwrite, cudaStream_t st) {
+  stream_mix<<<148 * 32, 256, 0, st>>>(reinterpret_cast<const double2*>(in), reinterpret_cast<double2*>(out), n / 2, nread,
+                                       nwrite);
+}
+
+// ------------------------------------------------------------------------------------------------
 // a5  restriction, one thread per parent cell, nr^3-point gather (216 for S4; 1 for injection on vertex-centred grids)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) restrict_ref(const __grid_constant__ RestrictArgs a) {
