@@ -351,6 +351,7 @@ def run_gpu(args):
     e2e = {"value": whole_job_value(world, upd_step, e2e_steps, e2e_s), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
            "d2h_bytes_per_step": state_bytes, "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps}
     finite = all(bool(torch.isfinite(t).all()) for t in host_out.values())
+    graph_stats = H.sc_debug_graph_stats()
     H.close()
 
     if rank != 0:
@@ -377,7 +378,7 @@ def run_gpu(args):
             "kernels": kinds, "zone_cycles_per_s": world * w.zone_cycles_per_coarse_step() * args.steps / (ms_total * 1e-3),
             "step_algorithmic_GB": step_bytes / 1e9,
             "step_roofline_frac": step_bytes / (ms_total / args.steps * 1e-3) / 1e9 / peak,
-            "stream_ceiling": ceiling, "graph": H.sc_debug_graph_stats(), "finite": finite}
+            "stream_ceiling": ceiling, "graph": graph_stats, "finite": finite}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

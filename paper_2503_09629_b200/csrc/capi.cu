@@ -911,7 +911,6 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     const BoxInfo& b = h->L.boxes[ib];
     h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
-    if (h->L.vertex) h->tmap_ok[ib] = 0;  // vertex-centred grids run the direct-load kernels (restriction = injection)
     h->kmap_ok[ib] = h->L.ko_sigma > 0.0 && h->L.integrator == 4 && h->L.fd_order == 4 && h->L.ko_order == 5 && h->L.outer_bc == 0 &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 5, h->kmaps[ib].bytes);
     h->gmap_ok[ib] = 1;

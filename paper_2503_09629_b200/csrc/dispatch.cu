@@ -16,10 +16,12 @@ void stage_box_dims(unsigned box[4]);
 void restrict_box_dims(unsigned box[4]);
 void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
 void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st);
+void launch_ghost_fill_tiled(const GhostArgs& a, cudaStream_t st);
 bool ghost_tma_takes(const GhostArgs& a);
 void ghost_box_dims(int axis, unsigned box[4]);
 void launch_restrict_ref(const RestrictArgs& a, cudaStream_t st);
 void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st);
+void launch_restrict_tiled(const RestrictArgs& a, cudaStream_t st);
 void launch_stage_ko_direct(const StageKOArgs& a, cudaStream_t st);
 void launch_stage_ko_tma(const StageKOArgs& a, cudaStream_t st);
 bool stage_ko_tma_takes(const StageKOArgs& a);
@@ -42,11 +44,14 @@ void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {
 }
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st) {
   const bool s3 = a.np == 5 && a.pmin == -2;  // the tuned kernel has the quartic cell-centred operator built in
-  if (g_mode == 0 || !s3 || !ghost_tma_takes(a)) launch_ghost_fill_direct(a, st);
+  if (g_mode == 0) launch_ghost_fill_direct(a, st);                          // SC_KERNELS=ref: the np^3-point gather
+  else if (!s3 || !ghost_tma_takes(a)) launch_ghost_fill_tiled(a, st);       // any width / stencil / shape, separable
   else launch_ghost_fill_tma(a, st);
 }
 void launch_restrict(const RestrictArgs& a, cudaStream_t st) {
-  if (g_mode == 0 || a.nr != 6 || !a.tmap) launch_restrict_ref(a, st);
+  if (g_mode == 0) launch_restrict_ref(a, st);
+  else if (a.nr == 1) launch_restrict_ref(a, st);  // injection: one load per parent cell
+  else if (a.nr != 6 || !a.tmap) launch_restrict_tiled(a, st);
   else launch_restrict_opt(a, st);
 }
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128) {
