@@ -911,7 +911,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     const BoxInfo& b = h->L.boxes[ib];
     h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
-    h->kmap_ok[ib] = h->L.ko_sigma > 0.0 && h->L.integrator == 4 && h->L.fd_order == 4 && h->L.ko_order == 5 && h->L.outer_bc == 0 &&
+    h->kmap_ok[ib] = h->L.general() && h->L.fd_order == 4 && (h->L.ko_sigma == 0.0 || h->L.ko_order == 5) && h->L.g >= 3 &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 5, h->kmaps[ib].bytes);
     h->gmap_ok[ib] = 1;
     for (int ax = 0; ax < 3; ++ax)

@@ -37,10 +37,13 @@ int launch_stage(const StageArgs& a, cudaStream_t st) {
   return launch_stage_tma(a, st);
 }
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {
-  // the tuned kernel is the RK4 / 4th-order / delta^6 / periodic case; everything else runs on stage_gen
-  const bool tuned_case = a.integrator == 4 && a.fd_order == 4 && a.ko_order == 5 && a.rad_nb == 0;
-  if (g_mode == 0 || !tuned_case || !stage_ko_tma_takes(a)) launch_stage_ko_direct(a, st);
-  else launch_stage_ko_tma(a, st);
+  if (g_mode == 0 || !stage_ko_tma_takes(a)) { launch_stage_ko_direct(a, st); return; }
+  launch_stage_ko_tma(a, st);
+  if (a.rad_nb > 0) {  // radiative level 0 (S29): the boundary points again, with the radiative operator
+    StageKOArgs z = a;
+    z.zone_only = 1;
+    launch_stage_ko_direct(z, st);
+  }
 }
 void launch_ghost_fill(const GhostArgs& a, cudaStream_t st) {
   const bool s3 = a.np == 5 && a.pmin == -2;  // the tuned kernel has the quartic cell-centred operator built in

@@ -94,6 +94,7 @@ struct StageKOArgs {
   int a_Yu, a_Yr;        // array indices of Yu, Yr (field 0) in the tensor map
   // radiative outer boundary (S29), level 0 only: cells within `rad_nb` of a face are boundary points
   int rad_nb;            // 0: none
+  int zone_only;         // 1: redo the boundary points only (after the tuned kernel took the whole box)
   double x0[3], dx[3];   // position of cell 0 (centre or grid point) and spacing
 };
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st);

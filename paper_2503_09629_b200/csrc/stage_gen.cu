@@ -72,7 +72,9 @@ __global__ void __launch_bounds__(256) stage_gen(const __grid_constant__ StageKO
   const double* R = a.Yr + o;
   double ku, kr;
   const int nb = a.rad_nb;
-  if (nb > 0 && (i < nb || i >= b.n[0] - nb || j < nb || j >= b.n[1] - nb || k < nb || k >= b.n[2] - nb)) {
+  const bool zone = nb > 0 && (i < nb || i >= b.n[0] - nb || j < nb || j >= b.n[1] - nb || k < nb || k >= b.n[2] - nb);
+  if (a.zone_only && !zone) return;
+  if (zone) {
     const int idx[3] = {i, j, k};
     const long long st[3] = {1, sy, sz};
     const double x[3] = {a.x0[0] + i * a.dx[0], a.x0[1] + j * a.dx[1], a.x0[2] + k * a.dx[2]};

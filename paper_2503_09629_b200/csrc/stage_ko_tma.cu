@@ -46,11 +46,15 @@ struct KoParams {
   int a_Yu, a_Yr;        // array indices (field 0) of the stage vector's u- and rho-part in the tensor map
   const double* yn_u;    // centre-only operands and outputs: field-0 arrays
   const double* yn_r;
+  // combine stage (FINAL): out = y_n + c2 (A2 - y_n) + c3 (A3 - y_n) + c4 (A4 - y_n) + adt k, centre-only operands A2..A4
+  // (null with a zero coefficient); RK4 stage 4: (Y_2, Y_3, Y_4; 1/3, 2/3, 1/3; dt/6); RK3 stage 2: (-, -, Y_2; -2; 2 dt);
+  // RK3 stage 3: (Y_2, -, Y_3; 1, 1/3; dt/6); RK2 stage 2: (dt); RK3's extra slope: no out, k only
   const double* U2; const double* U3; const double* R2; const double* R3;
-  const double* Y4u; const double* Y4r;   // stage 4: the centre of Y_4 again (global, L2-resident)
-  double* outU; double* outR;
-  double* K4u; double* K4r;
-  double adt;            // a_s dt (stages 1..3) or dt/6 (stage 4)
+  const double* Y4u; const double* Y4r;   // the centre of the stage's own input again (global, L2-resident)
+  double c2, c3, c4;
+  double* outU; double* outR;             // null: the slope only
+  double* K4u; double* K4r;               // where the slope k is kept, or null
+  double adt;            // a_s dt (simple stages) or the weight of k in the combine
   double w[3];           // 1 / (12 dx_a^2)
   double ko[3];          // sigma / (64 dx_a)
 };
@@ -118,8 +122,10 @@ __device__ __forceinline__ void scatter7(double2 (&acc)[7], double2 ct, double2 
 
 // (stage 4 keeps 8 more centre operands in flight per cell pair: one CTA per SM with the full register file;
 // the 4-deep TMA ring and the one-plane-ahead global loads still cover the memory latency)
-template <bool FINAL>
-__global__ void __launch_bounds__(NTHR, FINAL ? 1 : 2)
+// FINAL: 0 = simple stage (out = y_n + adt k), 1 = full combine (up to three more centre operands; one CTA per SM),
+// 2 = light combine (the stage's own input as the only extra operand: RK3 stage 2, RK2 stage 2, RK3's extra slope)
+template <int FINAL>
+__global__ void __launch_bounds__(NTHR, FINAL == 1 ? 1 : 2)
     stage_ko_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ KoParams p) {
   extern __shared__ unsigned char smraw[];
   // [NSTK][2] tiles (U, R), 128-byte aligned for TMA, then NSTK mbarriers
@@ -180,13 +186,23 @@ __global__ void __launch_bounds__(NTHR, FINAL ? 1 : 2)
       const long long o = cell0 + (long long)(z - 2 * dir) * b.plane;
       n_un = __ldg(reinterpret_cast<const double2*>(p.yn_u + o));
       n_rn = __ldg(reinterpret_cast<const double2*>(p.yn_r + o));
-      if (FINAL) {
-        n_u2 = __ldg(reinterpret_cast<const double2*>(p.U2 + o));
-        n_u3 = __ldg(reinterpret_cast<const double2*>(p.U3 + o));
-        n_r2 = __ldg(reinterpret_cast<const double2*>(p.R2 + o));
-        n_r3 = __ldg(reinterpret_cast<const double2*>(p.R3 + o));
+      if (FINAL == 2 && p.c4 != 0.0) {
         n_u4 = __ldg(reinterpret_cast<const double2*>(p.Y4u + o));
         n_r4 = __ldg(reinterpret_cast<const double2*>(p.Y4r + o));
+      }
+      if (FINAL == 1) {
+        if (p.c2 != 0.0) {
+          n_u2 = __ldg(reinterpret_cast<const double2*>(p.U2 + o));
+          n_r2 = __ldg(reinterpret_cast<const double2*>(p.R2 + o));
+        }
+        if (p.c3 != 0.0) {
+          n_u3 = __ldg(reinterpret_cast<const double2*>(p.U3 + o));
+          n_r3 = __ldg(reinterpret_cast<const double2*>(p.R3 + o));
+        }
+        if (p.c4 != 0.0) {
+          n_u4 = __ldg(reinterpret_cast<const double2*>(p.Y4u + o));
+          n_r4 = __ldg(reinterpret_cast<const double2*>(p.Y4r + o));
+        }
       }
     }
     mbar_wait_k(bar0 + 8 * st, (it / NSTK) & 1);
@@ -215,14 +231,28 @@ __global__ void __launch_bounds__(NTHR, FINAL ? 1 : 2)
       if (!FINAL) {
         *reinterpret_cast<double2*>(p.outU + o) = fma2k(p.adt, ku, un);
         *reinterpret_cast<double2*>(p.outR + o) = fma2k(p.adt, kr, rn);
+      } else if (FINAL == 2) {
+        if (p.outU) {
+          const double c4 = p.c4;
+          *reinterpret_cast<double2*>(p.outU + o) = make_double2(un.x + c4 * (u4.x - un.x) + p.adt * ku.x,
+                                                                 un.y + c4 * (u4.y - un.y) + p.adt * ku.y);
+          *reinterpret_cast<double2*>(p.outR + o) = make_double2(rn.x + c4 * (r4.x - rn.x) + p.adt * kr.x,
+                                                                 rn.y + c4 * (r4.y - rn.y) + p.adt * kr.y);
+        }
+        if (p.K4u) {
+          *reinterpret_cast<double2*>(p.K4u + o) = ku;
+          *reinterpret_cast<double2*>(p.K4r + o) = kr;
+        }
       } else {
-        const double third = 1.0 / 3.0;
-        *reinterpret_cast<double2*>(p.outU + o) = make_double2(
-            un.x + (third * ((u2.x - un.x) + (u4.x - un.x)) + (2.0 * third) * (u3.x - un.x)) + p.adt * ku.x,
-            un.y + (third * ((u2.y - un.y) + (u4.y - un.y)) + (2.0 * third) * (u3.y - un.y)) + p.adt * ku.y);
-        *reinterpret_cast<double2*>(p.outR + o) = make_double2(
-            rn.x + (third * ((r2.x - rn.x) + (r4.x - rn.x)) + (2.0 * third) * (r3.x - rn.x)) + p.adt * kr.x,
-            rn.y + (third * ((r2.y - rn.y) + (r4.y - rn.y)) + (2.0 * third) * (r3.y - rn.y)) + p.adt * kr.y);
+        if (p.outU) {
+          const double c2 = p.c2, c3 = p.c3, c4 = p.c4;
+          *reinterpret_cast<double2*>(p.outU + o) = make_double2(
+              un.x + ((c2 * (u2.x - un.x) + c4 * (u4.x - un.x)) + c3 * (u3.x - un.x)) + p.adt * ku.x,
+              un.y + ((c2 * (u2.y - un.y) + c4 * (u4.y - un.y)) + c3 * (u3.y - un.y)) + p.adt * ku.y);
+          *reinterpret_cast<double2*>(p.outR + o) = make_double2(
+              rn.x + ((c2 * (r2.x - rn.x) + c4 * (r4.x - rn.x)) + c3 * (r3.x - rn.x)) + p.adt * kr.x,
+              rn.y + ((c2 * (r2.y - rn.y) + c4 * (r4.y - rn.y)) + c3 * (r3.y - rn.y)) + p.adt * kr.y);
+        }
         if (p.K4u) {
           *reinterpret_cast<double2*>(p.K4u + o) = ku;
           *reinterpret_cast<double2*>(p.K4r + o) = kr;
@@ -247,7 +277,7 @@ __global__ void __launch_bounds__(NTHR, FINAL ? 1 : 2)
 // ---- host ------------------------------------------------------------------------------------------
 void stageko_box_dims(unsigned box[4]) { box[0] = HXK; box[1] = HYK; box[2] = 1; box[3] = 1; }
 
-template <bool FINAL>
+template <int FINAL>
 static void launch_ko_zmarch(const StageKOArgs& a, const KoParams& p0, cudaStream_t st) {
   constexpr size_t smem = (size_t)NSTK * 2 * TILEK * 8 + NSTK * 8 + 128;
   static bool configured = false;
@@ -256,15 +286,19 @@ static void launch_ko_zmarch(const StageKOArgs& a, const KoParams& p0, cudaStrea
     configured = true;
   }
   KoParams p = p0;
-  p.nchunks = stage_pick_chunks(a.b, a.F, FINAL ? 1 : 2, 6);
+  p.nchunks = stage_pick_chunks(a.b, a.F, FINAL == 1 ? 1 : 2, 6);
   p.chunk = (a.b.n[2] + p.nchunks - 1) / p.nchunks;
   p.nchunks = (a.b.n[2] + p.chunk - 1) / p.chunk;
   dim3 grd((a.b.n[0] + TX - 1) / TX, (a.b.n[1] + TY - 1) / TY, p.nchunks * a.F);
   stage_ko_zmarch<FINAL><<<grd, NTHR, smem, st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
 }
 
-// the tuned kernel takes uncoupled systems whose box has a tensor map; everything else goes to stage_ko
-bool stage_ko_tma_takes(const StageKOArgs& a) { return a.tmap && !a.A; }
+// the tuned kernel takes uncoupled systems whose box has a tensor map, 4th-order differences, no or fifth-order
+// dissipation, any integrator; on a radiative level 0 the boundary points are redone by the direct kernel afterwards
+// (dispatch.cu). Everything else goes to stage_gen.
+bool stage_ko_tma_takes(const StageKOArgs& a) {
+  return a.tmap && !a.A && a.fd_order == 4 && (a.ko_order == 0 || a.ko_order == 5) && a.b.g >= 3;
+}
 
 void launch_stage_ko_tma(const StageKOArgs& a, cudaStream_t st) {
   KoParams p{};
@@ -276,10 +310,27 @@ void launch_stage_ko_tma(const StageKOArgs& a, cudaStream_t st) {
   p.Y4u = a.Yu; p.Y4r = a.Yr;
   p.outU = a.outU; p.outR = a.outR;
   p.K4u = a.K4u; p.K4r = a.K4r;
-  p.adt = a.stage == 4 ? a.dt / 6.0 : (a.stage == 3 ? a.dt : 0.5 * a.dt);
-  for (int d = 0; d < 3; ++d) { p.w[d] = a.inv12dx2[d]; p.ko[d] = a.ko[d]; }
-  if (a.stage == 4) launch_ko_zmarch<true>(a, p, st);
-  else launch_ko_zmarch<false>(a, p, st);
+  for (int d = 0; d < 3; ++d) { p.w[d] = a.inv12dx2[d]; p.ko[d] = a.ko_order ? a.ko[d] : 0.0; }
+  const int S = a.integrator, s = a.stage;
+  bool combine = false;
+  if (s > S) {                       // RK3: k_4 = M y_{n+1} only
+    combine = true;
+    p.outU = p.outR = nullptr;
+  } else if (S == 4 && s == 4) {
+    combine = true; p.c2 = 1.0 / 3.0; p.c3 = 2.0 / 3.0; p.c4 = 1.0 / 3.0; p.adt = a.dt / 6.0;
+  } else if (S == 3 && s == 2) {     // Y_3 = y_n - 2 (Y_2 - y_n) + 2 dt k_2
+    combine = true; p.c4 = -2.0; p.adt = 2.0 * a.dt;
+  } else if (S == 3 && s == 3) {     // y_{n+1} = y_n + (Y_2 - y_n) + (Y_3 - y_n)/3 + dt/6 k_3;  k_3 kept where a child reads it
+    combine = true; p.c2 = 1.0; p.c4 = 1.0 / 3.0; p.adt = a.dt / 6.0;
+    p.K4u = a.K3u; p.K4r = a.K3r;
+  } else if (S == 2 && s == 2) {
+    combine = true; p.adt = a.dt;
+  } else {
+    p.adt = (S == 4 && s == 3 ? 1.0 : 0.5) * a.dt;
+  }
+  if (!combine) launch_ko_zmarch<0>(a, p, st);
+  else if (p.c2 == 0.0 && p.c3 == 0.0) launch_ko_zmarch<2>(a, p, st);
+  else launch_ko_zmarch<1>(a, p, st);
 }
 
 }  // namespace sc
