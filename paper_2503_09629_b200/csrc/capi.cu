@@ -911,8 +911,14 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     const BoxInfo& b = h->L.boxes[ib];
     h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
-    h->kmap_ok[ib] = h->L.general() && h->L.fd_order == 4 && (h->L.ko_sigma == 0.0 || h->L.ko_order == 5) && h->L.g >= 3 &&
-                     make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 5, h->kmaps[ib].bytes);
+    {  // the general path's stage tile: halo 3 (4th-order differences), 4 (8th order) or 5 (with delta^10)
+      const Layout& L = h->L;
+      const bool ko9 = L.ko_sigma > 0.0 && L.ko_order == 9;
+      const int kind = L.fd_order == 8 ? (ko9 ? 7 : 6) : 5;
+      const int need = kind == 7 ? 5 : (kind == 6 ? 4 : 3);
+      h->kmap_ok[ib] = L.general() && (kind != 5 || !ko9) && L.g >= need &&
+                       make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), kind, h->kmaps[ib].bytes);
+    }
     h->gmap_ok[ib] = 1;
     for (int ax = 0; ax < 3; ++ax)
       if (!make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 2 + ax, h->gmaps[ib].m[ax].bytes)) h->gmap_ok[ib] = 0;

@@ -26,6 +26,9 @@ void launch_stage_ko_direct(const StageKOArgs& a, cudaStream_t st);
 void launch_stage_ko_tma(const StageKOArgs& a, cudaStream_t st);
 bool stage_ko_tma_takes(const StageKOArgs& a);
 void stageko_box_dims(unsigned box[4]);
+void launch_stage_gen_tma(const StageKOArgs& a, cudaStream_t st);
+bool stage_gen_tma_takes(const StageKOArgs& a);
+void stagegen_box_dims(int H, unsigned box[4]);
 
 static int g_mode = 1;
 void select_kernels(int mode) { g_mode = mode; }
@@ -37,8 +40,9 @@ int launch_stage(const StageArgs& a, cudaStream_t st) {
   return launch_stage_tma(a, st);
 }
 void launch_stage_ko(const StageKOArgs& a, cudaStream_t st) {
-  if (g_mode == 0 || !stage_ko_tma_takes(a)) { launch_stage_ko_direct(a, st); return; }
-  launch_stage_ko_tma(a, st);
+  if (g_mode != 0 && stage_gen_tma_takes(a)) launch_stage_gen_tma(a, st);      // 8th-order differences
+  else if (g_mode != 0 && stage_ko_tma_takes(a)) launch_stage_ko_tma(a, st);   // 4th-order
+  else { launch_stage_ko_direct(a, st); return; }
   if (a.rad_nb > 0) {  // radiative level 0 (S29): the boundary points again, with the radiative operator
     StageKOArgs z = a;
     z.zone_only = 1;
@@ -62,11 +66,12 @@ bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, vo
   if (kind == 0) stage_box_dims(box);
   else if (kind == 1) restrict_box_dims(box);
   else if (kind <= 4) ghost_box_dims(kind - 2, box);
-  else stageko_box_dims(box);
+  else if (kind == 5) stageko_box_dims(box);
+  else stagegen_box_dims(kind == 7 ? 5 : 4, box);  // kinds 6, 7: the general path's halo-4 / halo-5 tiles
   // streaming tiles (stage, restriction) promote misses to 256-byte fetches; the ghost fill's footprint rows are
   // 64-160 bytes and isolated: promotion there only multiplies the DRAM traffic. The x-slab footprint (kind 2,
   // 64-byte rows) is swizzled so that one-thread-per-row reads are bank-conflict free (ghost_tma.cu).
-  return make_box_tensor_map_tma(b, narrays, base, box, (kind <= 1 || kind == 5) ? 256 : 0, kind == 2, out_map128);
+  return make_box_tensor_map_tma(b, narrays, base, box, (kind <= 1 || kind >= 5) ? 256 : 0, kind == 2, out_map128);
 }
 
 }  // namespace sc
