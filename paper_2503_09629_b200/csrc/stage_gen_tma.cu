@@ -7,11 +7,12 @@
 // Same data movement as stage_ko_tma.cu — a CTA owns a 32 x 16 column and marches a z-chunk, every plane of the two
 // halo-read arrays arrives as one TMA tiled load each into an mbarrier ring, the z-stencils live in registers in scatter
 // form (an arriving plane adds its in-plane part to its own output plane and its centre value, times the z weights, to
-// the 2H neighbouring output planes, H = max(RL, RQ); output plane p - H is complete when plane p has arrived) — but
-// ONE cell per thread and 512 threads per CTA: with radius 4-5 the two-cells-per-thread form needs 2 x (2H + 1) double2
-// accumulators plus 2 x (3H + 1) double2 neighbour values per thread and does not fit; one cell per thread keeps the
-// accumulators at 2 (2H + 1) doubles, and a warp is one 256-byte row of the tile (conflict-free shared loads, coalesced
-// stores). One CTA per SM, a 6-deep ring.
+// the 2H neighbouring output planes, H = max(RL, RQ); output plane p - H is complete when plane p has arrived). Tile
+// 64 x 8 cells, 256 threads, two x-adjacent cells per thread (every shared load is 16 bytes), one CTA per SM with the
+// whole register file (2 (2H + 1) double2 accumulators per thread), a 6-deep ring. Measured on the way (256^3, fd 8 +
+// delta^6 / delta^10): one cell per thread, 512 threads: 252 / 323 us, ncu: `mio_throttle` 2.7 stall cycles per issue
+// (30 8-byte shared loads per thread and plane); this form: 254 / 277 us; the direct-load stage_gen: 368 / 421 us. A
+// barrier-free ring hand-off (274 us) and a deeper ring (254 us) did not help.
 #include <cuda.h>
 
 #include <type_traits>
@@ -25,7 +26,7 @@ int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes)
 
 namespace {
 
-constexpr int GTX = 32, GTY = 16, GNTHR = GTX * GTY;
+constexpr int GTX = 64, GTY = 8, GNTHR = (GTX / 2) * GTY;  // two x-adjacent cells per thread: every shared load is 16 bytes
 constexpr int GNST = 6;  // planes in flight
 
 template <int H> struct TileGeo {
@@ -92,7 +93,7 @@ __global__ void __launch_bounds__(GNTHR, 1)
   const uint32_t bar0 = s0 + GNST * 2 * G::STRIDE;
 
   const BoxView& b = p.b;
-  const int tid = threadIdx.x, tx = tid % GTX, ty = tid / GTX;
+  const int tid = threadIdx.x, tx = tid % (GTX / 2), ty = tid / (GTX / 2);
   const int X0 = blockIdx.x * GTX, Y0 = blockIdx.y * GTY;
   const int f = blockIdx.z / p.nchunks, c = blockIdx.z % p.nchunks;
   const int zc0 = c * p.chunk, zc1 = min(b.n[2], zc0 + p.chunk);
@@ -123,87 +124,112 @@ __global__ void __launch_bounds__(GNTHR, 1)
   }
   __syncthreads();
 
-  const bool active = (X0 + tx < b.n[0]) && (Y0 + ty < b.n[1]);
-  const long long cell0 = (long long)f * b.vol + cell_offset(b, X0 + tx, Y0 + ty, 0);
+  const bool active = (X0 + 2 * tx < b.n[0]) && (Y0 + ty < b.n[1]);
+  const long long cell0 = (long long)f * b.vol + cell_offset(b, X0 + 2 * tx, Y0 + ty, 0);
   const double wx = p.w[0], wy = p.w[1], wz = p.w[2], kx = p.ko[0], ky = p.ko[1], kz = p.ko[2];
-  double accU[NS], accR[NS];
+  double2 accU[NS], accR[NS];
 #pragma unroll
-  for (int q = 0; q < NS; ++q) accU[q] = accR[q] = 0.0;
-  double n_un = 0.0, n_rn = 0.0, n_u2 = 0.0, n_r2 = 0.0, n_u3 = 0.0, n_r3 = 0.0, n_u4 = 0.0, n_r4 = 0.0;
+  for (int q = 0; q < NS; ++q) accU[q] = accR[q] = make_double2(0.0, 0.0);
+  const double2 zero2 = make_double2(0.0, 0.0);
+  double2 n_un = zero2, n_rn = zero2, n_u2 = zero2, n_r2 = zero2, n_u3 = zero2, n_r3 = zero2, n_u4 = zero2, n_r4 = zero2;
+  auto ld2 = [](const double* q) { return __ldg(reinterpret_cast<const double2*>(q)); };
 
   auto step = [&](auto Rc, int it) {
     constexpr int R = decltype(Rc)::value;
     const int st = it % GNST;
     const bool inpl = it >= H && it < narr - H;
     const int z = zs + dir * it;
-    const double un = n_un, rn = n_rn, u2 = n_u2, r2 = n_r2, u3 = n_u3, r3 = n_r3, u4 = n_u4, r4 = n_r4;
+    const double2 un = n_un, rn = n_rn, u2 = n_u2, r2 = n_r2, u3 = n_u3, r3 = n_r3, u4 = n_u4, r4 = n_r4;
     if (active && it + 1 >= 2 * H && it + 1 < narr) {  // the next iteration completes plane z + dir - H dir
       const long long o = cell0 + (long long)(z - (H - 1) * dir) * b.plane;
-      n_un = __ldg(p.yn_u + o);
-      n_rn = __ldg(p.yn_r + o);
+      n_un = ld2(p.yn_u + o);
+      n_rn = ld2(p.yn_r + o);
       if (COMBINE) {
-        if (p.c2 != 0.0) { n_u2 = __ldg(p.A2u + o); n_r2 = __ldg(p.A2r + o); }
-        if (p.c3 != 0.0) { n_u3 = __ldg(p.A3u + o); n_r3 = __ldg(p.A3r + o); }
-        if (p.c4 != 0.0) { n_u4 = __ldg(p.A4u + o); n_r4 = __ldg(p.A4r + o); }
+        if (p.c2 != 0.0) { n_u2 = ld2(p.A2u + o); n_r2 = ld2(p.A2r + o); }
+        if (p.c3 != 0.0) { n_u3 = ld2(p.A3u + o); n_r3 = ld2(p.A3r + o); }
+        if (p.c4 != 0.0) { n_u4 = ld2(p.A4u + o); n_r4 = ld2(p.A4r + o); }
       }
     }
     mbar_wait_s(bar0 + 8 * st, (it / GNST) & 1);
-    const double* __restrict__ tU = reinterpret_cast<const double*>(tiles + (st * 2) * G::STRIDE) + (ty + H) * G::HX + tx + G::HXE;
-    const double* __restrict__ tR = reinterpret_cast<const double*>(tiles + (st * 2 + 1) * G::STRIDE) + (ty + H) * G::HX + tx + G::HXE;
-    const double uc = tU[0], rc = tR[0];
-    double ctU = 0.0, ctR = 0.0;
+    // the thread's two cells (x, x + 1) sit at double2 index 0 of cU / cR; row neighbours at double2 offsets, rows HX apart
+    const double* __restrict__ tU = reinterpret_cast<const double*>(tiles + (st * 2) * G::STRIDE) + (ty + H) * G::HX + 2 * tx + G::HXE;
+    const double* __restrict__ tR = reinterpret_cast<const double*>(tiles + (st * 2 + 1) * G::STRIDE) + (ty + H) * G::HX + 2 * tx + G::HXE;
+    auto at2 = [](const double* q, int off) { return *reinterpret_cast<const double2*>(q + off); };
+    const double2 uc = at2(tU, 0), rc = at2(tR, 0);
+    double2 ctU = zero2, ctR = zero2;
     if (inpl) {
-      // in-plane parts: x and y neighbours at distance m, centre with all three axes' weights
-      double lx = 0.0, ly = 0.0, qux = 0.0, quy = 0.0, qrx = 0.0, qry = 0.0;
+      // row values x-4 .. x+5 (x-6 .. x+7 for H = 5) as double2: flat index q <-> x - HR + q, HR = even radius
+      constexpr int HR = (H + 1) & ~1, NV = HR + 1;
+      double2 vu[NV], vr[NV];
+#pragma unroll
+      for (int q = 0; q < NV; ++q) { vu[q] = at2(tU, 2 * q - HR); if (RQ > 0) vr[q] = at2(tR, 2 * q - HR); }
+      auto flat = [&](const double2 (&v)[NV], int q) { return (q & 1) ? v[q >> 1].y : v[q >> 1].x; };
+      double2 lx = zero2, ly = zero2, qux = zero2, quy = zero2, qrx = zero2, qry = zero2;
 #pragma unroll
       for (int m = 1; m <= H; ++m) {
-        const double ux = tU[-m] + tU[m], uy = tU[-m * G::HX] + tU[m * G::HX];
-        if (m <= RL) { lx = fma(lapw<RL>(m), ux, lx); ly = fma(lapw<RL>(m), uy, ly); }
+        // cell 0 sits at flat HR, cell 1 at flat HR + 1
+        const double2 ux = make_double2(flat(vu, HR - m) + flat(vu, HR + m), flat(vu, HR + 1 - m) + flat(vu, HR + 1 + m));
+        const double2 um = at2(tU, -m * G::HX), up = at2(tU, m * G::HX);
+        const double2 uy = make_double2(um.x + up.x, um.y + up.y);
+        if (m <= RL) {
+          lx.x = fma(lapw<RL>(m), ux.x, lx.x); lx.y = fma(lapw<RL>(m), ux.y, lx.y);
+          ly.x = fma(lapw<RL>(m), uy.x, ly.x); ly.y = fma(lapw<RL>(m), uy.y, ly.y);
+        }
         if (RQ > 0 && m <= RQ) {
-          const double rx = tR[-m] + tR[m], ry = tR[-m * G::HX] + tR[m * G::HX];
-          qux = fma(disw<RQ>(m), ux, qux); quy = fma(disw<RQ>(m), uy, quy);
-          qrx = fma(disw<RQ>(m), rx, qrx); qry = fma(disw<RQ>(m), ry, qry);
+          const double2 rx = make_double2(flat(vr, HR - m) + flat(vr, HR + m), flat(vr, HR + 1 - m) + flat(vr, HR + 1 + m));
+          const double2 rm = at2(tR, -m * G::HX), rp = at2(tR, m * G::HX);
+          const double2 ry = make_double2(rm.x + rp.x, rm.y + rp.y);
+          qux.x = fma(disw<RQ>(m), ux.x, qux.x); qux.y = fma(disw<RQ>(m), ux.y, qux.y);
+          quy.x = fma(disw<RQ>(m), uy.x, quy.x); quy.y = fma(disw<RQ>(m), uy.y, quy.y);
+          qrx.x = fma(disw<RQ>(m), rx.x, qrx.x); qrx.y = fma(disw<RQ>(m), rx.y, qrx.y);
+          qry.x = fma(disw<RQ>(m), ry.x, qry.x); qry.y = fma(disw<RQ>(m), ry.y, qry.y);
         }
       }
       const double lapc = lapw<RL>(0) * (wx + wy + wz);
-      double lU = fma(wx, lx, fma(wy, ly, lapc * uc));
-      double qU = 0.0, qR = 0.0;
+      const double2 lU = make_double2(fma(wx, lx.x, fma(wy, ly.x, lapc * uc.x)), fma(wx, lx.y, fma(wy, ly.y, lapc * uc.y)));
+      double2 qU = zero2, qR = zero2;
       if (RQ > 0) {
         const double qc = disw<RQ>(0) * (kx + ky + kz);
-        qU = fma(kx, qux, fma(ky, quy, qc * uc));
-        qR = fma(kx, qrx, fma(ky, qry, qc * rc));
+        qU = make_double2(fma(kx, qux.x, fma(ky, quy.x, qc * uc.x)), fma(kx, qux.y, fma(ky, quy.y, qc * uc.y)));
+        qR = make_double2(fma(kx, qrx.x, fma(ky, qry.x, qc * rc.x)), fma(kx, qrx.y, fma(ky, qry.y, qc * rc.y)));
       }
-      ctU = rc + qU;
-      ctR = lU + qR;
+      ctU = make_double2(rc.x + qU.x, rc.y + qU.y);
+      ctR = make_double2(lU.x + qR.x, lU.y + qR.y);
     }
     // scatter: slot (R + d) mod NS belongs to output plane (arrival + d); the slot of arrival + H is created here
 #pragma unroll
     for (int d = -H; d <= H; ++d) {
-      constexpr int dummy = 0; (void)dummy;
       const int m = d < 0 ? -d : d;
       const int slot = ((R + d) % NS + NS) % NS;
-      double zu = 0.0, zr = 0.0;
+      double2 zu = zero2, zr = zero2;
       if (d == 0) { zu = ctU; zr = ctR; }
       else {
-        if (RQ > 0 && m <= RQ) { zu = (kz * disw<RQ>(m)) * uc; zr = (kz * disw<RQ>(m)) * rc; }
-        if (m <= RL) zr = fma(wz * lapw<RL>(m), uc, zr);
+        if (RQ > 0 && m <= RQ) {
+          const double cq = kz * disw<RQ>(m);
+          zu = make_double2(cq * uc.x, cq * uc.y);
+          zr = make_double2(cq * rc.x, cq * rc.y);
+        }
+        if (m <= RL) { const double cl = wz * lapw<RL>(m); zr.x = fma(cl, uc.x, zr.x); zr.y = fma(cl, uc.y, zr.y); }
       }
       if (d == H) { accU[slot] = zu; accR[slot] = zr; }
-      else { accU[slot] += zu; accR[slot] += zr; }
+      else { accU[slot].x += zu.x; accU[slot].y += zu.y; accR[slot].x += zr.x; accR[slot].y += zr.y; }
     }
     if (it >= 2 * H && active) {  // output plane z - H dir is complete
       const long long o = cell0 + (long long)(z - H * dir) * b.plane;
       constexpr int done = ((R - H) % NS + NS) % NS;
-      const double ku = accU[done], kr = accR[done];
+      const double2 ku = accU[done], kr = accR[done];
+      auto st2 = [](double* q, double2 v) { *reinterpret_cast<double2*>(q) = v; };
       if (!COMBINE) {
-        p.outU[o] = fma(p.adt, ku, un);
-        p.outR[o] = fma(p.adt, kr, rn);
+        st2(p.outU + o, make_double2(fma(p.adt, ku.x, un.x), fma(p.adt, ku.y, un.y)));
+        st2(p.outR + o, make_double2(fma(p.adt, kr.x, rn.x), fma(p.adt, kr.y, rn.y)));
       } else {
         if (p.outU) {
-          p.outU[o] = un + ((p.c2 * (u2 - un) + p.c4 * (u4 - un)) + p.c3 * (u3 - un)) + p.adt * ku;
-          p.outR[o] = rn + ((p.c2 * (r2 - rn) + p.c4 * (r4 - rn)) + p.c3 * (r3 - rn)) + p.adt * kr;
+          st2(p.outU + o, make_double2(un.x + ((p.c2 * (u2.x - un.x) + p.c4 * (u4.x - un.x)) + p.c3 * (u3.x - un.x)) + p.adt * ku.x,
+                                       un.y + ((p.c2 * (u2.y - un.y) + p.c4 * (u4.y - un.y)) + p.c3 * (u3.y - un.y)) + p.adt * ku.y));
+          st2(p.outR + o, make_double2(rn.x + ((p.c2 * (r2.x - rn.x) + p.c4 * (r4.x - rn.x)) + p.c3 * (r3.x - rn.x)) + p.adt * kr.x,
+                                       rn.y + ((p.c2 * (r2.y - rn.y) + p.c4 * (r4.y - rn.y)) + p.c3 * (r3.y - rn.y)) + p.adt * kr.y));
         }
-        if (p.Ku) { p.Ku[o] = ku; p.Kr[o] = kr; }
+        if (p.Ku) { st2(p.Ku + o, ku); st2(p.Kr + o, kr); }
       }
     }
     __syncthreads();
