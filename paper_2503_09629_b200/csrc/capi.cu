@@ -168,6 +168,7 @@ struct Seq {
   uint64_t n = 0;
   bool sub = true;       // subcycled mode (parents keep k_4 for their children)
   bool capturing = false;       // the launches are being captured into a CUDA graph (fork / join allowed)
+  cudaError_t err = cudaSuccess;  // first failing fork / join call of the recording (reported by sc_step)
   std::vector<char> prefilled;  // per level: the next level-step's refinement ghosts are already written
 };
 
@@ -568,16 +569,17 @@ void prefill_second_substep(Seq& q, int level, double dt, bool in_line = false) 
   const Layout& L = h->L;
   cudaStream_t main = h->stream;
   const bool fork = q.capturing && !in_line;
+  auto chk = [&](cudaError_t e) { if (e != cudaSuccess && q.err == cudaSuccess) q.err = e; };
   if (fork) {
-    cudaEventRecord(h->ev_fork[level], main);
-    cudaStreamWaitEvent(h->side, h->ev_fork[level], 0);
+    chk(cudaEventRecord(h->ev_fork[level], main));
+    chk(cudaStreamWaitEvent(h->side, h->ev_fork[level], 0));
     h->stream = h->side;
   }
   if (L.general()) fill_level_dense_ko(q, level, 0.5, dt);
   else fill_level_dense(q, level, 0.5, dt);
   sibling_level(q, level, L.a_state(q.cur[level]), L.V);
   if (fork) {
-    cudaEventRecord(h->ev_join[level], h->side);
+    chk(cudaEventRecord(h->ev_join[level], h->side));
     h->stream = main;
   }
   q.prefilled[level] = fork ? 1 : 2;  // 2: written in line on the main stream, nothing to join
@@ -594,7 +596,10 @@ bool overlap_wanted(const sc_hierarchy* h, int level) {
 // true if the ghosts of the level-step about to start were prefilled (and, in a captured step, joins the branch)
 bool join_prefill(Seq& q, int level) {
   if (!q.prefilled[level]) return false;
-  if (q.prefilled[level] == 1 && q.capturing) cudaStreamWaitEvent(q.h->stream, q.h->ev_join[level], 0);
+  if (q.prefilled[level] == 1 && q.capturing) {
+    const cudaError_t e = cudaStreamWaitEvent(q.h->stream, q.h->ev_join[level], 0);
+    if (e != cudaSuccess && q.err == cudaSuccess) q.err = e;
+  }
   q.prefilled[level] = 0;
   return true;
 }
@@ -935,8 +940,8 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     h->ev_fork.assign(h->L.nlevels, nullptr);
     h->ev_join.assign(h->L.nlevels, nullptr);
     for (int l = 0; l < h->L.nlevels; ++l) {
-      cudaEventCreateWithFlags(&h->ev_fork[l], cudaEventDisableTiming);
-      cudaEventCreateWithFlags(&h->ev_join[l], cudaEventDisableTiming);
+      if ((ce = cudaEventCreateWithFlags(&h->ev_fork[l], cudaEventDisableTiming)) != cudaSuccess) return bail("cudaEventCreate", ce);
+      if ((ce = cudaEventCreateWithFlags(&h->ev_join[l], cudaEventDisableTiming)) != cudaSuccess) return bail("cudaEventCreate", ce);
     }
   }
   const char* eg = getenv("SC_GRAPH");
@@ -983,6 +988,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
   if (!h->use_graph || h->profiling) {
     record_step(q, dt_coarse, subcycling);
     SC_CUDA(cudaGetLastError());
+    SC_CUDA(q.err);
     h->launches += q.n;
   } else {
     GraphKey key{subcycling, 0};
@@ -997,6 +1003,7 @@ int32_t sc_step(sc_hierarchy* h, double dt_coarse, int32_t subcycling) {
       q.capturing = true;
       record_step(q, dt_coarse, subcycling);
       cudaError_t le = cudaGetLastError();
+      if (le == cudaSuccess) le = q.err;
       cudaError_t ee = cudaStreamEndCapture(h->stream, &g);
       ++h->n_captures;
       if (le != cudaSuccess || ee != cudaSuccess) {

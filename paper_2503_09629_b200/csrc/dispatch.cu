@@ -1,6 +1,7 @@
 // dispatch.cu — picks the kernel set: the tuned sm_100a kernels (default: stage_tma.cu, ghost_tma.cu,
 // restrict_zmarch.cu) or the straightforward direct-load kernels of kernels_basic.cu (environment
 // SC_KERNELS=ref; A/B checks and debugging only). Both are CUDA; there is no CPU path.
+#include <atomic>
 #include <cstdlib>
 
 #include "kernels.h"
@@ -30,9 +31,11 @@ void launch_stage_gen_tma(const StageKOArgs& a, cudaStream_t st);
 bool stage_gen_tma_takes(const StageKOArgs& a);
 void stagegen_box_dims(int H, unsigned box[4]);
 
-static int g_mode = 1;
-void select_kernels(int mode) { g_mode = mode; }
-int selected_kernels() { return g_mode; }
+// process-wide (it mirrors the environment variable SC_KERNELS, read when a hierarchy is created); atomic: hierarchies
+// may be created from several host threads
+static std::atomic<int> g_mode{1};
+void select_kernels(int mode) { g_mode.store(mode, std::memory_order_relaxed); }
+int selected_kernels() { return g_mode.load(std::memory_order_relaxed); }
 
 int launch_stage(const StageArgs& a, cudaStream_t st) {
   if (g_mode == 0) { launch_stage_direct(a, st); return 1; }

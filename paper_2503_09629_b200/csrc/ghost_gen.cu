@@ -17,6 +17,7 @@
 // parent point, S31); the footprint of fine cells [I0, I1) along an axis is parents (I0 >> 1) + pmin .. ((I1 - 1) >> 1)
 // + pmin + np - 1, inside the parent's interior by the nesting rule.
 #include "kernels.h"
+#include "launch_cfg.h"
 
 namespace sc {
 
@@ -185,7 +186,7 @@ void launch_ghost_fill_tiled(const GhostArgs& a, cudaStream_t st) {
   const size_t smem = sizeof(double) * ((size_t)GF_MAX_OUT * A.fpcap + A.bcap + (size_t)GT * GT * PL);
   dim3 grd(A.ntiles, a.F, a.nprob);
   auto go = [&](auto kernel) {
-    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);  // cheap; smem depends on g
+    ensure_dynamic_smem(kernel, smem);  // smem depends on g and np
     kernel<<<grd, GNT, smem, st>>>(A);
   };
   if (a.np == 5) go(ghost_fill_tiled<5>);

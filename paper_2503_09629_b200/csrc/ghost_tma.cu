@@ -38,6 +38,7 @@
 #include <cstdlib>
 
 #include "kernels.h"
+#include "launch_cfg.h"
 #include "pdl.h"
 
 namespace sc {
@@ -502,18 +503,10 @@ bool ghost_tma_takes(const GhostArgs& a) {
 }
 
 void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st) {
-  static const int nsm = [] {
-    int dev = 0, n = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    return n > 0 ? n : 148;
-  }();
+  const int nsm = device_sm_count();
   const int maxplanes = GF_MAX_OUT * a.child.g;
   const size_t smem = 1024 + sizeof(double) * ((size_t)GF_MAX_SRC * FOOTMAX + (size_t)maxplanes * TPLANE);
-  static size_t configured = 0;
-  if (smem > configured) {
-    cudaFuncSetAttribute(ghost_fill_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = smem;
-  }
+  ensure_dynamic_smem(ghost_fill_tma, smem);
   const long long nitems = (long long)a.nprob * a.ntiles * a.F;
   const int per_sm = smem <= 112 * 1024 ? 2 : 1;
   const long long want = (long long)nsm * per_sm;

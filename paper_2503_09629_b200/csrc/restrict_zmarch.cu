@@ -17,6 +17,7 @@
 #include <cstdlib>
 
 #include "kernels.h"
+#include "launch_cfg.h"
 #include "pdl.h"
 
 namespace sc {
@@ -141,16 +142,8 @@ void restrict_box_dims(unsigned box[4]) { box[0] = RPITCH; box[1] = RFY; box[2] 
 void launch_restrict_opt(const RestrictArgs& a, cudaStream_t st) {
   if (!a.tmap) { launch_restrict_ref(a, st); return; }
   static const int forced = [] { const char* e = getenv("SC_RCHUNKS"); return e ? atoi(e) : 0; }();
-  static const int nsm = [] {
-    int dev = 0, n = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    return n > 0 ? n : 148;
-  }();
-  static bool configured = false;
-  if (!configured) {
-    cudaFuncSetAttribute(restrict_zmarch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)restrict_smem());
-    configured = true;
-  }
+  const int nsm = device_sm_count();
+  ensure_dynamic_smem(restrict_zmarch, restrict_smem());
   const BoxView& ch = a.child;
   const int npx = ch.n[0] / 2, npy = ch.n[1] / 2, npz = ch.n[2] / 2;
   const int gx = (npx + RPX - 1) / RPX, gy = (npy + RPY - 1) / RPY;

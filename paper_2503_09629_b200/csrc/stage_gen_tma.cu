@@ -19,6 +19,7 @@
 #include <utility>
 
 #include "kernels.h"
+#include "launch_cfg.h"
 
 namespace sc {
 
@@ -252,11 +253,7 @@ template <int RL, int RQ, bool COMBINE>
 void launch_gen(const StageKOArgs& a, GenTmaParams p, cudaStream_t st) {
   constexpr int H = RL > RQ ? RL : RQ;
   constexpr size_t smem = (size_t)GNST * 2 * TileGeo<H>::STRIDE + GNST * 8 + 128;
-  static bool configured = false;
-  if (!configured) {
-    cudaFuncSetAttribute(stage_gen_zmarch<RL, RQ, COMBINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
-  }
+  ensure_dynamic_smem(stage_gen_zmarch<RL, RQ, COMBINE>, smem);
   p.nchunks = stage_pick_chunks(a.b, a.F, 1, 2 * H);
   p.chunk = (a.b.n[2] + p.nchunks - 1) / p.nchunks;
   p.nchunks = (a.b.n[2] + p.chunk - 1) / p.chunk;

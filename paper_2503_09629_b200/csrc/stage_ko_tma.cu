@@ -14,6 +14,7 @@
 #include <type_traits>
 
 #include "kernels.h"
+#include "launch_cfg.h"
 
 namespace sc {
 
@@ -280,11 +281,7 @@ void stageko_box_dims(unsigned box[4]) { box[0] = HXK; box[1] = HYK; box[2] = 1;
 template <int FINAL>
 static void launch_ko_zmarch(const StageKOArgs& a, const KoParams& p0, cudaStream_t st) {
   constexpr size_t smem = (size_t)NSTK * 2 * TILEK * 8 + NSTK * 8 + 128;
-  static bool configured = false;
-  if (!configured) {
-    cudaFuncSetAttribute(stage_ko_zmarch<FINAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
-  }
+  ensure_dynamic_smem(stage_ko_zmarch<FINAL>, smem);
   KoParams p = p0;
   p.nchunks = stage_pick_chunks(a.b, a.F, FINAL == 1 ? 1 : 2, 6);
   p.chunk = (a.b.n[2] + p.nchunks - 1) / p.nchunks;

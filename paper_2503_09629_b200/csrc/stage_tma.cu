@@ -20,6 +20,7 @@
 #include <type_traits>
 
 #include "kernels.h"
+#include "launch_cfg.h"
 #include "pdl.h"
 
 namespace sc {
@@ -304,11 +305,7 @@ size_t stage_smem() { return (size_t)NST * (MODE == STAGE_12 ? 2 : 3) * TILE_DOU
 // z-chunks per column: enough CTAs to fill the machine in whole waves, as few halo planes as possible
 int pick_chunks_impl(const BoxView& b, int F, int ctas_per_sm, int halo_planes) {
   static const int forced = [] { const char* e = getenv("SC_ZCHUNKS"); return e ? atoi(e) : 0; }();
-  static const int nsm = [] {
-    int dev = 0, n = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    return n > 0 ? n : 148;
-  }();
+  const int nsm = device_sm_count();
   if (forced > 0) return forced < b.n[2] ? forced : b.n[2];
   const long long cols = (long long)((b.n[0] + TX - 1) / TX) * ((b.n[1] + TY - 1) / TY) * F;
   const long long slots = (long long)nsm * ctas_per_sm;
@@ -329,12 +326,7 @@ int pick_chunks(const BoxView& b, int F, int ctas_per_sm) { return pick_chunks_i
 
 template <int MODE, bool COUPLED>
 void launch_zmarch(const StageArgs& a, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
-    cudaFuncSetAttribute(stage_zmarch<MODE, COUPLED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         (int)stage_smem<MODE>());
-    configured = true;
-  }
+  ensure_dynamic_smem(stage_zmarch<MODE, COUPLED>, stage_smem<MODE>());
   TmaStageParams p{};
   p.b = a.b;
   p.F = a.F;
