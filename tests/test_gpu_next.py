@@ -154,3 +154,30 @@ def test_radiative_pulse_leaves_the_box_without_the_oracle():
         errs.append(float(np.max(np.abs(G.sc_read_level(0, 0, 0) - wl.spherical_wave_exact(w, 0, 0, 0, steps * w.dt_coarse, 0.35)))))
         G.close()
     assert errs[0] < 0.05 and errs[1] < errs[0] / 3.0, errs
+
+
+@pytest.mark.parametrize("g,interp,vertex,fd", [(5, 0, 0, 4), (4, 1, 0, 8), (5, 1, 0, 8), (3, 0, 1, 4), (5, 1, 1, 8), (2, 0, 1, 4)])
+def test_general_ghost_and_restriction_geometry_sweep(g, interp, vertex, fd):
+    """The general separable ghost fill / restriction (ghost_gen.cu) on child boxes of every offset class (lo mod 4 per
+    axis), sizes that are no multiple of its 16 x 16 tiles or its 8 x 8 x 4 restriction tiles, the smallest box (n = 8) and
+    a child that reaches the nesting margin of each variant: one subcycled + one uniform step, every ghost and interior
+    value against the oracle, index map bit-exact."""
+    B = wl.Box
+    margin = (g + 1) // 2 + (2, 4, 3, 5)[interp + 2 * vertex]
+    cases = [
+        ((40, 32, 36), (2 * margin, 2 * margin, 2 * margin), (80 - 4 * margin, 64 - 4 * margin, 72 - 4 * margin)),  # child up to the margin on every side
+        ((64, 64, 64), (22, 20, 26), (44, 28, 18)),
+        ((64, 64, 64), (20, 22, 24), (30, 46, 34)),
+        ((48, 40, 36), (30, 26, 22), (8, 8, 8)),
+        ((36, 36, 36), (18, 22, 20), (20, 14, 34)),
+    ]
+    for dom, lo, n in cases:
+        w = wl.Workload(f"sweep {dom} {lo} {n} g={g} interp={interp} vertex={vertex}", [B(0, (0, 0, 0), dom), B(1, lo, n)], dom,
+                        ghost=g, interp=interp, vertex=vertex, fd_order=fd, init=wl.multi_gaussian_init(3))
+        G, O = sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+        for sub in (True, False):
+            G.sc_step(w.dt_coarse, sub)
+            O.step(w.dt_coarse, sub)
+            compare_state(G, O, w, what=w.name + f" sub={sub}")
+        assert np.array_equal(G.sc_debug_ghost_map(1, 0), O.ghost_map(1, 0))
+        G.close()
