@@ -50,7 +50,8 @@ typedef struct {
  *   - boxes sorted by level; level 0 is exactly one box with lo = 0 and n = domain_cells
  *     (the periodic domain, reading S9); every level 0..nlevels-1 has at least one box;
  *   - every level >= 1 box: lo and n even on every axis (it covers whole parent cells), n >= 8;
- *     it lies inside ONE box of level-1 with at least 4 parent cells of margin to that box's
+ *     it lies inside ONE box of level-1 with at least ceil(ghost/2) + 2 (= 4 at ghost 3; more with the interp_order /
+ *     centering options below) parent cells of margin to that box's
  *     interior edge (reading S13: the 5-point prolongation footprint never touches parent ghosts);
  *   - the interiors of the boxes of one level are disjoint. Boxes may abut or sit at any distance: every ghost
  *     cell of a box that lies in the interior of a box of the same level takes that box's value of the same
