@@ -9,6 +9,9 @@ section 4, reading S27):
   u components:   |delta| <= 1e-11 * max|u|     (max over the u components of all levels, boxes and fields, oracle
                                                  values, interiors) — exactly as stated; u is never given rho's scale;
   rho components: |delta| <= 1e-11 * max|rho| + F,   F = nsteps * 4 * 2^(L-1) * 2^-53 * (0.625 / dx_finest) * max|u|.
+  over n > 1 coarse steps the floor of rho accumulates (n F) and feeds u through u += dt rho:  the u bound gains
+  F_u(n) = dt_coarse * F(1) * n (n + 1) / 2  (7e-14 max|u| for n = 1 at cfg 5's depth: nothing; 1.4e-11 for its 20 steps), with
+  max|u| in F taken over the run (`floor_scale`: the pulse of cfg 5 decays to 0.3 of its initial height).
 F is the rounding floor of the DEFINITION, not an allowance for the kernels: one RHS evaluation forms Lap_h u from
 terms of size 30 |u| / (12 dx^2), so rho = d_t u is rounded by eps * 2.5 |u| dt / dx^2 = eps * 0.625 |u| / dx per
 evaluation (dt = dx / 4), and the finest of L levels is evaluated 4 * 2^(L-1) times per coarse step. For shallow
@@ -50,16 +53,22 @@ def rho_floor(w, su: float, nsteps: int = 1) -> float:
     return nsteps * 4.0 * (1 << (L - 1)) * 2.0 ** -53 * (0.625 / w.dx(L - 1)) * su
 
 
+def u_floor(w, su: float, nsteps: int = 1) -> float:
+    """F_u of the module docstring: what the accumulated rounding of rho adds to u over `nsteps` coarse steps."""
+    return w.dt_coarse * rho_floor(w, su, 1) * nsteps * (nsteps + 1) / 2.0
+
+
 def compare_state(G, O, w, padded: bool = True, what: str = "state", rtol: float = RTOL, levels=None,
-                  nsteps: int = 1) -> float:
+                  nsteps: int = 1, floor_scale: float = 0.0) -> float:
     """Assert the tolerance of the module docstring for every component of every box (ghosts included if `padded`);
     returns the worst difference in units of its component type's bound / rtol. One array pair is alive at a time.
-    `nsteps`: coarse steps taken since the two states were equal (only scales the rounding floor of rho; the default
-    1 is the strictest)."""
+    `nsteps`: coarse steps taken since the two states were equal (only scales the rounding floors; the default 1 is
+    the strictest); `floor_scale`: max|u| over the run if it was larger than it is now."""
     su = u_scale(O, w)
     assert su > 0.0 and np.isfinite(su), (what, su)
-    tol_u = rtol * su
-    tol_r = rtol * max(rho_scale(O, w), su) + rho_floor(w, su, nsteps)
+    fs = max(su, floor_scale)
+    tol_u = rtol * su + u_floor(w, fs, nsteps)
+    tol_r = rtol * max(rho_scale(O, w), su) + rho_floor(w, fs, nsteps)
     worst = 0.0
     for l in (range(w.nlevels) if levels is None else levels):
         for ib in range(len(w.level_boxes(l))):

@@ -914,7 +914,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   h->gmap_ok.assign(h->L.boxes.size(), 0);
   for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
     const BoxInfo& b = h->L.boxes[ib];
-    h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 0, h->tmaps[ib].bytes) &&
+    h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), stage_tile_variant(b.v, h->L.F) ? 8 : 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
     {  // the general path's stage tile: halo 3 (4th-order differences), 4 (8th order) or 5 (with delta^10)
       const Layout& L = h->L;

@@ -13,7 +13,7 @@ void launch_stage_fd8(const StageArgs& a, cudaStream_t st);
 int launch_stage_tma(const StageArgs& a, cudaStream_t st);
 bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned box[4], int l2_promotion,
                              bool swizzle64, void* out_map128);
-void stage_box_dims(unsigned box[4]);
+void stage_box_dims(int variant, unsigned box[4]);
 void restrict_box_dims(unsigned box[4]);
 void launch_ghost_fill_direct(const GhostArgs& a, cudaStream_t st);
 void launch_ghost_fill_tma(const GhostArgs& a, cudaStream_t st);
@@ -66,7 +66,7 @@ void launch_restrict(const RestrictArgs& a, cudaStream_t st) {
 }
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128) {
   unsigned box[4];
-  if (kind == 0) stage_box_dims(box);
+  if (kind == 0 || kind == 8) stage_box_dims(kind == 8, box);  // the stage kernels' halo tile: 32 x 16 or 64 x 7 cells
   else if (kind == 1) restrict_box_dims(box);
   else if (kind <= 4) ghost_box_dims(kind - 2, box);
   else if (kind == 5) stageko_box_dims(box);

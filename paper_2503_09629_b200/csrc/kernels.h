@@ -46,9 +46,11 @@ struct StageArgs {
   int a_yn, a_Y2r, a_Y3r;
 };
 int launch_stage(const StageArgs& a, cudaStream_t st);  // returns the number of kernels launched
+int stage_tile_variant(const BoxView& b, int F);          // which halo tile the tuned stage kernels use on this box (tensor map kind 0 / 8)
 // 128-byte CUtensorMaps of a box: dims (px, py, pz, narrays), fp64, no swizzle; kind 0: box = the stage
 // kernels' halo tile, kind 1: box = the restriction kernel's pair of fine planes, kinds 2..4: the ghost
-// fill's parent footprint of a tile of an x- / y- / z-slab, kind 5: the dissipative stage kernel's halo-3 tile. Returns false (and leaves
+// fill's parent footprint of a tile of an x- / y- / z-slab, kind 5: the dissipative stage kernel's halo-3 tile, kinds 6, 7: the
+// wide-stencil stage kernel's halo-4 / halo-5 tiles, kind 8: the stage kernels' 64 x 7 tile. Returns false (and leaves
 // the direct-load kernels in charge) when the driver entry point is unavailable or a TMA limit is violated.
 bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, void* out_map128);
 

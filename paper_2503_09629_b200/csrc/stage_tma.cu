@@ -1,7 +1,7 @@
 // stage_tma.cu — tuned RK4 stage kernels (eqs 1-9 on the wave system
 // PAPER.md:222-226), sm_100a: z-march with TMA-staged halo planes.
 //
-// One CTA owns a TX x TY column of cells and marches through a chunk of z-planes. Every plane of every
+// One CTA owns a TX x TY column of cells (32 x 16 or 64 x 7, chosen per box: Tile) and marches through a chunk of z-planes. Every plane of every
 // halo-read array arrives in shared memory as a (TX+4) x (TY+4) tile through ONE TMA tiled load
 // (cp.async.bulk.tensor.4d, box dims (x, y, 1 plane, 1 array)) signalled on an mbarrier; NST planes are in
 // flight so HBM latency never meets a warp. A thread owns two x-adjacent cells (16-byte shared loads and
@@ -26,15 +26,25 @@
 namespace sc {
 
 void launch_stage_direct(const StageArgs& a, cudaStream_t st);
+int stage_tile_variant(const BoxView& b, int F);
 
 namespace {
 
-constexpr int TX = 32, TY = 16;              // cells per CTA column
-constexpr int HX = TX + 4, HY = TY + 4;      // halo tile
-constexpr int NTHR = (TX / 2) * TY;          // 256 threads, two cells each
-constexpr int TILE_DOUBLES = HX * HY;        // 720 doubles = 5760 B (multiple of 128 B)
+// Tile of cells per CTA column, chosen per box (stage_tile_variant): 32 x 16 — 256 threads, halo tile 36 x 20 — or
+// 64 x 7 — 224 threads, halo tile 68 x 11. The second exists for boxes like 256^3, where 32 x 16 gives 128 columns x 2
+// z-chunks = 256 CTAs on the 296 resident slots of 148 SMs (40 SMs then carry one CTA and the launch lasts as long as
+// the SMs that carry two), while 64 x 7 gives 4 x 37 = 148 columns x 2 chunks = two CTAs on EVERY SM, all marching
+// in lock step: 136.5 -> 130.9 us per launch although its halo is larger (1.67x the interior instead of 1.41x).
+template <int TX_, int TY_> struct Tile {
+  static constexpr int TX = TX_, TY = TY_;
+  static constexpr int HX = TX + 4, HY = TY + 4;      // halo tile
+  static constexpr int NTHR = (TX / 2) * TY;          // two x-adjacent cells per thread
+  static constexpr int TILE_BYTES = HX * HY * 8;      // what one TMA tiled load writes
+  static constexpr int TILE_DOUBLES = (TILE_BYTES + 127) / 128 * 16;  // distance between tiles in shared memory (128-byte aligned)
+};
+using TileA = Tile<32, 16>;
+using TileB = Tile<64, 7>;
 constexpr int NST = 4;                       // planes in flight
-static_assert((TILE_DOUBLES * 8) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -81,6 +91,7 @@ struct Nbr {
   double2 xa, xb, xc;          // row y: columns x-2..x+3
   double2 ym2, ym1, yp1, yp2;  // columns x, x+1 of rows y-2, y-1, y+1, y+2
 };
+template <int HX>
 __device__ __forceinline__ Nbr load_nbr(const double* tile, int tx, int ty) {
   Nbr n;
   const double2* r = reinterpret_cast<const double2*>(tile + (ty + 2) * HX + 2 * tx);
@@ -91,6 +102,7 @@ __device__ __forceinline__ Nbr load_nbr(const double* tile, int tx, int ty) {
   n.yp2 = *reinterpret_cast<const double2*>(tile + (ty + 4) * HX + 2 * tx + 2);
   return n;
 }
+template <int HX>
 __device__ __forceinline__ double2 load_centre(const double* tile, int tx, int ty) {
   return *reinterpret_cast<const double2*>(tile + (ty + 2) * HX + 2 * tx + 2);
 }
@@ -128,10 +140,11 @@ __device__ __forceinline__ void scatter(double2 (&acc)[5], double2 centre_term, 
 
 }  // namespace
 
-template <int MODE, bool COUPLED>
-__global__ void __launch_bounds__(NTHR, 2)
+template <int MODE, bool COUPLED, class T>
+__global__ void __launch_bounds__(T::NTHR, 2)
     stage_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ TmaStageParams p) {
   constexpr int NH = MODE == STAGE_12 ? 2 : 3;  // halo-read arrays per plane
+  constexpr int TX = T::TX, TY = T::TY, HX = T::HX, TILE_DOUBLES = T::TILE_DOUBLES;
   pdl_enter();
   extern __shared__ unsigned char smraw[];
   // [NST][NH] tiles, 128-byte aligned for TMA, then NST mbarriers
@@ -155,7 +168,7 @@ __global__ void __launch_bounds__(NTHR, 2)
   auto issue = [&](int it) {  // one thread: arm the stage's mbarrier and request the plane's tiles
     const int st = it % NST;
     const uint32_t bar = bar0 + 8 * st;
-    mbar_expect_tx(bar, NH * TILE_DOUBLES * 8);
+    mbar_expect_tx(bar, NH * T::TILE_BYTES);
 #pragma unroll
     for (int h = 0; h < NH; ++h)
       tma_load_4d(s0 + (st * NH + h) * TILE_DOUBLES * 8, &tmap, XOFF + X0 - 2, b.g + Y0 - 2, b.g + zs + dir * it,
@@ -212,7 +225,7 @@ __global__ void __launch_bounds__(NTHR, 2)
     double2 ctA = make_double2(0.0, 0.0), ctB = ctA, zcA, zcB;
     if (MODE == STAGE_12) {
       if (inpl) {
-        const Nbr u = load_nbr(t0, tx, ty), r = load_nbr(t0 + TILE_DOUBLES, tx, ty);
+        const Nbr u = load_nbr<HX>(t0, tx, ty), r = load_nbr<HX>(t0 + TILE_DOUBLES, tx, ty);
         const Nbr w = axpy(hdt, r, u);
         const double2 iu = inplane(u, wxA, wyA, cA), iw = inplane(w, wxB, wyB, cB);
         ctA = make_double2(r.xb.x + iu.x, r.xb.y + iu.y);
@@ -221,15 +234,15 @@ __global__ void __launch_bounds__(NTHR, 2)
         zcA = make_double2(wzA * u.xb.x, wzA * u.xb.y);
         zcB = make_double2(wzB * w.xb.x, wzB * w.xb.y);
       } else {
-        const double2 uc = load_centre(t0, tx, ty), rc = load_centre(t0 + TILE_DOUBLES, tx, ty);
+        const double2 uc = load_centre<HX>(t0, tx, ty), rc = load_centre<HX>(t0 + TILE_DOUBLES, tx, ty);
         const double2 wc = fma2(hdt, rc, uc);
         zcA = make_double2(wzA * uc.x, wzA * uc.y);
         zcB = make_double2(wzB * wc.x, wzB * wc.y);
       }
     } else {
       if (inpl) {
-        const Nbr u = load_nbr(t0, tx, ty);
-        const Nbr y2 = load_nbr(t0 + TILE_DOUBLES, tx, ty), y3 = load_nbr(t0 + 2 * TILE_DOUBLES, tx, ty);
+        const Nbr u = load_nbr<HX>(t0, tx, ty);
+        const Nbr y2 = load_nbr<HX>(t0 + TILE_DOUBLES, tx, ty), y3 = load_nbr<HX>(t0 + 2 * TILE_DOUBLES, tx, ty);
         const Nbr w3 = axpy(hdt, y2, u), w4 = axpy(dt, y3, u);
         const double2 i3 = inplane(w3, wxA, wyA, cA), i4 = inplane(w4, wxB, wyB, cB);
         ctA = make_double2(rho_c.x + i3.x, rho_c.y + i3.y);
@@ -242,9 +255,9 @@ __global__ void __launch_bounds__(NTHR, 2)
         zcA = make_double2(wzA * w3.xb.x, wzA * w3.xb.y);
         zcB = make_double2(wzB * w4.xb.x, wzB * w4.xb.y);
       } else {
-        const double2 uc = load_centre(t0, tx, ty);
-        const double2 w3 = fma2(hdt, load_centre(t0 + TILE_DOUBLES, tx, ty), uc);
-        const double2 w4 = fma2(dt, load_centre(t0 + 2 * TILE_DOUBLES, tx, ty), uc);
+        const double2 uc = load_centre<HX>(t0, tx, ty);
+        const double2 w3 = fma2(hdt, load_centre<HX>(t0 + TILE_DOUBLES, tx, ty), uc);
+        const double2 w4 = fma2(dt, load_centre<HX>(t0 + 2 * TILE_DOUBLES, tx, ty), uc);
         zcA = make_double2(wzA * w3.x, wzA * w3.y);
         zcB = make_double2(wzB * w4.x, wzB * w4.y);
       }
@@ -299,38 +312,49 @@ EncodeTiledFn encode_tiled() {
   return fn;
 }
 
-template <int MODE>
-size_t stage_smem() { return (size_t)NST * (MODE == STAGE_12 ? 2 : 3) * TILE_DOUBLES * 8 + NST * 8 + 128; }
+template <int MODE, class T>
+size_t stage_smem() { return (size_t)NST * (MODE == STAGE_12 ? 2 : 3) * T::TILE_DOUBLES * 8 + NST * 8 + 128; }
 
-// z-chunks per column: enough CTAs to fill the machine in whole waves, as few halo planes as possible
-int pick_chunks_impl(const BoxView& b, int F, int ctas_per_sm, int halo_planes) {
+// z-chunks per column of tx x ty cells: enough CTAs to fill the machine in whole waves, as few halo planes as possible.
+// *cost_out: waves x (planes marched + pipeline fill), the launch's length in plane-steps of one CTA.
+int pick_chunks_impl(const BoxView& b, int F, int ctas_per_sm, int halo_planes, int tx = 32, int ty = 16,
+                     double* cost_out = nullptr) {
   static const int forced = [] { const char* e = getenv("SC_ZCHUNKS"); return e ? atoi(e) : 0; }();
   const int nsm = device_sm_count();
-  if (forced > 0) return forced < b.n[2] ? forced : b.n[2];
-  const long long cols = (long long)((b.n[0] + TX - 1) / TX) * ((b.n[1] + TY - 1) / TY) * F;
+  const long long cols = (long long)((b.n[0] + tx - 1) / tx) * ((b.n[1] + ty - 1) / ty) * F;
   const long long slots = (long long)nsm * ctas_per_sm;
   int best = 1;
   double best_cost = 1e300;
   const int maxch = b.n[2] / 8 > 1 ? b.n[2] / 8 : 1;
   for (int nch = 1; nch <= maxch; ++nch) {
+    if (forced > 0 && nch != (forced < b.n[2] ? forced : b.n[2])) continue;
     const int ch = (b.n[2] + nch - 1) / nch;
     const long long ctas = cols * ((b.n[2] + ch - 1) / ch);
     const long long waves = (ctas + slots - 1) / slots;
     const double cost = (double)waves * (ch + halo_planes + 6);  // time ~ waves x (planes marched + pipeline fill)
     if (cost < best_cost - 1e-9) { best_cost = cost; best = nch; }
   }
+  if (cost_out) *cost_out = best_cost;
   return best;
 }
 
-int pick_chunks(const BoxView& b, int F, int ctas_per_sm) { return pick_chunks_impl(b, F, ctas_per_sm, 4); }
+template <class T>
+double tile_cost(const BoxView& b, int F) {
+  // a CTA's time per plane grows with its cells; the larger halo of a flatter tile costs about a third of its share
+  // (measured on 256^3: 64 x 7 against 32 x 16, see Tile)
+  double planes = 0.0;
+  pick_chunks_impl(b, F, 2, 4, T::TX, T::TY, &planes);
+  const double halo = (double)(T::HX * T::HY) / (T::TX * T::TY);
+  return planes * T::TX * T::TY * (1.0 + 0.3 * (halo - 1.0));
+}
 
-template <int MODE, bool COUPLED>
+template <int MODE, bool COUPLED, class T>
 void launch_zmarch(const StageArgs& a, cudaStream_t st) {
-  ensure_dynamic_smem(stage_zmarch<MODE, COUPLED>, stage_smem<MODE>());
+  ensure_dynamic_smem(stage_zmarch<MODE, COUPLED, T>, stage_smem<MODE, T>());
   TmaStageParams p{};
   p.b = a.b;
   p.F = a.F;
-  p.nchunks = pick_chunks(a.b, a.F, 2);
+  p.nchunks = pick_chunks_impl(a.b, a.F, 2, 4, T::TX, T::TY);
   p.chunk = (a.b.n[2] + p.nchunks - 1) / p.nchunks;
   p.nchunks = (a.b.n[2] + p.chunk - 1) / p.chunk;
   p.write_Y4r = a.write_Y4r;
@@ -339,8 +363,14 @@ void launch_zmarch(const StageArgs& a, cudaStream_t st) {
   p.dt = a.dt;
   for (int d = 0; d < 3; ++d) p.w[d] = a.inv12dx2[d];
   p.S = a.S;
-  dim3 grd((a.b.n[0] + TX - 1) / TX, (a.b.n[1] + TY - 1) / TY, p.nchunks * a.F);
-  launch_pdl(stage_zmarch<MODE, COUPLED>, grd, dim3(NTHR), stage_smem<MODE>(), st, *static_cast<const CUtensorMap*>(a.tmap), p);
+  dim3 grd((a.b.n[0] + T::TX - 1) / T::TX, (a.b.n[1] + T::TY - 1) / T::TY, p.nchunks * a.F);
+  launch_pdl(stage_zmarch<MODE, COUPLED, T>, grd, dim3(T::NTHR), stage_smem<MODE, T>(), st,
+             *static_cast<const CUtensorMap*>(a.tmap), p);
+}
+template <int MODE, bool COUPLED>
+void launch_zmarch_v(const StageArgs& a, cudaStream_t st) {
+  if (stage_tile_variant(a.b, a.F)) launch_zmarch<MODE, COUPLED, TileB>(a, st);
+  else launch_zmarch<MODE, COUPLED, TileA>(a, st);
 }
 
 }  // namespace
@@ -435,7 +465,20 @@ int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes)
   return pick_chunks_impl(b, F, ctas_per_sm, halo_planes);
 }
 
-void stage_box_dims(unsigned box[4]) { box[0] = HX; box[1] = HY; box[2] = 1; box[3] = 1; }
+// which tile the stage kernels use on this box (0: 32 x 16, 1: 64 x 7): a function of the box and the device only, so
+// that the tensor map built at creation and every later launch agree. SC_STAGE_TILE=0|1 forces it (A/B checks).
+int stage_tile_variant(const BoxView& b, int F) {
+  static const int forced = [] { const char* e = getenv("SC_STAGE_TILE"); return e ? atoi(e) : -1; }();
+  if (forced >= 0) return forced ? 1 : 0;
+  return tile_cost<TileB>(b, F) < 0.97 * tile_cost<TileA>(b, F) ? 1 : 0;
+}
+
+void stage_box_dims(int variant, unsigned box[4]) {
+  box[0] = variant ? TileB::HX : TileA::HX;
+  box[1] = variant ? TileB::HY : TileA::HY;
+  box[2] = 1;
+  box[3] = 1;
+}
 
 bool make_box_tensor_map_tma(const BoxView& b, int narrays, void* base, const unsigned bx[4], int l2_promotion,
                              bool swizzle64, void* out_map128) {
@@ -464,11 +507,11 @@ int launch_stage_tma(const StageArgs& a, cudaStream_t st) {
   if (!a.tmap || (a.A && !(a.S && a.A_host))) { launch_stage_direct(a, st); return 1; }
   if (a.A) {  // coupling terms first (pointwise F x F product over all fields), then the per-field z-march
     launch_couple_matvec(a, st);
-    if (a.mode == STAGE_12) launch_zmarch<STAGE_12, true>(a, st);
-    else launch_zmarch<STAGE_34, true>(a, st);
+    if (a.mode == STAGE_12) launch_zmarch_v<STAGE_12, true>(a, st);
+    else launch_zmarch_v<STAGE_34, true>(a, st);
   } else {
-    if (a.mode == STAGE_12) launch_zmarch<STAGE_12, false>(a, st);
-    else launch_zmarch<STAGE_34, false>(a, st);
+    if (a.mode == STAGE_12) launch_zmarch_v<STAGE_12, false>(a, st);
+    else launch_zmarch_v<STAGE_34, false>(a, st);
   }
   return a.A ? 2 : 1;
 }
