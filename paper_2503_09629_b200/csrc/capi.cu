@@ -919,9 +919,9 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
     {  // the general path's stage tile: halo 3 (4th-order differences), 4 (8th order) or 5 (with delta^10)
       const Layout& L = h->L;
       const bool ko9 = L.ko_sigma > 0.0 && L.ko_order == 9;
-      const int kind = L.fd_order == 8 ? (ko9 ? 7 : 6) : 5;
-      const int need = kind == 7 ? 5 : (kind == 6 ? 4 : 3);
-      h->kmap_ok[ib] = L.general() && (kind != 5 || !ko9) && L.g >= need &&
+      const int kind = L.fd_order == 8 ? (ko9 ? 7 : 6) : (stage_tile_variant(b.v, L.F) ? 9 : 5);
+      const int need = kind == 7 ? 5 : (kind == 6 ? 4 : 3);  // kinds 5, 9: halo 3
+      h->kmap_ok[ib] = L.general() && (L.fd_order == 8 || !ko9) && L.g >= need &&
                        make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), kind, h->kmaps[ib].bytes);
     }
     h->gmap_ok[ib] = 1;

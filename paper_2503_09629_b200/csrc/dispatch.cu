@@ -26,7 +26,7 @@ void launch_restrict_tiled(const RestrictArgs& a, cudaStream_t st);
 void launch_stage_ko_direct(const StageKOArgs& a, cudaStream_t st);
 void launch_stage_ko_tma(const StageKOArgs& a, cudaStream_t st);
 bool stage_ko_tma_takes(const StageKOArgs& a);
-void stageko_box_dims(unsigned box[4]);
+void stageko_box_dims(int variant, unsigned box[4]);
 void launch_stage_gen_tma(const StageKOArgs& a, cudaStream_t st);
 bool stage_gen_tma_takes(const StageKOArgs& a);
 void stagegen_box_dims(int H, unsigned box[4]);
@@ -69,8 +69,8 @@ bool make_box_tensor_map(const BoxView& b, int narrays, void* base, int kind, vo
   if (kind == 0 || kind == 8) stage_box_dims(kind == 8, box);  // the stage kernels' halo tile: 32 x 16 or 64 x 7 cells
   else if (kind == 1) restrict_box_dims(box);
   else if (kind <= 4) ghost_box_dims(kind - 2, box);
-  else if (kind == 5) stageko_box_dims(box);
-  else stagegen_box_dims(kind == 7 ? 5 : 4, box);  // kinds 6, 7: the general path's halo-4 / halo-5 tiles
+  else if (kind == 5 || kind == 9) stageko_box_dims(kind == 9, box);  // the dissipative stage kernel's halo-3 tile, 32 x 16 / 64 x 7
+  else if (kind != 8) stagegen_box_dims(kind == 7 ? 5 : 4, box);  // kinds 6, 7: the general path's halo-4 / halo-5 tiles
   // streaming tiles (stage, restriction) promote misses to 256-byte fetches; the ghost fill's footprint rows are
   // 64-160 bytes and isolated: promotion there only multiplies the DRAM traffic. The x-slab footprint (kind 2,
   // 64-byte rows) is swizzled so that one-thread-per-row reads are bank-conflict free (ghost_tma.cu).

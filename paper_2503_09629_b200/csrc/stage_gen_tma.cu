@@ -8,7 +8,7 @@
 // halo-read arrays arrives as one TMA tiled load each into an mbarrier ring, the z-stencils live in registers in scatter
 // form (an arriving plane adds its in-plane part to its own output plane and its centre value, times the z weights, to
 // the 2H neighbouring output planes, H = max(RL, RQ); output plane p - H is complete when plane p has arrived). Tile
-// 64 x 8 cells, 256 threads, two x-adjacent cells per thread (every shared load is 16 bytes), one CTA per SM with the
+// 64 x 7 cells (4 x 37 = 148 columns of a 256^2 plane: one CTA on every SM), 224 threads, two x-adjacent cells per thread (every shared load is 16 bytes), one CTA per SM with the
 // whole register file (2 (2H + 1) double2 accumulators per thread), a 6-deep ring. Measured on the way (256^3, fd 8 +
 // delta^6 / delta^10): one cell per thread, 512 threads: 252 / 323 us, ncu: `mio_throttle` 2.7 stall cycles per issue
 // (30 8-byte shared loads per thread and plane); this form: 254 / 277 us; the direct-load stage_gen: 368 / 421 us. A
@@ -23,11 +23,11 @@
 
 namespace sc {
 
-int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes);
+int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes, int tx, int ty);
 
 namespace {
 
-constexpr int GTX = 64, GTY = 8, GNTHR = (GTX / 2) * GTY;  // two x-adjacent cells per thread: every shared load is 16 bytes
+constexpr int GTX = 64, GTY = 7, GNTHR = (GTX / 2) * GTY;  // two x-adjacent cells per thread: every shared load is 16 bytes
 constexpr int GNST = 6;  // planes in flight
 
 template <int H> struct TileGeo {
@@ -254,7 +254,7 @@ void launch_gen(const StageKOArgs& a, GenTmaParams p, cudaStream_t st) {
   constexpr int H = RL > RQ ? RL : RQ;
   constexpr size_t smem = (size_t)GNST * 2 * TileGeo<H>::STRIDE + GNST * 8 + 128;
   ensure_dynamic_smem(stage_gen_zmarch<RL, RQ, COMBINE>, smem);
-  p.nchunks = stage_pick_chunks(a.b, a.F, 1, 2 * H);
+  p.nchunks = stage_pick_chunks(a.b, a.F, 1, 2 * H, GTX, GTY);
   p.chunk = (a.b.n[2] + p.nchunks - 1) / p.nchunks;
   p.nchunks = (a.b.n[2] + p.chunk - 1) / p.chunk;
   dim3 grd((a.b.n[0] + GTX - 1) / GTX, (a.b.n[1] + GTY - 1) / GTY, p.nchunks * a.F);

@@ -18,16 +18,22 @@
 
 namespace sc {
 
-int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes);
+int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes, int tx, int ty);
 
 namespace {
 
-constexpr int TX = 32, TY = 16;
-constexpr int HXK = TX + 8, HYK = TY + 6;      // tile: x from X0-4 (even start), y from Y0-3
-constexpr int NTHR = (TX / 2) * TY;            // 256 threads, two x-adjacent cells each
-constexpr int TILEK = HXK * HYK;               // 880 doubles = 7040 B (multiple of 128 B)
+// Tile of cells per CTA column: 32 x 16 or 64 x 7, the same choice per box as stage_tma.cu (stage_tile_variant: on
+// 256^3 the second makes 148 columns, i.e. whole CTAs-per-SM multiples on 148 SMs with all columns in lock step)
+template <int TX_, int TY_> struct TileK {
+  static constexpr int TX = TX_, TY = TY_;
+  static constexpr int HXK = TX + 8, HYK = TY + 6;      // tile: x from X0-4 (even start), y from Y0-3
+  static constexpr int NTHR = (TX / 2) * TY;            // two x-adjacent cells per thread
+  static constexpr int TILE_BYTES = HXK * HYK * 8;      // what one TMA tiled load writes
+  static constexpr int TILEK = (TILE_BYTES + 127) / 128 * 16;  // doubles between tiles in shared memory (128-byte aligned)
+};
+using TileKA = TileK<32, 16>;
+using TileKB = TileK<64, 7>;
 constexpr int NSTK = 4;                        // planes in flight
-static_assert((TILEK * 8) % 128 == 0, "TMA destination tiles must stay 128-byte aligned");
 
 __device__ __forceinline__ uint32_t smem_u32k(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_wait_k(uint32_t bar, uint32_t parity) {
@@ -65,6 +71,7 @@ struct Nbr3 {
   double2 xa, xb, xc, xd, xe;                   // row y: columns x-4 .. x+5
   double2 ym3, ym2, ym1, yp1, yp2, yp3;         // columns x, x+1 of rows y-3 .. y+3
 };
+template <int HXK>
 __device__ __forceinline__ Nbr3 load_nbr3(const double* tile, int tx, int ty) {
   Nbr3 n;
   const double2* r = reinterpret_cast<const double2*>(tile + (ty + 3) * HXK + 2 * tx);
@@ -78,6 +85,7 @@ __device__ __forceinline__ Nbr3 load_nbr3(const double* tile, int tx, int ty) {
   n.yp3 = *reinterpret_cast<const double2*>(c + (ty + 6) * HXK);
   return n;
 }
+template <int HXK>
 __device__ __forceinline__ double2 load_centre3(const double* tile, int tx, int ty) {
   return *reinterpret_cast<const double2*>(tile + (ty + 3) * HXK + 2 * tx + 4);
 }
@@ -125,9 +133,10 @@ __device__ __forceinline__ void scatter7(double2 (&acc)[7], double2 ct, double2 
 // the 4-deep TMA ring and the one-plane-ahead global loads still cover the memory latency)
 // FINAL: 0 = simple stage (out = y_n + adt k), 1 = full combine (up to three more centre operands; one CTA per SM),
 // 2 = light combine (the stage's own input as the only extra operand: RK3 stage 2, RK2 stage 2, RK3's extra slope)
-template <int FINAL>
-__global__ void __launch_bounds__(NTHR, FINAL == 1 ? 1 : 2)
+template <int FINAL, class T>
+__global__ void __launch_bounds__(T::NTHR, FINAL == 1 ? 1 : 2)
     stage_ko_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ KoParams p) {
+  constexpr int TX = T::TX, TY = T::TY, HXK = T::HXK, TILEK = T::TILEK;
   extern __shared__ unsigned char smraw[];
   // [NSTK][2] tiles (U, R), 128-byte aligned for TMA, then NSTK mbarriers
   const uint32_t s0 = (smem_u32k(smraw) + 127u) & ~127u;
@@ -146,7 +155,7 @@ __global__ void __launch_bounds__(NTHR, FINAL == 1 ? 1 : 2)
   auto issue = [&](int it) {  // one thread: arm the stage's mbarrier and request the plane's two tiles
     const int st = it % NSTK;
     const uint32_t bar = bar0 + 8 * st;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(2 * TILEK * 8) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(2 * T::TILE_BYTES) : "memory");
 #pragma unroll
     for (int h = 0; h < 2; ++h)
       asm volatile(
@@ -211,8 +220,8 @@ __global__ void __launch_bounds__(NTHR, FINAL == 1 ? 1 : 2)
     const double* __restrict__ tR = tU + TILEK;
     double2 ctU = zero2, ctR = zero2, uc, rc;
     if (inpl) {
-      const Nbr3 U = load_nbr3(tU, tx, ty);
-      const Nbr3 Rr = load_nbr3(tR, tx, ty);
+      const Nbr3 U = load_nbr3<HXK>(tU, tx, ty);
+      const Nbr3 Rr = load_nbr3<HXK>(tR, tx, ty);
       uc = U.xc; rc = Rr.xc;
       const double2 qU = fma2k(kx, d6x(U), fma2k(ky, d6y(U), mul2(-20.0 * kz, uc)));
       const double2 qR = fma2k(kx, d6x(Rr), fma2k(ky, d6y(Rr), mul2(-20.0 * kz, rc)));
@@ -220,8 +229,8 @@ __global__ void __launch_bounds__(NTHR, FINAL == 1 ? 1 : 2)
       ctU = add2(rc, qU);
       ctR = add2(lU, qR);
     } else {
-      uc = load_centre3(tU, tx, ty);
-      rc = load_centre3(tR, tx, ty);
+      uc = load_centre3<HXK>(tU, tx, ty);
+      rc = load_centre3<HXK>(tR, tx, ty);
     }
     // z contributions of this plane: Q on U -> k_u;  Lap on U and Q on R -> k_rho
     scatter7<R>(accU, ctU, mul2(15.0 * kz, uc), mul2(-6.0 * kz, uc), mul2(kz, uc));
@@ -276,18 +285,28 @@ __global__ void __launch_bounds__(NTHR, FINAL == 1 ? 1 : 2)
 }
 
 // ---- host ------------------------------------------------------------------------------------------
-void stageko_box_dims(unsigned box[4]) { box[0] = HXK; box[1] = HYK; box[2] = 1; box[3] = 1; }
+void stageko_box_dims(int variant, unsigned box[4]) {
+  box[0] = variant ? TileKB::HXK : TileKA::HXK;
+  box[1] = variant ? TileKB::HYK : TileKA::HYK;
+  box[2] = 1;
+  box[3] = 1;
+}
 
-template <int FINAL>
-static void launch_ko_zmarch(const StageKOArgs& a, const KoParams& p0, cudaStream_t st) {
-  constexpr size_t smem = (size_t)NSTK * 2 * TILEK * 8 + NSTK * 8 + 128;
-  ensure_dynamic_smem(stage_ko_zmarch<FINAL>, smem);
+template <int FINAL, class T>
+static void launch_ko_zmarch_t(const StageKOArgs& a, const KoParams& p0, cudaStream_t st) {
+  constexpr size_t smem = (size_t)NSTK * 2 * T::TILEK * 8 + NSTK * 8 + 128;
+  ensure_dynamic_smem(stage_ko_zmarch<FINAL, T>, smem);
   KoParams p = p0;
-  p.nchunks = stage_pick_chunks(a.b, a.F, FINAL == 1 ? 1 : 2, 6);
+  p.nchunks = stage_pick_chunks(a.b, a.F, FINAL == 1 ? 1 : 2, 6, T::TX, T::TY);
   p.chunk = (a.b.n[2] + p.nchunks - 1) / p.nchunks;
   p.nchunks = (a.b.n[2] + p.chunk - 1) / p.chunk;
-  dim3 grd((a.b.n[0] + TX - 1) / TX, (a.b.n[1] + TY - 1) / TY, p.nchunks * a.F);
-  stage_ko_zmarch<FINAL><<<grd, NTHR, smem, st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
+  dim3 grd((a.b.n[0] + T::TX - 1) / T::TX, (a.b.n[1] + T::TY - 1) / T::TY, p.nchunks * a.F);
+  stage_ko_zmarch<FINAL, T><<<grd, T::NTHR, smem, st>>>(*static_cast<const CUtensorMap*>(a.tmap), p);
+}
+template <int FINAL>
+static void launch_ko_zmarch(const StageKOArgs& a, const KoParams& p0, cudaStream_t st) {
+  if (stage_tile_variant(a.b, a.F)) launch_ko_zmarch_t<FINAL, TileKB>(a, p0, st);
+  else launch_ko_zmarch_t<FINAL, TileKA>(a, p0, st);
 }
 
 // the tuned kernel takes uncoupled systems whose box has a tensor map, 4th-order differences, no or fifth-order

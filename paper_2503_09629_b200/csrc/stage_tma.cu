@@ -461,8 +461,8 @@ void launch_couple_matvec(const StageArgs& a, cudaStream_t st) {
 }
 }  // namespace
 
-int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes) {
-  return pick_chunks_impl(b, F, ctas_per_sm, halo_planes);
+int stage_pick_chunks(const BoxView& b, int F, int ctas_per_sm, int halo_planes, int tx, int ty) {
+  return pick_chunks_impl(b, F, ctas_per_sm, halo_planes, tx, ty);
 }
 
 // which tile the stage kernels use on this box (0: 32 x 16, 1: 64 x 7): a function of the box and the device only, so
