@@ -44,6 +44,12 @@ template <int TX_, int TY_> struct Tile {
 };
 using TileA = Tile<32, 16>;
 using TileB = Tile<64, 7>;
+// Tile B's 224 compute threads leave room for a PRODUCER warp inside the 256-thread, 128-register budget of two CTAs per
+// SM: warp 7 does nothing but wait for a ring stage to be released (an mbarrier the 7 compute warps arrive on when they
+// have read it) and refill it by TMA. The compute warps then never meet in a CTA barrier: they drift up to NST - 1
+// planes apart inside a CTA while the CTAs of neighbouring columns stay together (the ring depth bounds the drift).
+template <class T> struct Spec { static constexpr bool WS = false; static constexpr int THREADS = T::NTHR; };
+template <> struct Spec<TileB> { static constexpr bool WS = true; static constexpr int THREADS = TileB::NTHR + 32; };
 constexpr int NST = 4;                       // planes in flight
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -141,10 +147,11 @@ __device__ __forceinline__ void scatter(double2 (&acc)[5], double2 centre_term, 
 }  // namespace
 
 template <int MODE, bool COUPLED, class T>
-__global__ void __launch_bounds__(T::NTHR, 2)
+__global__ void __launch_bounds__(Spec<T>::THREADS, 2)
     stage_zmarch(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ TmaStageParams p) {
   constexpr int NH = MODE == STAGE_12 ? 2 : 3;  // halo-read arrays per plane
   constexpr int TX = T::TX, TY = T::TY, HX = T::HX, TILE_DOUBLES = T::TILE_DOUBLES;
+  constexpr bool WS = Spec<T>::WS;
   pdl_enter();
   extern __shared__ unsigned char smraw[];
   // [NST][NH] tiles, 128-byte aligned for TMA, then NST mbarriers
@@ -174,14 +181,28 @@ __global__ void __launch_bounds__(T::NTHR, 2)
       tma_load_4d(s0 + (st * NH + h) * TILE_DOUBLES * 8, &tmap, XOFF + X0 - 2, b.g + Y0 - 2, b.g + zs + dir * it,
                   arr[h], bar);
   };
+  const uint32_t ebar0 = bar0 + 8 * NST;  // WS: the "stage released" barriers
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < NST; ++s) mbar_init(bar0 + 8 * s, 1);
+    for (int s = 0; s < NST; ++s) {
+      mbar_init(bar0 + 8 * s, 1);
+      if (WS) mbar_init(ebar0 + 8 * s, T::NTHR / 32);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    for (int it = 0; it < NST && it < narr; ++it) issue(it);
+    if (!WS)
+      for (int it = 0; it < NST && it < narr; ++it) issue(it);
   }
   __syncthreads();
+  if (WS && tid >= T::NTHR) {  // the producer warp: one lane feeds the ring for the whole march
+    if (tid == T::NTHR) {
+      for (int it = 0; it < narr; ++it) {
+        if (it >= NST) mbar_wait(ebar0 + 8 * (it % NST), ((it / NST) - 1) & 1);
+        issue(it);
+      }
+    }
+    return;
+  }
 
   const bool active = (X0 + 2 * tx < b.n[0]) && (Y0 + ty < b.n[1]);
   const long long cell0 = cell_offset(b, X0 + 2 * tx, Y0 + ty, 0);
@@ -278,8 +299,13 @@ __global__ void __launch_bounds__(T::NTHR, 2)
         if (p.write_Y4r) *reinterpret_cast<double2*>(p.Y4r + o) = a;
       }
     }
-    __syncthreads();  // every thread is done with stage st: refill it with the plane NST arrivals ahead
-    if (tid == 0 && it + NST < narr) issue(it + NST);
+    if (WS) {         // release stage st: the producer refills it once all compute warps have
+      __syncwarp();
+      if ((tid & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ebar0 + 8 * st) : "memory");
+    } else {
+      __syncthreads();  // every thread is done with stage st: refill it with the plane NST arrivals ahead
+      if (tid == 0 && it + NST < narr) issue(it + NST);
+    }
   };
 
   for (int it0 = 0; it0 < narr; it0 += 5) {
@@ -313,7 +339,7 @@ EncodeTiledFn encode_tiled() {
 }
 
 template <int MODE, class T>
-size_t stage_smem() { return (size_t)NST * (MODE == STAGE_12 ? 2 : 3) * T::TILE_DOUBLES * 8 + NST * 8 + 128; }
+size_t stage_smem() { return (size_t)NST * (MODE == STAGE_12 ? 2 : 3) * T::TILE_DOUBLES * 8 + 2 * NST * 8 + 128; }
 
 // z-chunks per column of tx x ty cells: enough CTAs to fill the machine in whole waves, as few halo planes as possible.
 // *cost_out: waves x (planes marched + pipeline fill), the launch's length in plane-steps of one CTA.
@@ -364,7 +390,7 @@ void launch_zmarch(const StageArgs& a, cudaStream_t st) {
   for (int d = 0; d < 3; ++d) p.w[d] = a.inv12dx2[d];
   p.S = a.S;
   dim3 grd((a.b.n[0] + T::TX - 1) / T::TX, (a.b.n[1] + T::TY - 1) / T::TY, p.nchunks * a.F);
-  launch_pdl(stage_zmarch<MODE, COUPLED, T>, grd, dim3(T::NTHR), stage_smem<MODE, T>(), st,
+  launch_pdl(stage_zmarch<MODE, COUPLED, T>, grd, dim3(Spec<T>::THREADS), stage_smem<MODE, T>(), st,
              *static_cast<const CUtensorMap*>(a.tmap), p);
 }
 template <int MODE, bool COUPLED>
