@@ -207,6 +207,34 @@ int32_t sc_debug_stream(sc_hierarchy* h, int32_t nread, int32_t nwrite, uint64_t
 int32_t sc_profile(sc_hierarchy* h, int32_t enable);
 int32_t sc_profile_read(sc_hierarchy* h, int32_t kind, uint64_t* launches, double* ms, double* bytes);
 
+/* The blow-up check of sc_debug_max_abs for callers that must not allocate device memory: max |x[i]| over a dense
+ * array, with the same NaN / inf rule (*out is NaN as soon as one value is NaN, else +inf if one is infinite).
+ *
+ * Why it exists: sc_debug_max_abs works on a hierarchy, and creating one calls cudaMalloc. That is no use to an
+ * application that gave all device memory to its own pool at start-up (any further cudaMalloc fails), nor to a time
+ * loop that must not take the device-wide synchronisation cudaMalloc / cudaFree imply just to look for a NaN. This
+ * call allocates nothing and frees nothing: its working memory (one partial maximum per 8192 inputs and a counter)
+ * is a fixed array compiled into the library, about 64 KB, present on every GPU that loads libsubcycle.so until the
+ * process exits.
+ *
+ *   x            DEVICE, n contiguous doubles, read only (any 8-byte aligned address; may be NULL if n == 0)
+ *   n            number of doubles, at most SC_NOALLOC_MAX_DOUBLES (2^26, 512 MB of input; a padded 256^3 box is
+ *                1.8e7). A larger n is refused with SC_ERR_INVALID_ARG and a message naming the limit: split the
+ *                input and take the maximum of the pieces. n == 0 gives 0.0.
+ *   out          DEVICE, one double, written by the kernel. The call is asynchronous and does not synchronise:
+ *                read *out after the stream has passed this point.
+ *   cuda_stream  a cudaStream_t (as void*) of the CURRENT device; NULL is the default stream. x and out must belong
+ *                to the current device.
+ *
+ * Set-up: the first call on each GPU looks up where that GPU keeps the built-in array (cudaGetSymbolAddress, with
+ * that GPU current) and remembers it. Make that first call during start-up, outside any stream capture.
+ * Shared state: all calls on one GPU use the same array, which still holds the last call's partials; each call clears
+ * what it needs at zero itself. Calls that can run on the GPU at the same time (different streams without an event
+ * between them) race on the array and return garbage: keep them on one stream or order them.
+ * Returns SC_OK, SC_ERR_INVALID_ARG (null pointer, n over the limit) or SC_ERR_CUDA. */
+#define SC_NOALLOC_MAX_DOUBLES (1ull << 26)
+int32_t sc_max_abs_noalloc(const double* x, uint64_t n, double* out, void* cuda_stream);
+
 /* Free everything the library owns (never the caller's arena). Synchronises the stream. */
 int32_t sc_destroy(sc_hierarchy* h);
 

@@ -19,7 +19,8 @@ SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NESTING, SC_ERR_UNSUPPORTED, SC_ERR_OOM, SC_ER
 
 EXPORTS = ["sc_arena_bytes", "sc_create_hierarchy", "sc_set_state", "sc_step", "sc_read_level", "sc_time",
            "sc_launch_count", "sc_debug_ghost_map", "sc_debug_read_padded", "sc_debug_read_slot", "sc_destroy",
-           "sc_last_error", "sc_profile", "sc_profile_read", "sc_debug_max_abs", "sc_debug_graph_stats", "sc_debug_stream"]
+           "sc_last_error", "sc_profile", "sc_profile_read", "sc_debug_max_abs", "sc_debug_graph_stats", "sc_debug_stream",
+           "sc_max_abs_noalloc"]
 
 
 class sc_box(C.Structure):
@@ -81,6 +82,8 @@ def lib():
         L.sc_debug_graph_stats.argtypes = [H] + [C.POINTER(C.c_uint64)] * 4
         L.sc_debug_stream.restype = C.c_int32
         L.sc_debug_stream.argtypes = [H, C.c_int32, C.c_int32, C.c_uint64, C.POINTER(C.c_double)]
+        L.sc_max_abs_noalloc.restype = C.c_int32
+        L.sc_max_abs_noalloc.argtypes = [dp, C.c_uint64, dp, C.c_void_p]
         L.sc_destroy.restype = C.c_int32
         L.sc_destroy.argtypes = [H]
         L.sc_profile.restype = C.c_int32
@@ -133,6 +136,24 @@ def sc_arena_bytes(desc: sc_hierarchy_desc) -> int:
     if n == 0:
         raise SubcycleError(SC_ERR_INVALID_ARG, lib().sc_last_error().decode())
     return int(n)
+
+
+SC_NOALLOC_MAX_DOUBLES = 1 << 26
+
+
+def sc_max_abs_noalloc(x, out, stream=None) -> None:
+    """max |x| of a contiguous fp64 CUDA tensor into the one-element fp64 CUDA tensor `out`, NaN / inf reported as by
+    Hierarchy.sc_debug_max_abs — but without a hierarchy and without any device allocation, for programs whose memory
+    pool already owns the whole GPU or whose time loop cannot take cudaMalloc's device-wide synchronisation
+    (include/subcycle.h). Asynchronous on `stream` (default: torch's current stream on x's device); at most
+    SC_NOALLOC_MAX_DOUBLES elements; calls that may overlap on one GPU race on the library's built-in scratch array."""
+    import torch
+
+    assert x.is_cuda and out.is_cuda and x.device == out.device
+    assert x.dtype == torch.float64 and out.dtype == torch.float64 and x.is_contiguous() and out.numel() == 1
+    with torch.cuda.device(x.device):
+        st = torch.cuda.current_stream() if stream is None else stream
+        _check(lib().sc_max_abs_noalloc(x.data_ptr(), x.numel(), out.data_ptr(), st.cuda_stream))
 
 
 class Hierarchy:

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libsubcycle.so")
-SOURCES = ["hierarchy.cpp", "kernels_basic.cu", "stage_tma.cu", "stage_gen.cu", "stage_ko_tma.cu", "stage_gen_tma.cu", "stage_fd8.cu", "ghost_tma.cu", "ghost_gen.cu", "restrict_zmarch.cu", "dispatch.cu", "capi.cu"]
+SOURCES = ["hierarchy.cpp", "kernels_basic.cu", "stage_tma.cu", "stage_gen.cu", "stage_ko_tma.cu", "stage_gen_tma.cu", "stage_fd8.cu", "ghost_tma.cu", "ghost_gen.cu", "restrict_zmarch.cu", "dispatch.cu", "capi.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-Wall,-Wextra", "-shared", "-x", "cu", "-rdc=false", "-cudart", "shared"]
 
