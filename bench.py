@@ -117,7 +117,7 @@ def time_oracle(w, steps: int, warmup: int, sub: bool, max_levels: int, threads:
     return {"value": upd / dt, "unit": UNIT, "cores": used, "kind": "oracle", "cpu": cpu_model(),
             "flags": "g++ -O2 -fopenmp, no fast-math",
             "sample": f"{what}, {steps} coarse step(s), {'subcycled' if sub else 'uniform'}, {dt:.1f} s",
-            "_seconds": dt, "_steps": steps}
+            "_seconds": dt, "_steps": steps, "_levels": s.nlevels, "_updates_per_step": s.updates_per_coarse_step(sub)}
 
 
 def config_dict(w, sub: bool, world: int):
@@ -138,10 +138,17 @@ def run_reference(args):
     sub = args.mode == "sub"
     r = time_oracle(w, max(1, args.steps), min(args.warmup, 1), sub, max_levels=args.oracle_levels)
     ms = 1e3 * r.pop("_seconds") / r.pop("_steps")
+    # The config is the GPU arm's (the contract), but what was TIMED is a sample of it: say so in the config itself, so
+    # that ms_per_step is never read as the time of the full workload (value is a rate and compares per update).
+    cfg = config_dict(w, sub, 1)
+    lev, upd = r.pop("_levels"), r.pop("_updates_per_step")
+    cfg.update({"sampled": lev < w.nlevels, "sample_levels": lev, "sample_updates_per_step": upd,
+                "ms_per_step_is": "one coarse step of the SAMPLE (sample_updates_per_step updates), not of the workload"
+                                  if lev < w.nlevels else "one coarse step of the workload"})
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(w, sub, 1),
+            "config": cfg,
             "note": "CPU oracle (as it stands, all host threads) on a bounded SAMPLE of the workload: " + r["sample"],
             "cpu_baseline": r,
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -363,6 +370,7 @@ def run_gpu(args):
     if world == 1 and not args.no_cpu_baseline:
         cpu = time_oracle(w, 1, 0, sub, max_levels=args.oracle_levels)
         cpu.pop("_seconds"), cpu.pop("_steps")
+        cpu["sample_levels"], cpu["sample_updates_per_step"] = cpu.pop("_levels"), cpu.pop("_updates_per_step")
         if not args.no_cpu_1thread:  # one thread and all threads
             one = time_oracle(w, 1, 0, sub, max_levels=args.oracle_levels, threads=1)
             cpu["value_1thread"] = one["value"]

@@ -53,3 +53,16 @@ def test_reference_arm_line():
     d = _line("--impl", "reference", "--config", "1", "--steps", "1", "--warmup", "0")
     assert d["impl"] == "reference" and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+    c = d["config"]  # cfg 1 has two levels: the oracle times all of it, and the config says so
+    assert c["sampled"] is False and c["sample_levels"] == 2 and c["sample_updates_per_step"] == c["updates_per_step"]
+
+
+def test_reference_arm_says_when_it_timed_a_sample():
+    """The reference arm prints the GPU arm's config, but on deep hierarchies it times the first levels only: the
+    config carries the sample (identical configs on different work must not pass silently)."""
+    d = _line("--impl", "reference", "--config", "1", "--steps", "1", "--warmup", "0", "--oracle-levels", "1")
+    c = d["config"]
+    assert c["sampled"] is True and c["sample_levels"] == 1 and 0 < c["sample_updates_per_step"] < c["updates_per_step"]
+    assert "SAMPLE" in c["ms_per_step_is"] and "SAMPLE" in d["cpu_baseline"]["sample"]
+    # value is the sample's rate: updates of the sample / time of the sample
+    assert abs(d["value"] * d["ms_per_step"] * 1e-3 / c["sample_updates_per_step"] - 1.0) < 1e-6
