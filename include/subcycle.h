@@ -78,7 +78,8 @@ typedef struct {
  * outer_bc: 0 -> periodic level 0 (S9); 1 -> radiative (Sommerfeld) boundary (reading S29): the
  *   cells of level 0 within `ghost` cells of a domain face are boundary points, every evolved variable obeys
  *   d_t y = -[(x^i/r) d_i y + y/r] there (second-order centred / one-sided differences), at every stage; the ghost
- *   cells of level 0 are then unused. The domain must contain the origin strictly inside.
+ *   cells of level 0 are then unused. The origin must lie inside the domain, more than ghost * dx_0 from every face
+ *   (the boundary zone evaluates 1/r; SC_ERR_INVALID_ARG otherwise).
  * interp_order: 0 -> quartic prolongation, quintic restriction (S3, S4); 1 -> 9-point prolongation and 10-point
  *   restriction, the orders that follow 8th-order differences (reading S30; needs ghost >= 4; nesting margin
  *   ceil(g/2) + 4 parent cells).
@@ -196,6 +197,16 @@ int32_t sc_debug_graph_stats(const sc_hierarchy* h, uint64_t* captures, uint64_t
  * (nread + nwrite) * 8 * ndoubles bytes / time. Context for the roofline fractions (which stay against the copy peak):
  * what a kernel that only moves the same bytes reaches. Synchronises the stream. 1 <= nread, nwrite <= 8. */
 int32_t sc_debug_stream(sc_hierarchy* h, int32_t nread, int32_t nwrite, uint64_t ndoubles, double* gbps);
+
+/* Debug, host only (no GPU needed): the one-dimensional interpolation operators the library uses between levels for
+ * the given options (readings S3, S4, S30, S31; 3-D operators are their tensor products). Prolongation: the fine point
+ * of parity p (0: at -1/4 parent spacing from parent point 0 on cell-centred grids, ON it on vertex-centred grids;
+ * 1: at +1/4, resp. +1/2) is sum_m w_p[m] * parent[pmin + m], m < np. Restriction: parent point I is
+ * sum_m r[m] * fine[2 I + rmin + m], m < nr. The library derives them in exact integer arithmetic and rounds once,
+ * so each is the correctly rounded value of its rational (tests/golden/interp_weights*.txt). All out pointers HOST;
+ * w0, w1, r hold 10 doubles each (entries beyond np / nr are 0). */
+int32_t sc_debug_interp_weights(int32_t interp_order, int32_t centering, int32_t* np, int32_t* pmin, double* w0,
+                                double* w1, int32_t* nr, int32_t* rmin, double* r);
 
 /* Per-kernel timing for the roofline report. sc_profile(h, 1): from now on sc_step launches its kernels
  * one by one (no graph replay) with a CUDA-event pair around each on the hierarchy's stream;

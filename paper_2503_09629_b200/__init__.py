@@ -5,4 +5,5 @@ package is its thin Python binding plus the seeded synthetic workloads. Nothing 
 """
 from . import workloads  # noqa: F401
 from .binding import (EXPORTS, Hierarchy, SubcycleError, lib, make_desc, sc_arena_bytes,  # noqa: F401
-                      sc_box, sc_hierarchy_desc, sc_max_abs_noalloc, SC_NOALLOC_MAX_DOUBLES)
+                      sc_box, sc_hierarchy_desc, sc_max_abs_noalloc, SC_NOALLOC_MAX_DOUBLES,
+                      sc_debug_interp_weights)

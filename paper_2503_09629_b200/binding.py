@@ -20,7 +20,7 @@ SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NESTING, SC_ERR_UNSUPPORTED, SC_ERR_OOM, SC_ER
 EXPORTS = ["sc_arena_bytes", "sc_create_hierarchy", "sc_set_state", "sc_step", "sc_read_level", "sc_time",
            "sc_launch_count", "sc_debug_ghost_map", "sc_debug_read_padded", "sc_debug_read_slot", "sc_destroy",
            "sc_last_error", "sc_profile", "sc_profile_read", "sc_debug_max_abs", "sc_debug_graph_stats", "sc_debug_stream",
-           "sc_max_abs_noalloc"]
+           "sc_max_abs_noalloc", "sc_debug_interp_weights"]
 
 
 class sc_box(C.Structure):
@@ -84,6 +84,9 @@ def lib():
         L.sc_debug_stream.argtypes = [H, C.c_int32, C.c_int32, C.c_uint64, C.POINTER(C.c_double)]
         L.sc_max_abs_noalloc.restype = C.c_int32
         L.sc_max_abs_noalloc.argtypes = [dp, C.c_uint64, dp, C.c_void_p]
+        L.sc_debug_interp_weights.restype = C.c_int32
+        L.sc_debug_interp_weights.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32), dp, dp,
+                                              C.POINTER(C.c_int32), C.POINTER(C.c_int32), dp]
         L.sc_destroy.restype = C.c_int32
         L.sc_destroy.argtypes = [H]
         L.sc_profile.restype = C.c_int32
@@ -154,6 +157,17 @@ def sc_max_abs_noalloc(x, out, stream=None) -> None:
     with torch.cuda.device(x.device):
         st = torch.cuda.current_stream() if stream is None else stream
         _check(lib().sc_max_abs_noalloc(x.data_ptr(), x.numel(), out.data_ptr(), st.cuda_stream))
+
+
+def sc_debug_interp_weights(interp: int = 0, vertex: int = 0) -> dict:
+    """The library's 1-D prolongation / restriction operators for these options (host only; include/subcycle.h)."""
+    n = [C.c_int32() for _ in range(4)]
+    w0, w1, r = (np.zeros(10) for _ in range(3))
+    _check(lib().sc_debug_interp_weights(int(interp), int(vertex), C.byref(n[0]), C.byref(n[1]), w0.ctypes.data,
+                                         w1.ctypes.data, C.byref(n[2]), C.byref(n[3]), r.ctypes.data))
+    npts, pmin, nr, rmin = (int(x.value) for x in n)
+    return {"np": npts, "pmin": pmin, "w": (w0[:npts].copy(), w1[:npts].copy()), "nr": nr, "rmin": rmin, "r": r[:nr].copy(),
+            "tail": np.concatenate([w0[npts:], w1[npts:], r[nr:]])}
 
 
 class Hierarchy:

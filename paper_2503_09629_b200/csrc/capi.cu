@@ -1174,6 +1174,19 @@ int32_t sc_debug_stream(sc_hierarchy* h, int32_t nread, int32_t nwrite, uint64_t
   return SC_OK;
 }
 
+int32_t sc_debug_interp_weights(int32_t interp_order, int32_t centering, int32_t* np, int32_t* pmin, double* w0,
+                                double* w1, int32_t* nr, int32_t* rmin, double* r) {
+  if ((interp_order != 0 && interp_order != 1) || (centering != 0 && centering != 1)) {
+    set_error("interp_order and centering must be 0 or 1");
+    return SC_ERR_UNSUPPORTED;
+  }
+  if (!np || !pmin || !w0 || !w1 || !nr || !rmin || !r) { set_error("null out pointer"); return SC_ERR_INVALID_ARG; }
+  const InterpOps P = make_interp_ops(interp_order, centering);
+  *np = P.np; *pmin = P.pmin; *nr = P.nr; *rmin = P.rmin;
+  for (int m = 0; m < 10; ++m) { w0[m] = P.w[0][m]; w1[m] = P.w[1][m]; r[m] = P.r[m]; }
+  return SC_OK;
+}
+
 int32_t sc_profile(sc_hierarchy* h, int32_t enable) {
   if (!h) { set_error("null hierarchy"); return SC_ERR_INVALID_ARG; }
   SC_CUDA(cudaStreamSynchronize(h->stream));

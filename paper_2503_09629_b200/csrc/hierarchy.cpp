@@ -22,40 +22,52 @@ static int fail(std::string* err, int code, const char* fmt, int a = 0, int b = 
   return code;
 }
 
-// Lagrange weights of the interpolant through `n` nodes evaluated at x (host, long double accumulation).
-static void lagrange(const double* nodes, int n, double x, double* w) {
-  for (int m = 0; m < n; ++m) {
-    long double v = 1.0L;
-    for (int q = 0; q < n; ++q)
-      if (q != m) v *= ((long double)x - nodes[q]) / ((long double)nodes[m] - nodes[q]);
-    w[m] = (double)v;
+// ------------------------------------------------------------------------------------------------
+// Interpolation operators (readings S3, S4, S30, S31) as EXACT rationals.
+// Every operator here interpolates through equally spaced nodes to a target that is a whole number of QUARTER node
+// spacings away from them, so in quarter-spacing units all positions are integers and each Lagrange weight
+//     w_q = prod_{j != q} (T - X_j) / prod_{j != q} (X_q - X_j)
+// is a ratio of two integers below 2^53 (at most ten nodes: |numerator| <= 9.1e8, |denominator| <= 4^9 9!). One IEEE
+// division of the two then gives the correctly rounded value of the rational; no floating-point product is formed.
+// ------------------------------------------------------------------------------------------------
+struct Stencil {
+  int count;  // number of nodes
+  int first;  // offset of node 0 in cells / grid points
+  int shift;  // node q sits at quarter-position 4 * (first + q) + shift  (shift -2: nodes at half-integer offsets)
+};
+
+static void exact_weights(const Stencil& st, int target, double* w) {
+  for (int q = 0; q < st.count; ++q) {
+    const long long xq = 4ll * (st.first + q) + st.shift;
+    long long num = 1, den = 1;
+    for (int j = 0; j < st.count; ++j) {
+      if (j == q) continue;
+      const long long xj = 4ll * (st.first + j) + st.shift;
+      num *= target - xj;
+      den *= xq - xj;
+    }
+    w[q] = num == 0 ? 0.0 : (double)num / (double)den;  // (no -0.0 where the target sits on another node)
   }
 }
 
 InterpOps make_interp_ops(int interp, int vertex) {
+  // rows: [centering][interp_order];  prolongation stencil over parent points, restriction stencil over fine points
+  static const Stencil PROLONG[2][2] = {{{5, -2, 0}, {9, -4, 0}}, {{6, -2, 0}, {10, -4, 0}}};
+  static const Stencil RESTRICT[2][2] = {{{6, -2, -2}, {10, -4, -2}}, {{1, 0, 0}, {1, 0, 0}}};
+  const Stencil& p = PROLONG[vertex ? 1 : 0][interp ? 1 : 0];
+  const Stencil& r = RESTRICT[vertex ? 1 : 0][interp ? 1 : 0];
   InterpOps P;
-  double nodes[10];
   for (int m = 0; m < 10; ++m) P.w[0][m] = P.w[1][m] = P.r[m] = 0.0;
-  if (!vertex) {  // cell-centred (S1): fine centres at -+1/4 of the parent spacing; parent centre midway between fine cells
-    P.np = interp ? 9 : 5;
-    P.pmin = -(P.np / 2);
-    for (int m = 0; m < P.np; ++m) nodes[m] = P.pmin + m;
-    lagrange(nodes, P.np, -0.25, P.w[0]);
-    lagrange(nodes, P.np, 0.25, P.w[1]);
-    P.nr = interp ? 10 : 6;
-    P.rmin = -(P.nr / 2 - 1);
-    for (int m = 0; m < P.nr; ++m) nodes[m] = (P.rmin + m) - 0.5;
-    lagrange(nodes, P.nr, 0.0, P.r);
-  } else {        // vertex-centred (S31): even fine points coincide with parent points, odd ones sit midway
-    P.np = interp ? 10 : 6;
-    P.pmin = -(P.np / 2 - 1);
-    for (int m = 0; m < P.np; ++m) nodes[m] = P.pmin + m;
-    P.w[0][-P.pmin] = 1.0;
-    lagrange(nodes, P.np, 0.5, P.w[1]);
-    P.nr = 1;
-    P.rmin = 0;
-    P.r[0] = 1.0;
-  }
+  P.np = p.count;
+  P.pmin = p.first;
+  P.nr = r.count;
+  P.rmin = r.first;
+  // fine point of parity 0 / 1 relative to parent point 0: cell-centred -1/4, +1/4 (S1); vertex-centred 0, +1/2 (S31)
+  exact_weights(p, vertex ? 0 : -1, P.w[0]);
+  exact_weights(p, vertex ? 2 : +1, P.w[1]);
+  // the parent point lies midway between fine cells 2I and 2I + 1 (cell-centred: fine cell 2I + j at j - 1/2), or on
+  // fine point 0 (vertex-centred: the one-node stencil is injection)
+  exact_weights(r, 0, P.r);
   return P;
 }
 
@@ -99,9 +111,17 @@ int build_layout(const sc_hierarchy_desc* d, Layout* L, std::string* err) {
   if ((d->interp_order != 0 && d->interp_order != 1) || (d->centering != 0 && d->centering != 1))
     return fail(err, SC_ERR_UNSUPPORTED, "interp_order and centering must be 0 or 1");
   if (d->outer_bc == 1)
-    for (int a = 0; a < 3; ++a)
+    for (int a = 0; a < 3; ++a) {
       if (!(d->xlo[a] < 0.0 && d->xhi[a] > 0.0))
         return fail(err, SC_ERR_INVALID_ARG, "radiative boundary: the origin must lie strictly inside the domain (axis %d)", a);
+      // the boundary operator divides by r = |x| at every point within `ghost` level-0 points of a face (S29): keep the
+      // origin out of that zone, so that no boundary point (cell- or vertex-centred) can sit at r = 0
+      const double zone = d->ghost * (d->xhi[a] - d->xlo[a]) / d->domain_cells[a];
+      if (!(-d->xlo[a] > zone && d->xhi[a] > zone))
+        return fail(err, SC_ERR_INVALID_ARG,
+                    "radiative boundary: the origin must lie more than ghost * dx0 = %g from both faces of axis %d "
+                    "(the boundary zone evaluates 1/r)", zone, a);
+    }
 
   L->nlevels = d->nlevels;
   L->fd_order = fd;

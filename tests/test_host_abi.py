@@ -106,6 +106,10 @@ def test_nesting_validator_rejects_bad_hierarchies(built):
     assert rc(base, integrator=3)[0] != SC_ERR_UNSUPPORTED and rc(base, integrator=2)[0] != SC_ERR_UNSUPPORTED
     assert rc(base, outer_bc=2)[0] == SC_ERR_UNSUPPORTED
     assert rc(base, outer_bc=1, xlo=(0.5, -1.0, -1.0), xhi=(2.0, 1.0, 1.0))[0] == SC_ERR_INVALID_ARG  # origin outside
+    # ... or inside the boundary zone of `ghost` points at a face, where the operator evaluates 1/r (dx0 = 3/32, g = 3)
+    r_, msg_ = rc(base, outer_bc=1, xlo=(-0.25, -1.0, -1.0), xhi=(2.75, 1.0, 1.0))
+    assert r_ == SC_ERR_INVALID_ARG and "1/r" in msg_
+    assert rc(base, outer_bc=1, xlo=(-0.3, -1.0, -1.0), xhi=(2.7, 1.0, 1.0))[0] != SC_ERR_INVALID_ARG
     assert rc(base, ko_order=7)[0] == SC_ERR_UNSUPPORTED
     assert rc(base, interp=1)[0] == SC_ERR_UNSUPPORTED              # the 10-point restriction reads 4 ghost layers
     assert rc(base, interp=1, ghost=4)[0] != SC_ERR_UNSUPPORTED
@@ -143,3 +147,51 @@ def test_dissipation_in_the_description(built):
     d, keep = sc.make_desc(w.boxes, w.domain_cells, ghost=2, ko_sigma=0.1)   # Q reads 3 ghost layers
     assert sc.lib().sc_arena_bytes(d) == 0
     assert b"ghost" in sc.lib().sc_last_error()
+
+
+def _golden_rationals():
+    from fractions import Fraction
+    rows = {}
+    for name in ("interp_weights.txt", "interp_weights_next.txt"):
+        for line in open(os.path.join(ROOT, "tests", "golden", name)):
+            if line.strip() and not line.startswith("#"):
+                t = line.split()
+                rows[t[0]] = [Fraction(x) for x in t[1:]]
+    return rows
+
+
+def test_product_interpolation_weights_are_the_correctly_rounded_rationals(built):
+    """The LIBRARY's own prolongation / restriction operators (sc_debug_interp_weights; csrc/hierarchy.cpp derives them
+    in exact integer arithmetic) against the rational tables under tests/golden/ — the 5-/6-point rows are SURVEY 8(c)'s,
+    the 6-/9-/10-point rows come from make_interp_rationals.py (python fractions; neither oracle nor library) — and the
+    tables themselves against what defines them: exactness on monomials up to degree np - 1 at the geometric position of
+    the target, and NOT one degree more. float(Fraction) is correctly rounded, and so must the library's value be: ==."""
+    from fractions import Fraction as Fr
+    g = _golden_rationals()
+    cases = {  # (interp, vertex) -> (prolong parity-1 row, its target, restriction row)
+        (0, 0): ("prolong1", Fr(1, 4), "restrict"), (1, 0): ("prolong9_p1", Fr(1, 4), "restrict10"),
+        (0, 1): ("vertex6_mid", Fr(1, 2), None), (1, 1): ("vertex10_mid", Fr(1, 2), None)}
+    for (interp, vertex), (prow, x, rrow) in cases.items():
+        P = sc.sc_debug_interp_weights(interp, vertex)
+        assert not P["tail"].any()
+        w1 = g[prow]
+        assert P["np"] == len(w1) and [float(v) for v in w1] == list(P["w"][1])
+        nodes = [Fr(P["pmin"] + m) for m in range(P["np"])]
+        for k in range(P["np"] + 1):  # the rationals are the interpolation weights at x: exact to degree np - 1 only
+            assert (sum(w * xm ** k for w, xm in zip(w1, nodes)) == x ** k) == (k < P["np"])
+        if vertex:      # fine point 2J sits on parent point J: copy; restriction is injection
+            assert list(P["w"][0]) == [1.0 if P["pmin"] + m == 0 else 0.0 for m in range(P["np"])]
+            assert P["nr"] == 1 and P["rmin"] == 0 and list(P["r"]) == [1.0]
+            assert P["pmin"] == -(P["np"] // 2 - 1)
+        else:           # parity 0 is the mirror image about parent cell 0
+            assert list(P["w"][0]) == list(P["w"][1])[::-1] and P["pmin"] == -(P["np"] // 2)
+            r = g[rrow]
+            assert P["nr"] == len(r) and [float(v) for v in r] == list(P["r"])
+            fine = [Fr(2 * (P["rmin"] + m) - 1, 2) for m in range(P["nr"])]  # centre of fine cell 2I + j: j - 1/2 from the parent centre
+            assert fine[0] == -fine[-1]
+            for k in range(P["nr"] + 1):
+                # symmetric stencil: odd monomials vanish identically, so "one degree more" is tested on even k only
+                ok = sum(w * xm ** k for w, xm in zip(r, fine)) == (1 if k == 0 else 0)
+                assert ok == (k < P["nr"] or k % 2 == 1)
+    L = sc.lib()
+    assert L.sc_debug_interp_weights(2, 0, None, None, None, None, None, None, None) == sc.binding.SC_ERR_UNSUPPORTED
