@@ -50,6 +50,18 @@
 
 namespace {
 
+// The arithmetic type of everything below. The oracle is fp64 as shipped (`real` = double; the C interface at the end
+// of the file is double in and out in every build). Compiling the SAME source with -DORACLE_LONG_DOUBLE (x86 long
+// double: 64-bit mantissa, 11 more bits than fp64) gives the reference of higher precision that tests use to measure
+// how far an fp64 evaluation of this definition lies from its exact-arithmetic value at a given depth (S27):
+// state, slopes, weights and every accumulator are then long double. Constants are written so that they are exact in
+// either type (2/3 as real(2)/real(3), never as the quotient of two double literals).
+#ifdef ORACLE_LONG_DOUBLE
+using real = long double;
+#else
+using real = double;
+#endif
+
 constexpr int kStencilRadius = 2;
 
 // ---------------------------------------------------------------------------------------------
@@ -57,21 +69,21 @@ constexpr int kStencilRadius = 2;
 // ---------------------------------------------------------------------------------------------
 
 // m-th theta-derivative (m = 0..3) of b_i(theta), i = 1..4; eqs (11)-(13).
-double b_coeff(int i, int m, double th) {
+real b_coeff(int i, int m, real th) {
   switch (i) {
     case 1:  // b1 = th - 3/2 th^2 + 2/3 th^3
-      if (m == 0) return th - 1.5 * th * th + (2.0 / 3.0) * th * th * th;
+      if (m == 0) return th - 1.5 * th * th + (real(2) / real(3)) * th * th * th;
       if (m == 1) return 1.0 - 3.0 * th + 2.0 * th * th;
       if (m == 2) return -3.0 + 4.0 * th;
       return 4.0;
     case 2:
     case 3:  // b2 = b3 = th^2 - 2/3 th^3
-      if (m == 0) return th * th - (2.0 / 3.0) * th * th * th;
+      if (m == 0) return th * th - (real(2) / real(3)) * th * th * th;
       if (m == 1) return 2.0 * th - 2.0 * th * th;
       if (m == 2) return 2.0 - 4.0 * th;
       return -4.0;
     default:  // b4 = -1/2 th^2 + 2/3 th^3
-      if (m == 0) return -0.5 * th * th + (2.0 / 3.0) * th * th * th;
+      if (m == 0) return -0.5 * th * th + (real(2) / real(3)) * th * th * th;
       if (m == 1) return -th + 2.0 * th * th;
       if (m == 2) return -1.0 + 4.0 * th;
       return 4.0;
@@ -84,9 +96,9 @@ double b_coeff(int i, int m, double th) {
 //   stage 1..4: Y_1..Y_4 by eqs (15)-(18) with y, y', y'', y''' from eqs (10),(14) at theta, and
 //               f_y y'' = 4 (k3 - k2) / hp^2 (reading S5: the parent's step);
 //   stage 5:    y at "theta" by eq (10) alone (the caller passes theta + 1/2).
-double dense_stage(int stage, double theta, double hp, double y_old, const double k[4]) {
-  double y = y_old, d1 = 0.0, d2 = 0.0, d3 = 0.0;
-  double s0 = 0.0;
+real dense_stage(int stage, real theta, real hp, real y_old, const real k[4]) {
+  real y = y_old, d1 = 0.0, d2 = 0.0, d3 = 0.0;
+  real s0 = 0.0;
   for (int i = 1; i <= 4; ++i) {
     s0 += b_coeff(i, 0, theta) * k[i - 1];
     d1 += b_coeff(i, 1, theta) * k[i - 1];
@@ -97,8 +109,8 @@ double dense_stage(int stage, double theta, double hp, double y_old, const doubl
   d2 = d2 / hp;         // eq (14), m = 2
   d3 = d3 / (hp * hp);  // eq (14), m = 3
   if (stage == 1 || stage == 5) return y;  // eq (15) / eq (10)
-  const double h = 0.5 * hp;               // child step
-  const double fyy = 4.0 * (k[2] - k[1]) / (hp * hp);
+  const real h = 0.5 * hp;               // child step
+  const real fyy = 4.0 * (k[2] - k[1]) / (hp * hp);
   if (stage == 2) return y + 0.5 * h * d1;                                      // eq (16)
   if (stage == 3) return y + 0.5 * h * d1 + 0.25 * h * h * d2 + (h * h * h / 16.0) * (d3 - fyy);  // (17)
   return y + h * d1 + 0.5 * h * h * d2 + (h * h * h / 8.0) * (d3 + fyy);        // eq (18)
@@ -127,20 +139,20 @@ double dense_stage(int stage, double theta, double hp, double y_old, const doubl
 //          k3 - k4 = f(y + hp D1 + hp^2 D2 + ..) - f(y + hp D1 + hp^2/2 D2 + ..) = hp^2/2 f_y D2 + O(hp^3))
 //   RK2:  Y1 = y,  Y2 = y + h/2 D1
 // ---------------------------------------------------------------------------------------------
-double b_coeff_rk3(int i, int m, double th) {
+real b_coeff_rk3(int i, int m, real th) {
   switch (i) {
     case 1:
-      if (m == 0) return th - 1.5 * th * th + (2.0 / 3.0) * th * th * th;
+      if (m == 0) return th - 1.5 * th * th + (real(2) / real(3)) * th * th * th;
       if (m == 1) return 1.0 - 3.0 * th + 2.0 * th * th;
       if (m == 2) return -3.0 + 4.0 * th;
       return 4.0;
     case 2:
-      if (m == 0) return 2.0 * th * th - (4.0 / 3.0) * th * th * th;
+      if (m == 0) return 2.0 * th * th - (real(4) / real(3)) * th * th * th;
       if (m == 1) return 4.0 * th - 4.0 * th * th;
       if (m == 2) return 4.0 - 8.0 * th;
       return -8.0;
     case 3:
-      if (m == 0) return 0.5 * th * th - (1.0 / 3.0) * th * th * th;
+      if (m == 0) return 0.5 * th * th - (real(1) / real(3)) * th * th * th;
       if (m == 1) return th - th * th;
       if (m == 2) return 1.0 - 2.0 * th;
       return -2.0;
@@ -151,40 +163,40 @@ double b_coeff_rk3(int i, int m, double th) {
       return 6.0;
   }
 }
-double b_coeff_rk2(int i, int m, double th) {
+real b_coeff_rk2(int i, int m, real th) {
   if (i == 1) return m == 0 ? th - th * th : (m == 1 ? 1.0 - 2.0 * th : (m == 2 ? -2.0 : 0.0));
   return m == 0 ? th * th : (m == 1 ? 2.0 * th : (m == 2 ? 2.0 : 0.0));
 }
 // stage = 1..3 (RK3) / 1..2 (RK2): the ghost value of Y_stage; stage 5: y at `theta` by the dense output alone.
 // RK3: k[0..2] = k1..k3 of the parent's step, k[3] = k4 = f(y_{n+1}).
-double dense_stage_rk3(int stage, double theta, double hp, double y_old, const double k[4]) {
-  double s0 = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0;
+real dense_stage_rk3(int stage, real theta, real hp, real y_old, const real k[4]) {
+  real s0 = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0;
   for (int i = 1; i <= 4; ++i) {
     s0 += b_coeff_rk3(i, 0, theta) * k[i - 1];
     d1 += b_coeff_rk3(i, 1, theta) * k[i - 1];
     d2 += b_coeff_rk3(i, 2, theta) * k[i - 1];
     d3 += b_coeff_rk3(i, 3, theta) * k[i - 1];
   }
-  const double y = y_old + hp * s0;  // the analogue of eq (10)
+  const real y = y_old + hp * s0;  // the analogue of eq (10)
   d2 = d2 / hp;                      // eq (14), m = 2
   d3 = d3 / (hp * hp);               // eq (14), m = 3
   if (stage == 1 || stage == 5) return y;
-  const double h = 0.5 * hp;  // child step
+  const real h = 0.5 * hp;  // child step
   if (stage == 2) return y + 0.5 * h * d1;
-  const double fyy = 2.0 * (k[2] - k[3]) / (hp * hp);
+  const real fyy = 2.0 * (k[2] - k[3]) / (hp * hp);
   return y + h * d1 + h * h * d2 + (h * h * h / 4.0) * (d3 - fyy);
 }
-double dense_stage_rk2(int stage, double theta, double hp, double y_old, const double k[2]) {
-  double s0 = 0.0, d1 = 0.0;
+real dense_stage_rk2(int stage, real theta, real hp, real y_old, const real k[2]) {
+  real s0 = 0.0, d1 = 0.0;
   for (int i = 1; i <= 2; ++i) {
     s0 += b_coeff_rk2(i, 0, theta) * k[i - 1];
     d1 += b_coeff_rk2(i, 1, theta) * k[i - 1];
   }
-  const double y = y_old + hp * s0;
+  const real y = y_old + hp * s0;
   if (stage == 1 || stage == 5) return y;
   return y + 0.5 * (0.5 * hp) * d1;
 }
-double dense_stage_any(int integrator, int stage, double theta, double hp, double y_old, const double* k) {
+real dense_stage_any(int integrator, int stage, real theta, real hp, real y_old, const real* k) {
   if (integrator == 3) return dense_stage_rk3(stage, theta, hp, y_old, k);
   if (integrator == 2) return dense_stage_rk2(stage, theta, hp, y_old, k);
   return dense_stage(stage, theta, hp, y_old, k);
@@ -195,9 +207,9 @@ double dense_stage_any(int integrator, int stage, double theta, double hp, doubl
 // ---------------------------------------------------------------------------------------------
 
 // Lagrange basis weights: value at x of the polynomial through (nodes[m], f_m) = sum_m w[m] f_m.
-void lagrange_weights(const double* nodes, int n, double x, double* w) {
+void lagrange_weights(const real* nodes, int n, real x, real* w) {
   for (int m = 0; m < n; ++m) {
-    double v = 1.0;
+    real v = 1.0;
     for (int q = 0; q < n; ++q)
       if (q != m) v *= (x - nodes[q]) / (nodes[m] - nodes[q]);
     w[m] = v;
@@ -206,15 +218,15 @@ void lagrange_weights(const double* nodes, int n, double x, double* w) {
 
 // Prolongation (S3): quartic through the 5 parent cells J-2..J+2 (centres at offsets -2..2 in units of
 // the parent spacing) evaluated at the fine centre: -1/4 (parity 0) or +1/4 (parity 1).
-void prolong_weights(int parity, double w[5]) {
-  const double nodes[5] = {-2.0, -1.0, 0.0, 1.0, 2.0};
+void prolong_weights(int parity, real w[5]) {
+  const real nodes[5] = {-2.0, -1.0, 0.0, 1.0, 2.0};
   lagrange_weights(nodes, 5, parity ? 0.25 : -0.25, w);
 }
 
 // Restriction (S4): quintic through the 6 fine cells 2J-2..2J+3, whose centres sit at -2.5..+2.5 fine
 // spacings from the parent centre, evaluated at the parent centre.
-void restrict_weights(double r[6]) {
-  const double nodes[6] = {-2.5, -1.5, -0.5, 0.5, 1.5, 2.5};
+void restrict_weights(real r[6]) {
+  const real nodes[6] = {-2.5, -1.5, -0.5, 0.5, 1.5, 2.5};
   lagrange_weights(nodes, 6, 0.0, r);
 }
 
@@ -226,29 +238,29 @@ void restrict_weights(double r[6]) {
 // (interp 0, sextic-accurate) or J-4..J+5 (interp 1). All weights from the Lagrange formula.
 struct Interp {
   int np = 5, omin = -2;   // prolongation: parent offsets omin .. omin + np - 1 around J = floor(I / 2)
-  double w[2][10];         // [parity of the fine index][offset - omin]
+  real w[2][10];         // [parity of the fine index][offset - omin]
   int nr = 6, rmin = -2;   // restriction: fine offsets rmin .. rmin + nr - 1 around 2J
-  double r[10];
+  real r[10];
   int reach() const { return std::max(-omin, omin + np - 1); }  // parent cells the footprint extends beyond J
 };
 Interp make_interp(int interp, int vertex) {
   Interp P;
-  double nodes[10];
+  real nodes[10];
   if (!vertex) {
     P.np = interp ? 9 : 5;
     P.omin = -(P.np / 2);
-    for (int m = 0; m < P.np; ++m) nodes[m] = double(P.omin + m);
+    for (int m = 0; m < P.np; ++m) nodes[m] = real(P.omin + m);
     lagrange_weights(nodes, P.np, -0.25, P.w[0]);
     lagrange_weights(nodes, P.np, +0.25, P.w[1]);
     P.nr = interp ? 10 : 6;
     P.rmin = -(P.nr / 2 - 1);
     // fine cell 2J + q has its centre at (q - 1/2) fine spacings from the parent centre J
-    for (int m = 0; m < P.nr; ++m) nodes[m] = double(P.rmin + m) - 0.5;
+    for (int m = 0; m < P.nr; ++m) nodes[m] = real(P.rmin + m) - 0.5;
     lagrange_weights(nodes, P.nr, 0.0, P.r);
   } else {
     P.np = interp ? 10 : 6;
     P.omin = -(P.np / 2 - 1);
-    for (int m = 0; m < P.np; ++m) { nodes[m] = double(P.omin + m); P.w[0][m] = (P.omin + m == 0) ? 1.0 : 0.0; }
+    for (int m = 0; m < P.np; ++m) { nodes[m] = real(P.omin + m); P.w[0][m] = (P.omin + m == 0) ? 1.0 : 0.0; }
     lagrange_weights(nodes, P.np, 0.5, P.w[1]);
     P.nr = 1;
     P.rmin = 0;
@@ -265,7 +277,7 @@ inline int pos_mod(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
 // ---------------------------------------------------------------------------------------------
 struct Field {  // one padded array of one box: index (i,j,k) in [-g, n+g)
   int n[3] = {0, 0, 0}, g = 0;
-  std::vector<double> v;
+  std::vector<real> v;
   void init(const int nn[3], int gg) {
     for (int a = 0; a < 3; ++a) n[a] = nn[a];
     g = gg;
@@ -274,8 +286,8 @@ struct Field {  // one padded array of one box: index (i,j,k) in [-g, n+g)
   inline size_t idx(int i, int j, int k) const {
     return size_t(i + g) + size_t(n[0] + 2 * g) * (size_t(j + g) + size_t(n[1] + 2 * g) * size_t(k + g));
   }
-  inline double& at(int i, int j, int k) { return v[idx(i, j, k)]; }
-  inline double at(int i, int j, int k) const { return v[idx(i, j, k)]; }
+  inline real& at(int i, int j, int k) { return v[idx(i, j, k)]; }
+  inline real at(int i, int j, int k) const { return v[idx(i, j, k)]; }
 };
 
 struct BoxData {
@@ -288,9 +300,9 @@ struct BoxData {
 struct Hier {
   int nlevels = 0, g = 3, F = 1;
   int domain[3] = {0, 0, 0};
-  double xlo[3], xhi[3];
-  std::vector<double> A;  // F*F coupling or empty
-  double sigma = 0.0;     // Kreiss-Oliger dissipation strength (eqs 35-36); 0 = none
+  real xlo[3], xhi[3];
+  std::vector<real> A;  // F*F coupling or empty
+  real sigma = 0.0;     // Kreiss-Oliger dissipation strength (eqs 35-36); 0 = none
   int fd_order = 4;       // order of the centred finite differences of the RHS: 4 (S2) or 8 (NEXT-3)
   int ko_order = 5;       // 5: delta^6 (eq 36 with r = 4); 9: delta^10 (eq 36 with r = 8, "ninth-order")
   int integrator = 4;     // 4: RK4 (eqs 1-9); 3: Kutta's RK3; 2: midpoint RK2
@@ -299,8 +311,8 @@ struct Hier {
   Interp P = make_interp(0, 0);
   std::vector<BoxData> boxes;
   std::vector<std::vector<int>> level_boxes;
-  double time = 0.0;
-  double dx(int level, int a) const { return (xhi[a] - xlo[a]) / (double(domain[a]) * double(1 << level)); }
+  real time = 0.0;
+  real dx(int level, int a) const { return (xhi[a] - xlo[a]) / (real(domain[a]) * real(1 << level)); }
 };
 
 inline bool is_interior(const BoxData& b, int i, int j, int k) {
@@ -319,8 +331,8 @@ void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& 
   if (H.ko_order == 9) {
     // eq (36) with r = 8 ("ninth-order KO dissipation"): (-1)^4 sigma / 2^10 sum_i h_i^9 (D+ D-)^5 y
     //   = sigma / 1024 sum_i delta_i^10 y / h_i,  delta^10 = (1, -10, 45, -120, 210, -252, 210, -120, 45, -10, 1). 5 ghost layers.
-    static const double d10[11] = {1.0, -10.0, 45.0, -120.0, 210.0, -252.0, 210.0, -120.0, 45.0, -10.0, 1.0};
-    double c[3];
+    static const real d10[11] = {1.0, -10.0, 45.0, -120.0, 210.0, -252.0, 210.0, -120.0, 45.0, -10.0, 1.0};
+    real c[3];
     for (int a = 0; a < 3; ++a) c[a] = H.sigma / (1024.0 * H.dx(b.level, a));
     for (int v = 0; v < V; ++v) {
       const Field& y = Y[v];
@@ -329,7 +341,7 @@ void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& 
       for (int k = 0; k < b.n[2]; ++k)
         for (int j = 0; j < b.n[1]; ++j)
           for (int i = 0; i < b.n[0]; ++i) {
-            double sx = 0.0, sy = 0.0, sz = 0.0;
+            real sx = 0.0, sy = 0.0, sz = 0.0;
             for (int m = -5; m <= 5; ++m) {
               sx += d10[m + 5] * y.at(i + m, j, k);
               sy += d10[m + 5] * y.at(i, j + m, k);
@@ -340,7 +352,7 @@ void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& 
     }
     return;
   }
-  double c[3];
+  real c[3];
   for (int a = 0; a < 3; ++a) c[a] = H.sigma / (64.0 * H.dx(b.level, a));
   for (int v = 0; v < V; ++v) {
     const Field& y = Y[v];
@@ -349,11 +361,11 @@ void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& 
     for (int k = 0; k < b.n[2]; ++k)
       for (int j = 0; j < b.n[1]; ++j)
         for (int i = 0; i < b.n[0]; ++i) {
-          const double d6x = y.at(i - 3, j, k) - 6.0 * y.at(i - 2, j, k) + 15.0 * y.at(i - 1, j, k) - 20.0 * y.at(i, j, k) +
+          const real d6x = y.at(i - 3, j, k) - 6.0 * y.at(i - 2, j, k) + 15.0 * y.at(i - 1, j, k) - 20.0 * y.at(i, j, k) +
                              15.0 * y.at(i + 1, j, k) - 6.0 * y.at(i + 2, j, k) + y.at(i + 3, j, k);
-          const double d6y = y.at(i, j - 3, k) - 6.0 * y.at(i, j - 2, k) + 15.0 * y.at(i, j - 1, k) - 20.0 * y.at(i, j, k) +
+          const real d6y = y.at(i, j - 3, k) - 6.0 * y.at(i, j - 2, k) + 15.0 * y.at(i, j - 1, k) - 20.0 * y.at(i, j, k) +
                              15.0 * y.at(i, j + 1, k) - 6.0 * y.at(i, j + 2, k) + y.at(i, j + 3, k);
-          const double d6z = y.at(i, j, k - 3) - 6.0 * y.at(i, j, k - 2) + 15.0 * y.at(i, j, k - 1) - 20.0 * y.at(i, j, k) +
+          const real d6z = y.at(i, j, k - 3) - 6.0 * y.at(i, j, k - 2) + 15.0 * y.at(i, j, k - 1) - 20.0 * y.at(i, j, k) +
                              15.0 * y.at(i, j, k + 1) - 6.0 * y.at(i, j, k + 2) + y.at(i, j, k + 3);
           kv.at(i, j, k) += c[0] * d6x + c[1] * d6y + c[2] * d6z;
         }
@@ -372,9 +384,9 @@ void add_dissipation(const Hier& H, const BoxData& b, const std::vector<Field>& 
 // ---------------------------------------------------------------------------------------------
 void radiative_rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vector<Field>& kout) {
   const int V = 2 * H.F, nb = H.g;
-  double dx[3];
+  real dx[3];
   for (int a = 0; a < 3; ++a) dx[a] = H.dx(b.level, a);
-  const double shift = H.vertex ? 0.0 : 0.5;
+  const real shift = H.vertex ? 0.0 : 0.5;
   for (int v = 0; v < V; ++v) {
     const Field& y = Y[v];
     Field& kv = kout[v];
@@ -387,9 +399,9 @@ void radiative_rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y,
           for (int a = 0; a < 3; ++a)
             if (idx[a] < nb || idx[a] >= b.n[a] - nb) zone = true;
           if (!zone) continue;
-          double x[3], d[3];
+          real x[3], d[3];
           for (int a = 0; a < 3; ++a) {
-            x[a] = H.xlo[a] + (double(b.lo[a] + idx[a]) + shift) * dx[a];
+            x[a] = H.xlo[a] + (real(b.lo[a] + idx[a]) + shift) * dx[a];
             int e[3] = {0, 0, 0};
             e[a] = 1;
             auto Yat = [&](int m) { return y.at(i + m * e[0], j + m * e[1], k + m * e[2]); };
@@ -397,7 +409,7 @@ void radiative_rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y,
             else if (idx[a] == b.n[a] - 1) d[a] = (3.0 * Yat(0) - 4.0 * Yat(-1) + Yat(-2)) / (2.0 * dx[a]);
             else d[a] = (Yat(1) - Yat(-1)) / (2.0 * dx[a]);
           }
-          const double r = std::sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+          const real r = std::sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
           kv.at(i, j, k) = -((x[0] * d[0] + x[1] * d[1] + x[2] * d[2]) / r + y.at(i, j, k) / r);
         }
   }
@@ -409,9 +421,9 @@ void radiative_rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y,
 // ---------------------------------------------------------------------------------------------
 void rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vector<Field>& kout) {
   const int F = H.F;
-  double inv12dx2[3];
+  real inv12dx2[3];
   for (int a = 0; a < 3; ++a) {
-    const double d = H.dx(b.level, a);
+    const real d = H.dx(b.level, a);
     inv12dx2[a] = 1.0 / (12.0 * d * d);
   }
   for (int f = 0; f < F; ++f) {
@@ -423,29 +435,29 @@ void rhs(const Hier& H, const BoxData& b, const std::vector<Field>& Y, std::vect
     for (int k = 0; k < b.n[2]; ++k)
       for (int j = 0; j < b.n[1]; ++j)
         for (int i = 0; i < b.n[0]; ++i) {
-          const double dxx = (-u.at(i - 2, j, k) + 16.0 * u.at(i - 1, j, k) - 30.0 * u.at(i, j, k) +
+          const real dxx = (-u.at(i - 2, j, k) + 16.0 * u.at(i - 1, j, k) - 30.0 * u.at(i, j, k) +
                               16.0 * u.at(i + 1, j, k) - u.at(i + 2, j, k)) * inv12dx2[0];
-          const double dyy = (-u.at(i, j - 2, k) + 16.0 * u.at(i, j - 1, k) - 30.0 * u.at(i, j, k) +
+          const real dyy = (-u.at(i, j - 2, k) + 16.0 * u.at(i, j - 1, k) - 30.0 * u.at(i, j, k) +
                               16.0 * u.at(i, j + 1, k) - u.at(i, j + 2, k)) * inv12dx2[1];
-          const double dzz = (-u.at(i, j, k - 2) + 16.0 * u.at(i, j, k - 1) - 30.0 * u.at(i, j, k) +
+          const real dzz = (-u.at(i, j, k - 2) + 16.0 * u.at(i, j, k - 1) - 30.0 * u.at(i, j, k) +
                               16.0 * u.at(i, j, k + 1) - u.at(i, j, k + 2)) * inv12dx2[2];
           if (H.fd_order == 8) {  // the paper's BBH discretisation: 8th-order centred, 9 points per axis
-            static const double c8[9] = {-1.0 / 560.0, 8.0 / 315.0, -1.0 / 5.0, 8.0 / 5.0, -205.0 / 72.0,
-                                         8.0 / 5.0,    -1.0 / 5.0,  8.0 / 315.0, -1.0 / 560.0};
-            double sx = 0.0, sy = 0.0, sz = 0.0;
+            static const real c8[9] = {real(-1) / real(560), real(8) / real(315), real(-1) / real(5), real(8) / real(5), real(-205) / real(72),
+                                       real(8) / real(5),    real(-1) / real(5),  real(8) / real(315), real(-1) / real(560)};
+            real sx = 0.0, sy = 0.0, sz = 0.0;
             for (int m = -4; m <= 4; ++m) {
               sx += c8[m + 4] * u.at(i + m, j, k);
               sy += c8[m + 4] * u.at(i, j + m, k);
               sz += c8[m + 4] * u.at(i, j, k + m);
             }
-            double src8 = 0.0;
+            real src8 = 0.0;
             if (!H.A.empty())
               for (int q = 0; q < F; ++q) src8 += H.A[size_t(f) * F + q] * Y[q].at(i, j, k);
             ku.at(i, j, k) = rho.at(i, j, k);
             kr.at(i, j, k) = sx * 12.0 * inv12dx2[0] + sy * 12.0 * inv12dx2[1] + sz * 12.0 * inv12dx2[2] + src8;
             continue;
           }
-          double src = 0.0;
+          real src = 0.0;
           if (!H.A.empty())
             for (int q = 0; q < F; ++q) src += H.A[size_t(f) * F + q] * Y[q].at(i, j, k);
           ku.at(i, j, k) = rho.at(i, j, k);
@@ -491,11 +503,11 @@ void prolong_into_ghosts(const Hier& H, const BoxData& child, const BoxData& par
           p[a] = I[a] - 2 * Jg;             // 0: fine centre at -dx_p/4, 1: at +dx_p/4 (vertex grids: 0 = on the parent point)
           J[a] = Jg - par.lo[a];            // parent-box-local
         }
-        double sz = 0.0;
+        real sz = 0.0;
         for (int c = 0; c < P.np; ++c) {
-          double sy = 0.0;
+          real sy = 0.0;
           for (int bb = 0; bb < P.np; ++bb) {
-            double sx = 0.0;
+            real sx = 0.0;
             for (int a = 0; a < P.np; ++a) sx += P.w[p[0]][a] * C.at(J[0] + P.omin + a, J[1] + P.omin + bb, J[2] + P.omin + c);
             sy += P.w[p[1]][bb] * sx;
           }
@@ -508,7 +520,7 @@ void prolong_into_ghosts(const Hier& H, const BoxData& child, const BoxData& par
 // fill(l, stage, theta) for a level >= 1 box in SUBCYCLED mode: evaluate the
 // parent's dense output at every parent cell (combine), then prolong once into the child's ghosts.
 void dense_ghost_fill(const Hier& H, const BoxData& child, const BoxData& par, std::vector<Field>& dst,
-                      int stage, double theta, double hp) {
+                      int stage, real theta, real hp) {
   Field C;
   C.init(par.n, H.g);
   // parent cells any ghost cell of the child can reach: ceil(g/2) cells beyond the child's coverage
@@ -524,7 +536,7 @@ void dense_ghost_fill(const Hier& H, const BoxData& child, const BoxData& par, s
     for (int k = lo[2]; k < hi[2]; ++k)
       for (int j = lo[1]; j < hi[1]; ++j)
         for (int i = lo[0]; i < hi[0]; ++i) {
-          const double kk[4] = {par.k[0][c].at(i, j, k), par.k[1][c].at(i, j, k), par.k[2][c].at(i, j, k),
+          const real kk[4] = {par.k[0][c].at(i, j, k), par.k[1][c].at(i, j, k), par.k[2][c].at(i, j, k),
                                 par.k[3][c].at(i, j, k)};
           C.at(i, j, k) = dense_stage_any(H.integrator, stage, theta, hp, par.y_old[c].at(i, j, k), kk);
         }
@@ -546,11 +558,11 @@ void restrict_to_parent(const Hier& H, const BoxData& child, BoxData& par) {
     for (int K = 0; K < nc[2]; ++K)
       for (int J = 0; J < nc[1]; ++J)
         for (int I = 0; I < nc[0]; ++I) {
-          double sz = 0.0;
+          real sz = 0.0;
           for (int cc = 0; cc < P.nr; ++cc) {
-            double sy = 0.0;
+            real sy = 0.0;
             for (int bb = 0; bb < P.nr; ++bb) {
-              double sx = 0.0;
+              real sx = 0.0;
               for (int a = 0; a < P.nr; ++a)
                 sx += P.r[a] * yc.at(2 * I + P.rmin + a, 2 * J + P.rmin + bb, 2 * K + P.rmin + cc);
               sy += P.r[bb] * sx;
@@ -594,7 +606,7 @@ void sibling_exchange(Hier& H, int level, std::vector<Field> BoxData::*which) {
 // ---------------------------------------------------------------------------------------------
 // time stepping
 // ---------------------------------------------------------------------------------------------
-void axpy_interior(const BoxData& b, std::vector<Field>& out, const std::vector<Field>& y0, double a,
+void axpy_interior(const BoxData& b, std::vector<Field>& out, const std::vector<Field>& y0, real a,
                    const std::vector<Field>& kk) {
   for (size_t c = 0; c < out.size(); ++c) {
 #pragma omp parallel for schedule(static)
@@ -604,7 +616,7 @@ void axpy_interior(const BoxData& b, std::vector<Field>& out, const std::vector<
   }
 }
 
-void fill(Hier& H, int level, std::vector<Field> BoxData::*which, int stage, double theta, double dt) {
+void fill(Hier& H, int level, std::vector<Field> BoxData::*which, int stage, real theta, real dt) {
   for (int ib : H.level_boxes[level]) {
     BoxData& b = H.boxes[ib];
     if (level == 0) { if (H.outer_bc == 0) periodic_fill(b, b.*which); }  // radiative: no ghosts, boundary points evolve
@@ -615,9 +627,9 @@ void fill(Hier& H, int level, std::vector<Field> BoxData::*which, int stage, dou
 
 // Stage vector Y_{s+1} from y_n and the slopes so far, and the final update, on the interior of one box, for the
 // integrator in use: RK4 eqs (5), (7)-(9); RK3 / RK2 the tableaux of reading S28 (see b_coeff_rk3).
-void next_stage_vector(const Hier& H, BoxData& b, int s, double dt) {
+void next_stage_vector(const Hier& H, BoxData& b, int s, real dt) {
   if (H.integrator == 4) {
-    const double a_s[3] = {0.5, 0.5, 1.0};
+    const real a_s[3] = {0.5, 0.5, 1.0};
     axpy_interior(b, b.Y, b.y_old, a_s[s - 1] * dt, b.k[s - 1]);  // eqs (7)-(9)
     return;
   }
@@ -630,7 +642,7 @@ void next_stage_vector(const Hier& H, BoxData& b, int s, double dt) {
           b.Y[c].at(i, j, k) = b.y_old[c].at(i, j, k) + dt * (-b.k[0][c].at(i, j, k) + 2.0 * b.k[1][c].at(i, j, k));
   }
 }
-void final_update(const Hier& H, BoxData& b, double dt) {
+void final_update(const Hier& H, BoxData& b, real dt) {
   for (int c = 0; c < 2 * H.F; ++c) {
 #pragma omp parallel for schedule(static)
     for (int k = 0; k < b.n[2]; ++k)
@@ -651,7 +663,7 @@ void final_update(const Hier& H, BoxData& b, double dt) {
 
 // One RK step of all boxes of one level (RK4: eqs 1-9), ghosts by fill(); theta = where this step starts
 // inside the parent's step (0 or 1/2; ignored on level 0).
-void rk4_level_step(Hier& H, int level, double dt, double theta) {
+void rk4_level_step(Hier& H, int level, real dt, real theta) {
   const int S = H.integrator;  // number of stages: RK4 4, RK3 3, RK2 2
   for (int ib : H.level_boxes[level]) {
     BoxData& b = H.boxes[ib];
@@ -673,7 +685,7 @@ void rk4_level_step(Hier& H, int level, double dt, double theta) {
 }
 
 // Steps 1-7.
-void advance(Hier& H, int level, double dt, double theta) {
+void advance(Hier& H, int level, real dt, real theta) {
   rk4_level_step(H, level, dt, theta);
   if (level + 1 < H.nlevels) {
     advance(H, level + 1, 0.5 * dt, 0.0);
@@ -694,7 +706,7 @@ void same_time_fill(Hier& H, int level, std::vector<Field> BoxData::*which) {
   sibling_exchange(H, level, which);
 }
 
-void uniform_step(Hier& H, double dt) {
+void uniform_step(Hier& H, real dt) {
   const int L = H.nlevels, S = H.integrator;
   for (BoxData& b : H.boxes) b.y_old = b.y;
   for (int l = 0; l < L; ++l) same_time_fill(H, l, &BoxData::y_old);
@@ -788,10 +800,21 @@ int oc_max_threads() {
 // unit-level entry points used by the pins
 double oc_b(int i, int m, double theta) { return b_coeff(i, m, theta); }
 double oc_dense_stage(int stage, double theta, double hp, double y_old, const double* k4) {
-  return dense_stage(stage, theta, hp, y_old, k4);
+  const real k[4] = {k4[0], k4[1], k4[2], k4[3]};
+  return dense_stage(stage, theta, hp, y_old, k);
 }
-void oc_prolong_weights(int parity, double* w5) { prolong_weights(parity, w5); }
-void oc_restrict_weights(double* r6) { restrict_weights(r6); }
+void oc_prolong_weights(int parity, double* w5) {
+  real w[5];
+  prolong_weights(parity, w);
+  for (int m = 0; m < 5; ++m) w5[m] = double(w[m]);
+}
+void oc_restrict_weights(double* r6) {
+  real r[6];
+  restrict_weights(r);
+  for (int m = 0; m < 6; ++m) r6[m] = double(r[m]);
+}
+// sizeof of the arithmetic type of this build (8: the fp64 oracle; 16: the long double reference of DESIGN.md S27)
+int oc_real_bytes() { return int(sizeof(real)); }
 
 void* oc_create(int nlevels, int nboxes, const int* box_level, const int* box_lo, const int* box_n, int ghost,
                 int nfields, const int* domain_cells, const double* xlo, const double* xhi,
@@ -894,7 +917,10 @@ double oc_b_rk(int integrator, int i, int m, double theta) {
   return integrator == 3 ? b_coeff_rk3(i, m, theta) : (integrator == 2 ? b_coeff_rk2(i, m, theta) : b_coeff(i, m, theta));
 }
 double oc_dense_stage_rk(int integrator, int stage, double theta, double hp, double y_old, const double* k) {
-  return dense_stage_any(integrator, stage, theta, hp, y_old, k);
+  const int nk = integrator == 2 ? 2 : 4;  // slopes the formulas of this integrator read (RK3: k_1..k_3 and k_4 = f(y_{n+1}))
+  real kr[4] = {0, 0, 0, 0};
+  for (int s = 0; s < nk; ++s) kr[s] = k[s];
+  return dense_stage_any(integrator, stage, theta, hp, y_old, kr);
 }
 
 int oc_set_state(void* h, int level, int box, int comp, const double* src) {

@@ -38,7 +38,8 @@ def u_scale(O, w) -> float:
 
 
 def rho_scale(O, w) -> float:
-    """max|rho| over the rho components (comp >= nfields); never below max|u| * 1e-3 (rho = 0 initial data)."""
+    """max|rho| over the rho components (comp >= nfields), from the oracle. May be 0 (rho = 0 initial data, no step
+    taken): compare_state uses max(rho_scale, u_scale)."""
     s = 0.0
     for l in range(w.nlevels):
         for ib in range(len(w.level_boxes(l))):

@@ -294,6 +294,17 @@ def cfg5(n: int = 256, nlevels: int = 6) -> Workload:
                     init=gaussian_init(2 * 0.05 ** 2))
 
 
+def cfg5_spacings(n: int = 64, nlevels: int = 6) -> Workload:
+    """cfg 5's finest grid spacing (2 / 8192) and its spacing ratio between levels, on `nlevels` nested n^3 boxes: the
+    domain shrinks instead of the resolution. With nlevels = 6 every level has cfg 5's dx and dt and the finest level
+    cfg 5's 128 RHS evaluations per coarse step — the rounding behaviour of the full configuration at a size the oracle
+    steps in seconds (S27). The pulse is cfg 5's (periodic images overlap a little at the small domain's
+    edge: irrelevant to what this input is for)."""
+    half = n * 2.0 ** (nlevels - 1) / 8192.0
+    return Workload(f"cfg5 spacings (dx_finest = 2/8192), {nlevels} levels x {n}^3", nested_cubes(nlevels, n), (n, n, n),
+                    xlo=(-half,) * 3, xhi=(half,) * 3, coarse_steps=1, init=gaussian_init(2 * 0.05 ** 2))
+
+
 def ragged_small() -> Workload:
     """Test-only: non-cubic, odd-tile sizes, off-centre child, two grandchildren; F = 2 with coupling."""
     boxes = [Box(0, (0, 0, 0), (40, 24, 28)),

@@ -41,8 +41,12 @@ r, w = dist.get_rank(), dist.get_world_size()
 local_ms = 10.0 + 5.0 * r                      # rank 1 is the slow replica
 ms = bench.max_over_ranks(local_ms, dist, "cpu")
 v = bench.whole_job_value(w, 1000.0, 4, ms * 1e-3)
+for turn in range(w):                          # one rank prints at a time: two ranks writing to the one pipe at the
+    dist.barrier()                             # same moment can interleave within a line
+    if turn == r:
+        sys.stdout.write(json.dumps({{"rank": r, "world": w, "ms": ms, "value": v}}) + "\n")
+        sys.stdout.flush()
 dist.barrier()
-print(json.dumps({{"rank": r, "world": w, "ms": ms, "value": v}}), flush=True)
 dist.destroy_process_group()
 """
 
