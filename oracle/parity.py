@@ -16,9 +16,11 @@ F is the rounding floor of the DEFINITION, not an allowance for the kernels: one
 terms of size 30 |u| / (12 dx^2), so rho = d_t u is rounded by eps * 2.5 |u| dt / dx^2 = eps * 0.625 |u| / dx per
 evaluation (dt = dx / 4), and the finest of L levels is evaluated 4 * 2^(L-1) times per coarse step. For shallow
 hierarchies F is nothing (3 levels of 32^3: 7e-14); at cfg 5's depth (dx = 2 / 8192, 128 evaluations) it is 3.5e-11 max|u|,
-above 1e-11 * max|rho| after one step from rho = 0. That the floor is real and not a kernel defect is pinned without any
-kernel: the oracle recompiled with contracted multiply-adds (every a*b+c rounded once instead of twice) moves by
-2e-11 max|u| in rho at that depth and by 1e-15 max|u| in u (tests/test_oracle_scheme.py::test_rounding_floor_of_the_oracle).
+above 1e-11 * max|rho| after one step from rho = 0. That the floor is real and not a kernel defect is MEASURED at that
+depth without any kernel (tests/test_oracle_scheme.py::test_rounding_floor_of_the_oracle, DESIGN.md S27): on six levels with
+cfg 5's dx and dt the fp64 oracle lies 7.0e-12 max|u| in rho (7e-16 in u) from the oracle built in long double, and its
+plain and FMA-contracted fp64 builds lie 9.3e-12 max|u| apart. F covers the measured distance five times. How close the
+CUDA path is to that long double value is tests/test_gpu_truth.py (2.0-2.4e-11 at cfg 5's depth; GPU - oracle = 0.67 F).
 """
 from __future__ import annotations
 

@@ -73,6 +73,7 @@ struct sc_hierarchy {
   std::vector<TMap> tmaps;        // per box: CUtensorMap over all arrays of the box (stage-kernel tile)
   std::vector<TMap> rmaps;        // per box: same tensor, box = the restriction kernel's fine-plane pair
   std::vector<char> tmap_ok;
+  std::vector<char> tile_variant; // per box: stage tile (stage_tile_variant) chosen at creation; maps and launches both use it
   struct GMaps { TMap m[3]; };
   std::vector<GMaps> gmaps;       // per box: ghost-fill footprint maps of the box as PARENT (thin axis x, y, z)
   std::vector<char> gmap_ok;
@@ -220,7 +221,7 @@ void prof_end(sc_hierarchy* h) {
   cudaEventRecord(h->prof.back().e1, h->stream);
 }
 
-// ---- one launch per (level, kernel): all boxes of the level -------------------------------------------
+// ---- per (level, kernel): a loop over the boxes of the level, ONE LAUNCH PER BOX ---------------------------
 void stage_level(Seq& q, int level, int mode, double dt) {
   sc_hierarchy* h = q.h;
   const Layout& L = h->L;
@@ -250,6 +251,7 @@ void stage_level(Seq& q, int level, int mode, double dt) {
     a.A_host = a.A ? h->coupling_host.data() : nullptr;
     a.S = a.A ? h->arr(ib, L.a_scratch()) : nullptr;
     a.tmap = h->tmap_ok[ib] ? h->tmaps[ib].bytes : nullptr;
+    a.tile_variant = h->tile_variant[ib];
     prof_begin(h, KIND_STAGE, stage_bytes(a.b, L.F, mode, a.write_Y4r));
     q.n += launch_stage(a, h->stream);
     prof_end(h);
@@ -455,6 +457,7 @@ void stage_ko_level(Seq& q, int level, int s, double dt) {
     a.rad_nb = (level == 0 && L.outer_bc == 1) ? L.g : 0;
     a.A = h->coupling();
     a.tmap = h->kmap_ok[ib] ? h->kmaps[ib].bytes : nullptr;
+    a.tile_variant = h->tile_variant[ib];
     a.a_Yu = in_u;
     a.a_Yr = in_r;
     // reads: Y_s (2 arrays); + y_n (2) for s >= 2; + the earlier stage vectors of the final combine.  writes: 2 (+ 2 per kept slope)
@@ -907,6 +910,7 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   }
   h->tmaps.resize(h->L.boxes.size());
   h->tmap_ok.assign(h->L.boxes.size(), 0);
+  h->tile_variant.assign(h->L.boxes.size(), 0);
   h->rmaps.resize(h->L.boxes.size());
   h->gmaps.resize(h->L.boxes.size());
   h->kmaps.resize(h->L.boxes.size());
@@ -914,12 +918,14 @@ int32_t sc_create_hierarchy(const sc_hierarchy_desc* desc, sc_hierarchy** out) {
   h->gmap_ok.assign(h->L.boxes.size(), 0);
   for (size_t ib = 0; ib < h->L.boxes.size(); ++ib) {
     const BoxInfo& b = h->L.boxes[ib];
-    h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), stage_tile_variant(b.v, h->L.F) ? 8 : 0, h->tmaps[ib].bytes) &&
+    // decided here, once, with the hierarchy's device current (the choice reads its SM count); ADVICE r2
+    h->tile_variant[ib] = (char)stage_tile_variant(b.v, h->L.F);
+    h->tmap_ok[ib] = make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), h->tile_variant[ib] ? 8 : 0, h->tmaps[ib].bytes) &&
                      make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), 1, h->rmaps[ib].bytes);
     {  // the general path's stage tile: halo 3 (4th-order differences), 4 (8th order) or 5 (with delta^10)
       const Layout& L = h->L;
       const bool ko9 = L.ko_sigma > 0.0 && L.ko_order == 9;
-      const int kind = L.fd_order == 8 ? (ko9 ? 7 : 6) : (stage_tile_variant(b.v, L.F) ? 9 : 5);
+      const int kind = L.fd_order == 8 ? (ko9 ? 7 : 6) : (h->tile_variant[ib] ? 9 : 5);
       const int need = kind == 7 ? 5 : (kind == 6 ? 4 : 3);  // kinds 5, 9: halo 3
       h->kmap_ok[ib] = L.general() && (L.fd_order == 8 || !ko9) && L.g >= need &&
                        make_box_tensor_map(b.v, b.narrays, h->arr((int)ib, 0), kind, h->kmaps[ib].bytes);

@@ -43,6 +43,8 @@ struct StageArgs {
   double* S;           // coupled systems: 2F scratch arrays for the coupling terms (A W) of the two operands
   // TMA path: tensor map of the box (all arrays as the 4th dimension) and the array indices of the roles
   const void* tmap;    // host pointer to the box's CUtensorMap, or null -> direct-load kernel
+  int tile_variant;    // halo tile the map was built for (0: 32 x 16, 1: 64 x 7), decided ONCE at sc_create_hierarchy on the
+                       // device the hierarchy lives on: the launch must use this, never re-derive it from the current device
   int a_yn, a_Y2r, a_Y3r;
 };
 int launch_stage(const StageArgs& a, cudaStream_t st);  // returns the number of kernels launched
@@ -74,6 +76,7 @@ struct StageKOArgs {
   int integrator;        // 4 | 3 | 2
   int fd_order;          // 4 | 8
   int ko_order;          // 0: no dissipation (ko_sigma = 0); 5: delta^6; 9: delta^10
+  int tile_variant;      // as StageArgs::tile_variant (tensor map kind 5 / 9), fixed at creation
   const double* Yu;      // u- and rho-part of the stage vector Y_s (stage 1: the state y_n), read with ghost layers
   const double* Yr;
   const double* yn_u;    // y_n, centre only

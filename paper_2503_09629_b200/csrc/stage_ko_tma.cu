@@ -305,7 +305,7 @@ static void launch_ko_zmarch_t(const StageKOArgs& a, const KoParams& p0, cudaStr
 }
 template <int FINAL>
 static void launch_ko_zmarch(const StageKOArgs& a, const KoParams& p0, cudaStream_t st) {
-  if (stage_tile_variant(a.b, a.F)) launch_ko_zmarch_t<FINAL, TileKB>(a, p0, st);
+  if (a.tile_variant) launch_ko_zmarch_t<FINAL, TileKB>(a, p0, st);  // the tile the box's tensor map was built for
   else launch_ko_zmarch_t<FINAL, TileKA>(a, p0, st);
 }
 

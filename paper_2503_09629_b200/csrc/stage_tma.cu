@@ -395,7 +395,7 @@ void launch_zmarch(const StageArgs& a, cudaStream_t st) {
 }
 template <int MODE, bool COUPLED>
 void launch_zmarch_v(const StageArgs& a, cudaStream_t st) {
-  if (stage_tile_variant(a.b, a.F)) launch_zmarch<MODE, COUPLED, TileB>(a, st);
+  if (a.tile_variant) launch_zmarch<MODE, COUPLED, TileB>(a, st);  // the tile the box's tensor map was built for
   else launch_zmarch<MODE, COUPLED, TileA>(a, st);
 }
 

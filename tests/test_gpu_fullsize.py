@@ -101,6 +101,30 @@ def test_cfg5_all_twenty_steps_vs_oracle():
     O.close()
 
 
+def test_cfg5_depth_all_twenty_steps_vs_oracle():
+    """The multi-step deep comparison of the DEFAULT suite: six levels of 64^3 with cfg 5's spacing and time step on
+    every level (wl.cfg5_spacings: 128 finest-level RHS evaluations per coarse step, as cfg 5), all of cfg 5's 20
+    subcycled coarse steps, then every element of every level against the oracle, ghosts included, at the tolerance of
+    oracle/parity.py with nsteps = 20. About a minute of oracle. (The 256^3 run above stays gated.)"""
+    w = wl.cfg5_spacings(64, 6)
+    nsteps = wl.cfg5().coarse_steps
+    from oracle.parity import u_scale
+    G, O = sc.Hierarchy.from_workload(w), oracle.OracleHierarchy.from_workload(w)
+    su0 = u_scale(O, w)
+    for _ in range(nsteps):
+        G.sc_step(w.dt_coarse, True)
+        O.step(w.dt_coarse, True)
+    su = u_scale(O, w)
+    for l in range(w.nlevels):
+        du = float(np.max(np.abs(G.sc_read_level(l, 0, 0) - O.read_level(l, 0, 0))))
+        dr = float(np.max(np.abs(G.sc_read_level(l, 0, 1) - O.read_level(l, 0, 1))))
+        print(f"level {l}: max|du| = {du / su:.2e}, max|drho| = {dr / su:.2e} (units of max|u| = {su:.3f}; {su0:.3f} at t = 0)")
+    rel = compare_state(G, O, w, padded=True, what="cfg 5 spacings, 20 subcycled steps", nsteps=nsteps, floor_scale=su0)
+    print(f"cfg 5 spacings 6 x 64^3, {nsteps} steps: worst difference = {rel:.2e} of its bound's scale")
+    G.close()
+    O.close()
+
+
 def test_cfg4_full_depth_vs_oracle():
     """BASELINE config 4 exactly as stated (7 levels x 96^3, the finest = two 80x96x96 boxes, 22 coupled fields),
     one subcycled coarse step against the oracle, every element of all 44 components, ghosts included."""

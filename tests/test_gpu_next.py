@@ -21,7 +21,7 @@ def _run_pair(w, sub, steps=None):
     for _ in range(n):
         G.sc_step(w.dt_coarse, sub)
         O.step(w.dt_coarse, sub)
-    rel = compare_state(G, O, w, what=f"{w.name} sub={sub}", nsteps=n)
+    rel = compare_state(G, O, w, what=f"{w.name} sub={sub}")  # nsteps = 1: the strictest floors (shallow hierarchies: F is nothing)
     G.close()
     return rel
 
